@@ -1,0 +1,174 @@
+"""CPU oracle for the k-shell rasterise-and-composite path -- TEST INFRASTRUCTURE ONLY.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this package.  It shares no code with the CUDA path (paper_2409_02482_b200/csrc, binding.py) and does
+not import it; scenes come from paper_2409_02482_b200.synth, which holds none of the method's
+arithmetic.  The arithmetic lives in oracle/vs_oracle.c (plain C, each function cites the passage it
+follows); this file only marshals numpy arrays through ctypes.
+"""
+from __future__ import annotations
+
+import ctypes as C
+
+import numpy as np
+
+from .build import ensure_built
+
+MISS = 0xFFFFFFFF
+
+
+class _Layer(C.Structure):
+    _fields_ = [("positions", C.c_void_p), ("uvs", C.c_void_p), ("indices", C.c_void_p),
+                ("texture", C.c_void_p), ("num_vertices", C.c_uint32), ("num_triangles", C.c_uint32),
+                ("tex_w", C.c_uint32), ("tex_h", C.c_uint32)]
+
+
+_lib = None
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        L = C.CDLL(ensure_built())
+        L.vso_render.restype = C.c_int
+        L.vso_render.argtypes = [C.POINTER(_Layer), C.c_uint32, C.c_uint32, C.c_int, C.c_void_p,
+                                 C.c_uint32, C.c_uint32, C.c_float, C.c_double, C.c_void_p,
+                                 C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                 C.c_void_p, C.c_int]
+        L.vso_half_to_double.restype = C.c_double
+        L.vso_half_to_double.argtypes = [C.c_uint16]
+        L.vso_sh_basis.argtypes = [C.c_int, C.c_void_p, C.c_void_p]
+        L.vso_sample_bilinear.argtypes = [C.c_void_p, C.c_int, C.c_uint32, C.c_uint32, C.c_uint32,
+                                          C.c_double, C.c_double, C.c_void_p]
+        L.vso_decode_rgba.argtypes = [C.c_uint32, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.vso_blend.argtypes = [C.c_uint32, C.c_void_p, C.c_void_p, C.c_double, C.c_void_p, C.c_void_p]
+        L.vso_transform_vertex.argtypes = [C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p,
+                                           C.c_void_p, C.c_void_p]
+        L.vso_max_threads.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _ptr(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def _dtype_code(tex: np.ndarray) -> int:
+    if tex.dtype == np.float32:
+        return 0
+    if tex.dtype == np.float16:
+        return 1
+    raise TypeError("texture dtype must be float32 or float16")
+
+
+def max_threads() -> int:
+    return int(lib().vso_max_threads())
+
+
+def render_view(layers, sh_degree: int, camera, width: int, height: int, *, near_plane: float = 0.05,
+                t_min: float = 2.0 ** -14, background=(0.0, 0.0, 0.0), num_threads: int = 0,
+                want_qp: bool = False, want_layer_rgba: bool = False, want_layer_uv: bool = False):
+    """Render one view.  `layers`: objects with positions/uvs/indices/texture numpy arrays
+    (outermost first).  Returns dict(rgba [H,W,4] f64, ids [k,H,W] u32, stats [2] u64, ...)."""
+    k = len(layers)
+    n = (sh_degree + 1) ** 2
+    keep = []
+    arr = (_Layer * k)()
+    code = None
+    for i, L in enumerate(layers):
+        pos = np.ascontiguousarray(L.positions, dtype=np.float32)
+        uv = np.ascontiguousarray(L.uvs, dtype=np.float32)
+        idx = np.ascontiguousarray(L.indices, dtype=np.uint32)
+        tex = np.ascontiguousarray(L.texture)
+        c = _dtype_code(tex)
+        if code is None:
+            code = c
+        assert c == code, "all layers must share one texture dtype"
+        assert tex.ndim == 4 and tex.shape[2] == n and tex.shape[3] == 4, tex.shape
+        assert pos.ndim == 2 and pos.shape[1] == 3 and uv.shape == (pos.shape[0], 2)
+        assert idx.ndim == 2 and idx.shape[1] == 3
+        assert idx.size == 0 or int(idx.max()) < pos.shape[0]
+        keep += [pos, uv, idx, tex]
+        arr[i] = _Layer(_ptr(pos), _ptr(uv), _ptr(idx), _ptr(tex), pos.shape[0], idx.shape[0],
+                        tex.shape[1], tex.shape[0])
+    cam = np.ascontiguousarray(camera, dtype=np.float32)
+    assert cam.shape == (16,)
+    bg = np.asarray(background, dtype=np.float64)
+    rgba = np.empty((height, width, 4), dtype=np.float64)
+    ids = np.empty((k, height, width), dtype=np.uint32)
+    qp = np.empty((k, height, width), dtype=np.float32) if want_qp else None
+    lrgba = np.empty((k, height, width, 4), dtype=np.float64) if want_layer_rgba else None
+    luv = np.empty((k, height, width, 2), dtype=np.float64) if want_layer_uv else None
+    stats = np.zeros(2, dtype=np.uint64)
+    rc = lib().vso_render(arr, k, sh_degree, code, _ptr(cam), width, height, near_plane, t_min, _ptr(bg),
+                          _ptr(rgba), _ptr(ids), _ptr(qp) if want_qp else None,
+                          _ptr(lrgba) if want_layer_rgba else None, _ptr(luv) if want_layer_uv else None,
+                          _ptr(stats), num_threads)
+    if rc != 0:
+        raise ValueError("vso_render rejected its arguments (rc=%d)" % rc)
+    out = dict(rgba=rgba, ids=ids, stats=stats)
+    if want_qp:
+        out["qp"] = qp
+    if want_layer_rgba:
+        out["layer_rgba"] = lrgba
+    if want_layer_uv:
+        out["layer_uv"] = luv
+    return out
+
+
+def render_scene(scene, views=None, **kw):
+    """Render the given view indices (default: all) of a synth.Scene; returns a list of dicts."""
+    views = range(len(scene.cameras)) if views is None else views
+    kw.setdefault("near_plane", scene.near_plane)
+    kw.setdefault("t_min", scene.t_min)
+    kw.setdefault("background", scene.background)
+    return [render_view(scene.layers, scene.sh_degree, scene.cameras[v], scene.width, scene.height, **kw)
+            for v in views]
+
+
+# ---- single-function entry points, used by the pins -------------------------------------------
+
+def half_to_double(bits: int) -> float:
+    return float(lib().vso_half_to_double(int(bits)))
+
+
+def sh_basis(degree: int, v) -> np.ndarray:
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    Y = np.zeros(16, dtype=np.float64)
+    lib().vso_sh_basis(degree, _ptr(v), _ptr(Y))
+    return Y[: (degree + 1) ** 2]
+
+
+def sample_bilinear(tex: np.ndarray, u: float, v: float) -> np.ndarray:
+    tex = np.ascontiguousarray(tex)
+    H, W, n, _ = tex.shape
+    out = np.empty((n, 4), dtype=np.float64)
+    lib().vso_sample_bilinear(_ptr(tex), _dtype_code(tex), W, H, n, float(u), float(v), _ptr(out))
+    return out
+
+
+def decode_rgba(coef: np.ndarray, Y: np.ndarray) -> np.ndarray:
+    coef = np.ascontiguousarray(coef, dtype=np.float64)
+    Y = np.ascontiguousarray(Y, dtype=np.float64)
+    out = np.empty(4, dtype=np.float64)
+    lib().vso_decode_rgba(coef.shape[0], _ptr(coef), _ptr(Y), _ptr(out))
+    return out
+
+
+def blend(layer_rgba, hit=None, t_min: float = 0.0, background=(0.0, 0.0, 0.0)) -> np.ndarray:
+    layer_rgba = np.ascontiguousarray(layer_rgba, dtype=np.float64)
+    k = layer_rgba.shape[0]
+    hit = np.ones(k, dtype=np.int32) if hit is None else np.ascontiguousarray(hit, dtype=np.int32)
+    bg = np.asarray(background, dtype=np.float64)
+    out = np.empty(4, dtype=np.float64)
+    lib().vso_blend(k, _ptr(layer_rgba), _ptr(hit), float(t_min), _ptr(bg), _ptr(out))
+    return out
+
+
+def transform_vertex(camera, near_plane: float, p):
+    cam = np.ascontiguousarray(camera, dtype=np.float32)
+    p = np.ascontiguousarray(p, dtype=np.float32)
+    X, Y, bad = C.c_int32(), C.c_int32(), C.c_int32()
+    q = C.c_float()
+    lib().vso_transform_vertex(_ptr(cam), near_plane, _ptr(p), C.byref(X), C.byref(Y), C.byref(q), C.byref(bad))
+    return X.value, Y.value, q.value, bad.value
