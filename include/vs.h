@@ -1,0 +1,163 @@
+/*
+ * vs.h -- C ABI of the B200-native k-shell renderer for "Volumetric Surfaces" (arXiv 2409.02482).
+ *
+ * The library renders the paper's baked representation: k (1..9; the paper uses 3 <= k <= 9,
+ * PAPER.md:L10) semi-transparent, UV-textured mesh shells, "rendered in fixed layer order from
+ * outermost to innermost" with no sorting.  Per pixel and per
+ * layer it finds the nearest fragment of that layer ("only sampling the first intersection with
+ * each surface", PAPER.md:L101 Fig. "sampling" c), interpolates UV, fetches the layer's texture of
+ * spherical-harmonics coefficients bilinearly at texel centres (§4.5),
+ * decodes RGBA with the view direction (§4.5; view-dependent opacity L58, L118) and
+ * blends the layers front to back in that fixed order (§4.2 "Surface Blending";
+ * "rasterizes all meshes in a fixed order and blends them in the final frame buffer", L464).
+ * The exact arithmetic (projection op order, 24.8 snapping, top-left rule, depth key, tie-break,
+ * texel addressing, SH convention, activation, blend) is DESIGN.md §3; the readings of the paper it
+ * rests on are DESIGN.md §5.
+ *
+ * Everything runs in hand-written CUDA kernels for sm_100a on ONE GPU (the current device of the
+ * calling thread at vs_scene_create time).  There is no CPU fallback: without a usable CUDA device
+ * every entry point returns VS_ERR_CUDA.
+ *
+ * Conventions
+ *   - Plain C99, no torch / C++ types.  "DEVICE" = pointer to memory of the scene's GPU,
+ *     "HOST" = ordinary host memory (pageable or pinned).
+ *   - Every function returns a vs_status and never throws or aborts across the ABI.  On error
+ *     nothing has been written to the outputs, *out_scene is NULL, and vs_last_error() describes
+ *     the failure (thread-local string, valid until the next call on that thread).
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ */
+#ifndef VS_H_
+#define VS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct vs_scene vs_scene; /* opaque */
+
+typedef enum {
+    VS_OK = 0,
+    VS_ERR_INVALID_ARG = 1,   /* NULL pointer, k outside 1..9, degree > 3, zero size, index >= num_vertices,
+                                 non-finite vertex / camera, near_plane <= 0, reserved flag bits set */
+    VS_ERR_OUT_OF_MEMORY = 2, /* a device or host allocation failed */
+    VS_ERR_CUDA = 3,          /* no device, or a CUDA call / kernel failed; see vs_last_error() */
+    VS_ERR_UNSUPPORTED = 4    /* e.g. image larger than 16384 px on a side, texture larger than 32768 */
+} vs_status;
+
+typedef enum { VS_F32 = 0, VS_F16 = 1 } vs_dtype;           /* texture element type (IEEE binary32/16) */
+typedef enum { VS_MEM_DEVICE = 0, VS_MEM_HOST = 1 } vs_memory; /* where a descriptor's arrays live */
+
+/* One shell ("Mesh baking": a lightweight UV-mapped triangle mesh per surface;
+ * §4.5: per mesh, (deg+1)^2 RGBA coefficient images -- here one interleaved array). */
+typedef struct {
+    const float*    positions;     /* [num_vertices][3] world space, finite                              */
+    const float*    uvs;           /* [num_vertices][2]; seams = duplicated vertices; values outside
+                                      [0,1] are legal and clamp to the edge texels                       */
+    uint32_t        num_vertices;
+    const uint32_t* indices;       /* [num_triangles][3]; triangle id = row index; any winding
+                                      (no culling: both orientations rasterise, the nearest wins)         */
+    uint32_t        num_triangles; /* 0 is legal (an empty shell never hits)                             */
+    const void*     texture;       /* [tex_h][tex_w][(deg+1)^2][4]; channel 0-2 = RGB, 3 = opacity;
+                                      raw (pre-sigmoid) SH coefficients, coefficient index c = l*l+l+m;
+                                      row j of memory is v-row j (no flip)                                */
+    uint32_t        tex_w, tex_h;  /* >= 1, <= 32768                                                       */
+} vs_layer_desc;
+
+typedef struct {
+    uint32_t             num_layers; /* 1..9; layers[0] is the OUTERMOST shell                            */
+    uint32_t             sh_degree;  /* 0..3, shared by colour and opacity                                 */
+    vs_dtype             tex_dtype;  /* all layers share one element type                                  */
+    vs_memory            memory;     /* where positions / uvs / indices / texture of ALL layers live      */
+    const vs_layer_desc* layers;     /* HOST array of num_layers descriptors                               */
+} vs_scene_desc;
+
+/* Pinhole camera (the paper gives none).  x_cam = R * x_world + t with
+ * +x right, +y DOWN, +z forward; pixel (i,j) has its centre at (i+0.5, j+0.5), origin top-left. */
+typedef struct {
+    float fx, fy, cx, cy; /* pixels */
+    float R[9];           /* row-major */
+    float t[3];
+} vs_camera;
+
+enum {
+    VS_FLAG_REFERENCE_PATH = 1u << 0 /* debugging aid: brute-force kernel (one thread per pixel, every
+                                        triangle tested), same arithmetic and outputs; small scenes only */
+};
+
+typedef struct {
+    uint32_t width, height;   /* 1..16384                                                                  */
+    float    near_plane;      /* > 0; a triangle with any vertex at depth w < near_plane is DROPPED (not
+                                 clipped), as is one with a vertex projecting outside +-16384 px           */
+    float    t_min;           /* >= 0; compositing stops after the layer that brings the transmittance
+                                 below t_min (0 disables).  Recommended 2^-14 (reading Q15)      */
+    float    background[3];   /* rgb_out = C + T * background ; (0,0,0) => premultiplied colour            */
+    uint32_t flags;           /* VS_FLAG_* ; other bits must be 0                                          */
+    uint32_t views_per_chunk; /* cameras processed per internal pass; 0 = choose automatically             */
+} vs_render_params;
+
+/* Counters of the most recent vs_render / vs_render_host on a scene (summed over its cameras). */
+typedef struct {
+    uint64_t dropped_triangles;    /* near-plane / guard-band drops (0 on all BASELINE.json configs)      */
+    uint64_t degenerate_triangles; /* zero area after snapping                                             */
+    uint64_t tile_refs;            /* (triangle, tile) pairs binned                                        */
+    uint64_t scratch_bytes;        /* peak device scratch of the call                                      */
+} vs_render_stats;
+
+/*
+ * vs_scene_create -- S0: upload / re-lay-out the baked asset once.
+ *   Copies every array (the caller may free or overwrite its inputs as soon as the call returns: the
+ *   function synchronises `cuda_stream` before returning), validates indices and finiteness, and
+ *   converts each texture to the internal texel-interleaved layout.  The scene is
+ *   immutable afterwards.  Device memory held: ~ sum over layers of 16 B/vertex... see DESIGN.md §6.
+ */
+vs_status vs_scene_create(const vs_scene_desc* desc, void* cuda_stream, vs_scene** out_scene);
+
+/*
+ * vs_render -- the hot path, steps S1-S7 of DESIGN.md §1 for a batch of cameras:
+ *   S1 vertex transform + S2 triangle setup, S3 screen-tile binning (count / scan / scatter),
+ *   S4 coverage + per-layer nearest-fragment resolve, S5 perspective-correct UV + bilinear fetch,
+ *   S6 SH evaluation + sigmoid, S7 fixed-order front-to-back compositing.
+ *
+ *   cameras      HOST  [num_cameras]
+ *   out_rgba     DEVICE [num_cameras][height][width][4] float: rgb = C + T*background, a = 1 - T.
+ *                A pixel no layer hits is a value (background, alpha 0), not an error.
+ *   out_tri_ids  DEVICE [num_cameras][num_layers][height][width] uint32 or NULL: id of the nearest
+ *                covering triangle of each layer, 0xFFFFFFFF = miss (the AOV the parity tests read).
+ *
+ *   All kernels are enqueued on `cuda_stream`; outputs are complete once that stream has drained.
+ *   The call may block the host while it sizes scratch from the binning count pass (one small
+ *   device->host read per chunk of cameras) but does not wait for the rendering itself.  Scratch is
+ *   owned by the scene and reused between calls, so calls on one scene must not overlap in time.
+ */
+vs_status vs_render(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
+                    const vs_render_params* params, float* out_rgba, uint32_t* out_tri_ids,
+                    void* cuda_stream);
+
+/*
+ * vs_render_host -- the same call with HOST output buffers (end-to-end path): renders chunk by
+ * chunk into device staging and copies each finished chunk back while the next one renders.
+ *   out_rgba / out_tri_ids  HOST, same shapes as vs_render (pinned memory makes the copies async;
+ *   pageable memory works but serialises).  Returns after everything has landed in the host buffers.
+ */
+vs_status vs_render_host(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
+                         const vs_render_params* params, float* out_rgba, uint32_t* out_tri_ids,
+                         void* cuda_stream);
+
+/* Counters of the last render on this scene; synchronises the stream that render used. */
+vs_status vs_query_last_render(vs_scene* scene, vs_render_stats* out_stats);
+
+/* Frees all device memory of the scene after synchronising the device.  NULL is a no-op. */
+void vs_scene_destroy(vs_scene* scene);
+
+/* Thread-local description of the last error on this thread ("" if none). */
+const char* vs_last_error(void);
+
+/* Library version, e.g. "vs-b200 0.1 (sm_100a)". */
+const char* vs_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* VS_H_ */

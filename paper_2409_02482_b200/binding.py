@@ -1,0 +1,255 @@
+"""Thin ctypes binding of the C-ABI library (include/vs.h): argument marshalling only -- every step
+of the path runs in the CUDA kernels of libvs_b200.so.  PyTorch supplies device memory and streams.
+
+There is no fallback: if the library is missing and cannot be built, or no CUDA device is present,
+the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libvs_b200.so")
+
+VS_OK, VS_ERR_INVALID_ARG, VS_ERR_OUT_OF_MEMORY, VS_ERR_CUDA, VS_ERR_UNSUPPORTED = range(5)
+VS_F32, VS_F16 = 0, 1
+VS_MEM_DEVICE, VS_MEM_HOST = 0, 1
+VS_FLAG_REFERENCE_PATH = 1
+MISS = 0xFFFFFFFF
+
+EXPORTS = ["vs_scene_create", "vs_render", "vs_render_host", "vs_query_last_render", "vs_scene_destroy",
+           "vs_last_error", "vs_version"]
+
+
+class VsError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__("vs status %d: %s" % (status, msg))
+        self.status = status
+
+
+class vs_layer_desc(C.Structure):
+    _fields_ = [("positions", C.c_void_p), ("uvs", C.c_void_p), ("num_vertices", C.c_uint32),
+                ("indices", C.c_void_p), ("num_triangles", C.c_uint32), ("texture", C.c_void_p),
+                ("tex_w", C.c_uint32), ("tex_h", C.c_uint32)]
+
+
+class vs_scene_desc(C.Structure):
+    _fields_ = [("num_layers", C.c_uint32), ("sh_degree", C.c_uint32), ("tex_dtype", C.c_int),
+                ("memory", C.c_int), ("layers", C.POINTER(vs_layer_desc))]
+
+
+class vs_camera(C.Structure):
+    _fields_ = [("fx", C.c_float), ("fy", C.c_float), ("cx", C.c_float), ("cy", C.c_float),
+                ("R", C.c_float * 9), ("t", C.c_float * 3)]
+
+
+class vs_render_params(C.Structure):
+    _fields_ = [("width", C.c_uint32), ("height", C.c_uint32), ("near_plane", C.c_float),
+                ("t_min", C.c_float), ("background", C.c_float * 3), ("flags", C.c_uint32),
+                ("views_per_chunk", C.c_uint32)]
+
+
+class vs_render_stats(C.Structure):
+    _fields_ = [("dropped_triangles", C.c_uint64), ("degenerate_triangles", C.c_uint64),
+                ("tile_refs", C.c_uint64), ("scratch_bytes", C.c_uint64)]
+
+
+_lib = None
+
+
+def load_library(build_if_missing: bool = True):
+    """dlopen libvs_b200.so (building it with nvcc first if it is absent or stale)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build_if_missing:
+        from .build import ensure_built
+        try:
+            ensure_built()
+        except Exception as e:  # no nvcc on this machine: use the shipped .so if there is one
+            if not os.path.exists(LIB_PATH):
+                raise RuntimeError("libvs_b200.so is missing and could not be built: %s" % e)
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError("libvs_b200.so is missing (run `python -m paper_2409_02482_b200.build`)")
+    L = C.CDLL(LIB_PATH)
+    L.vs_scene_create.restype = C.c_int
+    L.vs_scene_create.argtypes = [C.POINTER(vs_scene_desc), C.c_void_p, C.POINTER(C.c_void_p)]
+    for name in ("vs_render", "vs_render_host"):
+        f = getattr(L, name)
+        f.restype = C.c_int
+        f.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(vs_render_params), C.c_void_p,
+                      C.c_void_p, C.c_void_p]
+    L.vs_query_last_render.restype = C.c_int
+    L.vs_query_last_render.argtypes = [C.c_void_p, C.POINTER(vs_render_stats)]
+    L.vs_scene_destroy.restype = None
+    L.vs_scene_destroy.argtypes = [C.c_void_p]
+    L.vs_last_error.restype = C.c_char_p
+    L.vs_version.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _check(status):
+    if status != VS_OK:
+        raise VsError(status, load_library().vs_last_error().decode())
+
+
+def _stream_ptr(stream):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def make_params(width, height, near_plane=0.05, t_min=2.0 ** -14, background=(0.0, 0.0, 0.0), flags=0,
+                views_per_chunk=0):
+    p = vs_render_params()
+    p.width, p.height, p.near_plane, p.t_min = int(width), int(height), float(near_plane), float(t_min)
+    p.background = (C.c_float * 3)(*[float(b) for b in background])
+    p.flags, p.views_per_chunk = int(flags), int(views_per_chunk)
+    return p
+
+
+# ---- the C-ABI calls, same names ---------------------------------------------------------------
+
+def vs_scene_create(layers, sh_degree: int, stream=None) -> int:
+    """`layers`: sequence of objects with .positions [V,3] f32, .uvs [V,2] f32, .indices [T,3]
+    u32/int32, .texture [H,W,n,4] f32|f16 -- all torch CUDA tensors (device pointers) or all numpy
+    arrays (host pointers).  Returns the opaque scene handle."""
+    import torch
+    L = load_library()
+    k = len(layers)
+    arr = (vs_layer_desc * max(k, 1))()
+    keep = []
+    on_host = k > 0 and isinstance(layers[0].positions, np.ndarray)
+    dtype_code = None
+    for i, ly in enumerate(layers):
+        if on_host:
+            pos = np.ascontiguousarray(ly.positions, dtype=np.float32)
+            uv = np.ascontiguousarray(ly.uvs, dtype=np.float32)
+            idx = np.ascontiguousarray(ly.indices, dtype=np.uint32)
+            tex = np.ascontiguousarray(ly.texture)
+            code = {np.dtype(np.float32): VS_F32, np.dtype(np.float16): VS_F16}[tex.dtype]
+            ptr = lambda a: a.ctypes.data
+        else:
+            pos = ly.positions.contiguous()
+            uv = ly.uvs.contiguous()
+            idx = ly.indices.contiguous()
+            tex = ly.texture.contiguous()
+            assert pos.is_cuda and uv.is_cuda and idx.is_cuda and tex.is_cuda
+            assert pos.dtype == torch.float32 and uv.dtype == torch.float32
+            assert idx.dtype in (torch.int32, torch.uint32)
+            code = {torch.float32: VS_F32, torch.float16: VS_F16}[tex.dtype]
+            ptr = lambda a: a.data_ptr()
+        if dtype_code is None:
+            dtype_code = code
+        assert code == dtype_code, "all layers must share one texture dtype"
+        assert tex.ndim == 4 and tex.shape[3] == 4 and tex.shape[2] == (sh_degree + 1) ** 2, tuple(tex.shape)
+        keep += [pos, uv, idx, tex]
+        arr[i] = vs_layer_desc(ptr(pos), ptr(uv), pos.shape[0], ptr(idx), idx.shape[0], ptr(tex),
+                               tex.shape[1], tex.shape[0])
+    desc = vs_scene_desc(k, sh_degree, dtype_code or 0, VS_MEM_HOST if on_host else VS_MEM_DEVICE, arr)
+    handle = C.c_void_p()
+    _check(L.vs_scene_create(C.byref(desc), _stream_ptr(stream), C.byref(handle)))
+    return handle.value
+
+
+def _cams(cameras):
+    cams = np.ascontiguousarray(cameras, dtype=np.float32)
+    assert cams.ndim == 2 and cams.shape[1] == 16
+    return cams
+
+
+def vs_render(scene: int, cameras, params: vs_render_params, out_rgba, out_tri_ids=None, stream=None):
+    """cameras: HOST [B,16] float32; out_rgba: CUDA float32 [B,H,W,4]; out_tri_ids: CUDA int32/uint32
+    [B,k,H,W] or None.  Asynchronous on `stream` (default: torch's current stream)."""
+    cams = _cams(cameras)
+    assert out_rgba.is_cuda and out_rgba.is_contiguous() and out_rgba.numel() == cams.shape[0] * params.width * params.height * 4
+    ids_ptr = None
+    if out_tri_ids is not None:
+        assert out_tri_ids.is_cuda and out_tri_ids.is_contiguous() and out_tri_ids.element_size() == 4
+        ids_ptr = out_tri_ids.data_ptr()
+    _check(load_library().vs_render(scene, cams.ctypes.data, cams.shape[0], C.byref(params),
+                                    out_rgba.data_ptr(), ids_ptr, _stream_ptr(stream)))
+
+
+def vs_render_host(scene: int, cameras, params: vs_render_params, out_rgba, out_tri_ids=None, stream=None):
+    """Same, with HOST outputs (numpy arrays or CPU torch tensors, pinned for async copies).  Blocks
+    until the images are in the host buffers."""
+    cams = _cams(cameras)
+
+    def host_ptr(a):
+        return a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr()
+
+    _check(load_library().vs_render_host(scene, cams.ctypes.data, cams.shape[0], C.byref(params),
+                                         host_ptr(out_rgba), host_ptr(out_tri_ids) if out_tri_ids is not None else None,
+                                         _stream_ptr(stream)))
+
+
+def vs_query_last_render(scene: int) -> dict:
+    st = vs_render_stats()
+    _check(load_library().vs_query_last_render(scene, C.byref(st)))
+    return {f: int(getattr(st, f)) for f, _ in vs_render_stats._fields_}
+
+
+def vs_scene_destroy(scene: int):
+    if scene:
+        load_library().vs_scene_destroy(scene)
+
+
+def vs_version() -> str:
+    return load_library().vs_version().decode()
+
+
+# ---- convenience -----------------------------------------------------------------------------------
+
+class Renderer:
+    """Owns a scene handle built from a synth.Scene-like object (numpy arrays are uploaded through
+    torch so that the descriptor carries device pointers)."""
+
+    def __init__(self, scene, device="cuda:0"):
+        import torch
+        import types
+        self.k = len(scene.layers)
+        self.sh_degree = scene.sh_degree
+        self.device = torch.device(device)
+        with torch.cuda.device(self.device):
+            self.handle = None
+            layers = []
+            for ly in scene.layers:
+                layers.append(types.SimpleNamespace(
+                    positions=torch.from_numpy(np.ascontiguousarray(ly.positions, dtype=np.float32)).to(self.device),
+                    uvs=torch.from_numpy(np.ascontiguousarray(ly.uvs, dtype=np.float32)).to(self.device),
+                    indices=torch.from_numpy(np.ascontiguousarray(ly.indices, dtype=np.uint32).view(np.int32)).to(self.device),
+                    texture=torch.from_numpy(np.ascontiguousarray(ly.texture)).to(self.device)))
+            self.handle = vs_scene_create(layers, scene.sh_degree)
+            del layers
+            torch.cuda.empty_cache()
+
+    def render(self, cameras, params, want_ids=False, out_rgba=None, out_ids=None):
+        import torch
+        B = len(cameras)
+        with torch.cuda.device(self.device):
+            if out_rgba is None:
+                out_rgba = torch.empty((B, params.height, params.width, 4), dtype=torch.float32, device=self.device)
+            if want_ids and out_ids is None:
+                out_ids = torch.empty((B, self.k, params.height, params.width), dtype=torch.int32, device=self.device)
+            vs_render(self.handle, cameras, params, out_rgba, out_ids)
+        return out_rgba, out_ids
+
+    def stats(self):
+        return vs_query_last_render(self.handle)
+
+    def close(self):
+        if self.handle:
+            vs_scene_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

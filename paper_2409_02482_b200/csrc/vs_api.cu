@@ -1,0 +1,382 @@
+// vs_api.cu -- the C-ABI of include/vs.h: argument validation, scene upload, scratch management and
+// the per-chunk launch sequence S1..S7.  No arithmetic of the method lives here.
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/vs.h"
+#include "vs_common.cuh"
+
+static thread_local char g_err[512] = "";
+
+static vs_status fail(vs_status s, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return s;
+}
+
+#define CU(call)                                                                                         \
+    do {                                                                                                 \
+        cudaError_t e_ = (call);                                                                         \
+        if (e_ != cudaSuccess)                                                                           \
+            return fail(e_ == cudaErrorMemoryAllocation ? VS_ERR_OUT_OF_MEMORY : VS_ERR_CUDA, "%s: %s", #call, \
+                        cudaGetErrorString(e_));                                                         \
+    } while (0)
+
+struct DevBuf {
+    void* p = nullptr;
+    size_t cap = 0;
+    cudaError_t reserve(size_t bytes)
+    {
+        if (bytes <= cap) return cudaSuccess;
+        if (p) cudaFree(p);
+        p = nullptr; cap = 0;
+        size_t want = bytes + bytes / 8;
+        cudaError_t e = cudaMalloc(&p, want);
+        if (e != cudaSuccess) { e = cudaMalloc(&p, bytes); want = bytes; }
+        if (e == cudaSuccess) cap = want; else p = nullptr;
+        return e;
+    }
+    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+};
+
+struct vs_scene {
+    int device = 0;
+    VsSceneDev dev{};
+    int tex_f16 = 0;
+    std::vector<void*> owned;
+    // scratch, reused between calls
+    DevBuf cams, vtx, tile_count, tile_off, tile_cursor, tile_tris, counters, stage_rgba[2], stage_ids[2];
+    uint32_t* host_total = nullptr;  // pinned
+    cudaStream_t last_stream = nullptr;
+    cudaStream_t copy_stream = nullptr;
+    cudaEvent_t ev_render[2] = {nullptr, nullptr}, ev_copy[2] = {nullptr, nullptr};
+    size_t scratch_peak = 0;
+    ~vs_scene()
+    {
+        for (void* p : owned) cudaFree(p);
+        DevBuf* bufs[] = {&cams, &vtx, &tile_count, &tile_off, &tile_cursor, &tile_tris, &counters,
+                          &stage_rgba[0], &stage_rgba[1], &stage_ids[0], &stage_ids[1]};
+        for (DevBuf* b : bufs) b->release();
+        if (host_total) cudaFreeHost(host_total);
+        if (copy_stream) cudaStreamDestroy(copy_stream);
+        for (int i = 0; i < 2; ++i) {
+            if (ev_render[i]) cudaEventDestroy(ev_render[i]);
+            if (ev_copy[i]) cudaEventDestroy(ev_copy[i]);
+        }
+    }
+};
+
+extern "C" const char* vs_last_error(void) { return g_err; }
+extern "C" const char* vs_version(void) { return "vs-b200 0.1 (sm_100a)"; }
+
+extern "C" void vs_scene_destroy(vs_scene* scene)
+{
+    if (!scene) return;
+    cudaSetDevice(scene->device);
+    cudaDeviceSynchronize();
+    delete scene;
+}
+
+static vs_status dev_alloc(vs_scene* s, void** p, size_t bytes)
+{
+    CU(cudaMalloc(p, bytes ? bytes : 16));
+    s->owned.push_back(*p);
+    return VS_OK;
+}
+
+// Copy `bytes` from a descriptor array (device or host) to fresh device staging if needed.
+static vs_status stage_in(const void* src, size_t bytes, vs_memory mem, cudaStream_t st, std::vector<void*>& temps,
+                          const void** out)
+{
+    if (mem == VS_MEM_DEVICE || bytes == 0) { *out = src; return VS_OK; }
+    void* d = nullptr;
+    CU(cudaMalloc(&d, bytes));
+    temps.push_back(d);
+    CU(cudaMemcpyAsync(d, src, bytes, cudaMemcpyHostToDevice, st));
+    *out = d;
+    return VS_OK;
+}
+
+static vs_status scene_create_impl(const vs_scene_desc* desc, cudaStream_t st, vs_scene* s, std::vector<void*>& temps)
+{
+    const uint32_t k = desc->num_layers;
+    const uint32_t n = (desc->sh_degree + 1) * (desc->sh_degree + 1);
+    const int f16 = desc->tex_dtype == VS_F16;
+    const uint32_t cpv = f16 ? 2 : 1;
+    VsSceneDev& d = s->dev;
+    d.k = k; d.sh_degree = desc->sh_degree; d.n_coef = n; d.texel_vecs = (n + cpv - 1) / cpv;
+    s->tex_f16 = f16;
+    uint64_t vt = 0, tt = 0;
+    for (uint32_t l = 0; l < k; ++l) {
+        const vs_layer_desc& L = desc->layers[l];
+        if (L.num_vertices == 0 && L.num_triangles != 0) return fail(VS_ERR_INVALID_ARG, "layer %u: triangles but no vertices", l);
+        if ((L.num_vertices && (!L.positions || !L.uvs)) || (L.num_triangles && !L.indices) || !L.texture)
+            return fail(VS_ERR_INVALID_ARG, "layer %u: NULL array", l);
+        if (L.tex_w == 0 || L.tex_h == 0) return fail(VS_ERR_INVALID_ARG, "layer %u: empty texture", l);
+        if (L.tex_w > 32768 || L.tex_h > 32768 || (uint64_t)L.tex_w * L.tex_h * d.texel_vecs >= (1ull << 32))
+            return fail(VS_ERR_UNSUPPORTED, "layer %u: texture %ux%u too large", l, L.tex_w, L.tex_h);
+        d.tri_off[l] = (uint32_t)tt;
+        vt += L.num_vertices; tt += L.num_triangles;
+        if (vt >= (1ull << 31) || tt >= (1ull << 31)) return fail(VS_ERR_UNSUPPORTED, "scene too large");
+    }
+    for (uint32_t l = k; l <= VS_MAX_LAYERS; ++l) d.tri_off[l] = (uint32_t)tt;
+    d.v_total = (uint32_t)vt; d.t_total = (uint32_t)tt;
+
+    float* pos; float2* uvs; uint4* tris; uint32_t* flag;
+    vs_status r;
+    if ((r = dev_alloc(s, (void**)&pos, vt * 12)) != VS_OK) return r;
+    if ((r = dev_alloc(s, (void**)&uvs, vt * 8)) != VS_OK) return r;
+    if ((r = dev_alloc(s, (void**)&tris, tt * 16)) != VS_OK) return r;
+    if ((r = dev_alloc(s, (void**)&flag, 16)) != VS_OK) return r;
+    CU(cudaMemsetAsync(flag, 0, 16, st));
+    uint64_t voff = 0;
+    const cudaMemcpyKind kind = desc->memory == VS_MEM_HOST ? cudaMemcpyHostToDevice : cudaMemcpyDeviceToDevice;
+    for (uint32_t l = 0; l < k; ++l) {
+        const vs_layer_desc& L = desc->layers[l];
+        if (L.num_vertices) {
+            CU(cudaMemcpyAsync(pos + 3 * voff, L.positions, (size_t)L.num_vertices * 12, kind, st));
+            CU(cudaMemcpyAsync(uvs + voff, L.uvs, (size_t)L.num_vertices * 8, kind, st));
+        }
+        const void* idx = nullptr;
+        if ((r = stage_in(L.indices, (size_t)L.num_triangles * 12, desc->memory, st, temps, &idx)) != VS_OK) return r;
+        CU(vs_launch_pack_tris((const uint32_t*)idx, L.num_triangles, L.num_vertices, (uint32_t)voff, l,
+                               tris + d.tri_off[l], flag, st));
+        // texture -> internal layout (same element order, texel padded to a multiple of 16 bytes)
+        const size_t texels = (size_t)L.tex_w * L.tex_h;
+        const size_t src_bytes = texels * n * 4 * (f16 ? 2 : 4);
+        uint4* tex;
+        if ((r = dev_alloc(s, (void**)&tex, texels * d.texel_vecs * 16)) != VS_OK) return r;
+        if (d.texel_vecs * 16 == n * 4 * (f16 ? 2u : 4u)) {
+            CU(cudaMemcpyAsync(tex, L.texture, src_bytes, kind, st));
+        } else {
+            const void* tsrc = nullptr;
+            if ((r = stage_in(L.texture, src_bytes, desc->memory, st, temps, &tsrc)) != VS_OK) return r;
+            CU(vs_launch_pack_texture(tsrc, f16, (uint32_t)texels, n, d.texel_vecs, tex, st));
+        }
+        d.tex[l] = tex; d.tex_w[l] = L.tex_w; d.tex_h[l] = L.tex_h;
+        voff += L.num_vertices;
+    }
+    CU(vs_launch_check_finite(pos, (size_t)vt * 3, flag, st));
+    CU(vs_launch_check_finite((const float*)uvs, (size_t)vt * 2, flag, st));
+    uint32_t hflag = 0;
+    CU(cudaMemcpyAsync(&hflag, flag, 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    if (hflag & 1u) return fail(VS_ERR_INVALID_ARG, "a triangle index is >= num_vertices of its layer");
+    if (hflag & 2u) return fail(VS_ERR_INVALID_ARG, "a vertex position or uv is not finite");
+    d.positions = pos; d.uvs = uvs; d.tris = tris;
+    CU(cudaHostAlloc((void**)&s->host_total, 64, cudaHostAllocDefault));
+    CU(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 2; ++i) {
+        CU(cudaEventCreateWithFlags(&s->ev_render[i], cudaEventDisableTiming));
+        CU(cudaEventCreateWithFlags(&s->ev_copy[i], cudaEventDisableTiming));
+    }
+    return VS_OK;
+}
+
+extern "C" vs_status vs_scene_create(const vs_scene_desc* desc, void* cuda_stream, vs_scene** out_scene)
+{
+    g_err[0] = 0;
+    if (out_scene) *out_scene = nullptr;
+    if (!desc || !out_scene) return fail(VS_ERR_INVALID_ARG, "NULL argument");
+    if (desc->num_layers < 1 || desc->num_layers > VS_MAX_LAYERS) return fail(VS_ERR_INVALID_ARG, "num_layers must be 1..9");
+    if (desc->sh_degree > 3) return fail(VS_ERR_INVALID_ARG, "sh_degree must be 0..3");
+    if (desc->tex_dtype != VS_F32 && desc->tex_dtype != VS_F16) return fail(VS_ERR_INVALID_ARG, "bad tex_dtype");
+    if (desc->memory != VS_MEM_DEVICE && desc->memory != VS_MEM_HOST) return fail(VS_ERR_INVALID_ARG, "bad memory kind");
+    if (!desc->layers) return fail(VS_ERR_INVALID_ARG, "NULL layers");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(VS_ERR_CUDA, "no CUDA device available (this library has no CPU fallback)");
+    }
+    vs_scene* s = new (std::nothrow) vs_scene();
+    if (!s) return fail(VS_ERR_OUT_OF_MEMORY, "host allocation failed");
+    cudaGetDevice(&s->device);
+    std::vector<void*> temps;
+    vs_status r = scene_create_impl(desc, (cudaStream_t)cuda_stream, s, temps);
+    cudaStreamSynchronize((cudaStream_t)cuda_stream);
+    for (void* p : temps) cudaFree(p);
+    if (r != VS_OK) {
+        delete s;
+        cudaGetLastError();
+        return r;
+    }
+    *out_scene = s;
+    return VS_OK;
+}
+
+static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, uint32_t n, const vs_render_params* p,
+                                 const void* out_rgba)
+{
+    if (!scene || !p || !out_rgba || (n && !cams)) return fail(VS_ERR_INVALID_ARG, "NULL argument");
+    if (p->width == 0 || p->height == 0) return fail(VS_ERR_INVALID_ARG, "empty image");
+    if (p->width > 16384 || p->height > 16384) return fail(VS_ERR_UNSUPPORTED, "image larger than 16384 px");
+    if (!(p->near_plane > 0.0f) || !std::isfinite(p->near_plane)) return fail(VS_ERR_INVALID_ARG, "near_plane must be > 0");
+    if (!(p->t_min >= 0.0f) || !std::isfinite(p->t_min)) return fail(VS_ERR_INVALID_ARG, "t_min must be >= 0");
+    if (p->flags & ~(uint32_t)VS_FLAG_REFERENCE_PATH) return fail(VS_ERR_INVALID_ARG, "reserved flag bits set");
+    for (int i = 0; i < 3; ++i)
+        if (!std::isfinite(p->background[i])) return fail(VS_ERR_INVALID_ARG, "background not finite");
+    for (uint32_t c = 0; c < n; ++c) {
+        const float* f = &cams[c].fx;
+        for (int i = 0; i < 16; ++i)
+            if (!std::isfinite(f[i])) return fail(VS_ERR_INVALID_ARG, "camera %u not finite", c);
+        if (!(cams[c].fx > 0.0f) || !(cams[c].fy > 0.0f)) return fail(VS_ERR_INVALID_ARG, "camera %u: fx, fy must be > 0", c);
+    }
+    return VS_OK;
+}
+
+static uint32_t pick_chunk(const vs_scene* s, const vs_render_params* p, uint32_t n)
+{
+    if (p->views_per_chunk) return p->views_per_chunk < n ? p->views_per_chunk : n;
+    // keep the per-chunk transformed vertices + outputs within a few hundred MB
+    const size_t per_view = (size_t)s->dev.v_total * 16 + (size_t)p->width * p->height * 4;
+    size_t c = (size_t)(256u << 20) / (per_view ? per_view : 1);
+    if (c < 1) c = 1;
+    if (c > 16) c = 16;
+    return (uint32_t)(c < n ? c : n);
+}
+
+// Render `views` cameras starting at cams[0] into device outputs.  All work on `st`.
+static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views, const vs_render_params* p,
+                              float* out_rgba, uint32_t* out_ids, cudaStream_t st)
+{
+    VsFrame fr;
+    fr.width = p->width; fr.height = p->height;
+    fr.tiles_x = (p->width + VS_TILE_W - 1) / VS_TILE_W; fr.tiles_y = (p->height + VS_TILE_H - 1) / VS_TILE_H;
+    fr.near_plane = p->near_plane; fr.t_min = p->t_min;
+    for (int i = 0; i < 3; ++i) fr.bg[i] = p->background[i];
+    const size_t ntile = (size_t)views * fr.tiles_x * fr.tiles_y;
+    if (ntile >= (1ull << 31)) return fail(VS_ERR_UNSUPPORTED, "too many tiles in one chunk");
+
+    CU(s->cams.reserve(sizeof(VsCamDev) * views));
+    CU(s->vtx.reserve((size_t)s->dev.v_total * views * 16 + 16));
+    CU(s->tile_count.reserve(ntile * 4));
+    CU(s->tile_off.reserve((ntile + 1) * 4));
+    CU(s->tile_cursor.reserve(ntile * 4));
+
+    VsChunk ch{};
+    ch.views = views;
+    ch.cams = (const VsCamDev*)s->cams.p;
+    ch.vtx = (int4*)s->vtx.p;
+    ch.tile_count = (uint32_t*)s->tile_count.p;
+    ch.tile_off = (uint32_t*)s->tile_off.p;
+    ch.tile_cursor = (uint32_t*)s->tile_cursor.p;
+    ch.counters = (unsigned long long*)s->counters.p;
+    ch.out_rgba = out_rgba;
+    ch.out_ids = out_ids;
+
+    static_assert(sizeof(VsCamDev) == sizeof(vs_camera), "camera layout");
+    CU(cudaMemcpyAsync(s->cams.p, cams, sizeof(VsCamDev) * views, cudaMemcpyHostToDevice, st));
+    CU(vs_launch_transform(s->dev, fr, ch, st));
+    if (p->flags & VS_FLAG_REFERENCE_PATH) {
+        CU(vs_launch_reference(s->dev, s->tex_f16, fr, ch, st));
+        return VS_OK;
+    }
+    CU(cudaMemsetAsync(ch.tile_count, 0, ntile * 4, st));
+    CU(cudaMemsetAsync(ch.tile_cursor, 0, ntile * 4, st));
+    CU(vs_launch_bin_count(s->dev, fr, ch, st));
+    CU(vs_launch_bin_scan(fr, ch, st));
+    // size the reference list from the count pass (one 4-byte read)
+    CU(cudaMemcpyAsync(s->host_total, ch.tile_off + ntile, 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    const size_t total = *s->host_total;
+    CU(s->tile_tris.reserve(total * 4 + 16));
+    ch.tile_tris = (uint32_t*)s->tile_tris.p;
+    CU(vs_launch_bin_scatter(s->dev, fr, ch, st));
+    CU(vs_launch_raster_shade(s->dev, s->tex_f16, fr, ch, st));
+    const size_t scratch = s->cams.cap + s->vtx.cap + s->tile_count.cap + s->tile_off.cap + s->tile_cursor.cap + s->tile_tris.cap;
+    if (scratch > s->scratch_peak) s->scratch_peak = scratch;
+    return VS_OK;
+}
+
+static vs_status begin_render(vs_scene* s, cudaStream_t st)
+{
+    CU(cudaSetDevice(s->device));
+    CU(s->counters.reserve(VS_CNT_N * 8));
+    CU(cudaMemsetAsync(s->counters.p, 0, VS_CNT_N * 8, st));
+    s->last_stream = st;
+    s->scratch_peak = 0;
+    return VS_OK;
+}
+
+extern "C" vs_status vs_render(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
+                               const vs_render_params* params, float* out_rgba, uint32_t* out_tri_ids,
+                               void* cuda_stream)
+{
+    g_err[0] = 0;
+    vs_status r = validate_render(scene, cameras, num_cameras, params, out_rgba);
+    if (r != VS_OK) return r;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((r = begin_render(scene, st)) != VS_OK) return r;
+    if (num_cameras == 0) return VS_OK;
+    const uint32_t chunk = pick_chunk(scene, params, num_cameras);
+    const size_t px = (size_t)params->width * params->height;
+    for (uint32_t v0 = 0; v0 < num_cameras; v0 += chunk) {
+        const uint32_t nv = num_cameras - v0 < chunk ? num_cameras - v0 : chunk;
+        r = render_chunk(scene, cameras + v0, nv, params, out_rgba + (size_t)v0 * px * 4,
+                         out_tri_ids ? out_tri_ids + (size_t)v0 * scene->dev.k * px : nullptr, st);
+        if (r != VS_OK) return r;
+    }
+    return VS_OK;
+}
+
+extern "C" vs_status vs_render_host(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
+                                    const vs_render_params* params, float* out_rgba, uint32_t* out_tri_ids,
+                                    void* cuda_stream)
+{
+    g_err[0] = 0;
+    vs_status r = validate_render(scene, cameras, num_cameras, params, out_rgba);
+    if (r != VS_OK) return r;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    if ((r = begin_render(scene, st)) != VS_OK) return r;
+    if (num_cameras == 0) return VS_OK;
+    const uint32_t chunk = pick_chunk(scene, params, num_cameras);
+    const size_t px = (size_t)params->width * params->height;
+    const size_t rgba_bytes = px * 16, ids_bytes = px * 4 * scene->dev.k;
+    uint32_t b = 0;
+    bool used[2] = {false, false};
+    for (uint32_t v0 = 0; v0 < num_cameras; v0 += chunk, b ^= 1u) {
+        const uint32_t nv = num_cameras - v0 < chunk ? num_cameras - v0 : chunk;
+        CU(scene->stage_rgba[b].reserve(rgba_bytes * chunk));
+        if (out_tri_ids) CU(scene->stage_ids[b].reserve(ids_bytes * chunk));
+        if (used[b]) CU(cudaStreamWaitEvent(st, scene->ev_copy[b], 0));  // staging buffer b is free again
+        r = render_chunk(scene, cameras + v0, nv, params, (float*)scene->stage_rgba[b].p,
+                         out_tri_ids ? (uint32_t*)scene->stage_ids[b].p : nullptr, st);
+        if (r != VS_OK) return r;
+        CU(cudaEventRecord(scene->ev_render[b], st));
+        CU(cudaStreamWaitEvent(scene->copy_stream, scene->ev_render[b], 0));
+        CU(cudaMemcpyAsync(out_rgba + (size_t)v0 * px * 4, scene->stage_rgba[b].p, rgba_bytes * nv, cudaMemcpyDeviceToHost,
+                           scene->copy_stream));
+        if (out_tri_ids)
+            CU(cudaMemcpyAsync(out_tri_ids + (size_t)v0 * scene->dev.k * px, scene->stage_ids[b].p, ids_bytes * nv,
+                               cudaMemcpyDeviceToHost, scene->copy_stream));
+        CU(cudaEventRecord(scene->ev_copy[b], scene->copy_stream));
+        used[b] = true;
+    }
+    CU(cudaStreamSynchronize(scene->copy_stream));
+    CU(cudaStreamSynchronize(st));
+    return VS_OK;
+}
+
+extern "C" vs_status vs_query_last_render(vs_scene* scene, vs_render_stats* out)
+{
+    g_err[0] = 0;
+    if (!scene || !out) return fail(VS_ERR_INVALID_ARG, "NULL argument");
+    memset(out, 0, sizeof(*out));
+    if (!scene->counters.p) return VS_OK;
+    CU(cudaSetDevice(scene->device));
+    CU(cudaStreamSynchronize(scene->last_stream));
+    unsigned long long h[VS_CNT_N];
+    CU(cudaMemcpy(h, scene->counters.p, sizeof(h), cudaMemcpyDeviceToHost));
+    out->dropped_triangles = h[VS_CNT_DROPPED];
+    out->degenerate_triangles = h[VS_CNT_DEGENERATE];
+    out->tile_refs = h[VS_CNT_REFS];
+    out->scratch_bytes = scene->scratch_peak;
+    return VS_OK;
+}

@@ -1,0 +1,204 @@
+// vs_common.cuh -- shared declarations of the CUDA path (never included by oracle/).
+// Arithmetic contract: DESIGN.md §3 (fp32-exact steps use the _rn intrinsics, which nvcc never
+// contracts or relaxes; integer steps are exact by construction).
+#pragma once
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include <stdint.h>
+
+#define VS_MAX_LAYERS 9
+#define VS_MAX_COEF 16
+#define VS_TILE_W 16
+#define VS_TILE_H 16
+#define VS_TILE_PIX (VS_TILE_W * VS_TILE_H)
+#define VS_MISS 0xFFFFFFFFu
+
+// Device-side description of an immutable scene (passed by value to kernels).
+struct VsSceneDev {
+    const float* positions;   // [v_total][3], all layers concatenated
+    const float2* uvs;        // [v_total]
+    const uint4* tris;        // [t_total] {i0, i1, i2 : global vertex index, w : layer}
+    uint32_t v_total, t_total;
+    uint32_t k, sh_degree, n_coef;
+    uint32_t texel_vecs;                  // 16-byte vectors per texel in the internal layout
+    uint32_t tri_off[VS_MAX_LAYERS + 1];  // global triangle id of each layer's triangle 0
+    const uint4* tex[VS_MAX_LAYERS];      // [tex_h][tex_w][texel_vecs] 16-byte vectors
+    uint32_t tex_w[VS_MAX_LAYERS], tex_h[VS_MAX_LAYERS];
+};
+
+struct VsCamDev {  // == vs_camera
+    float fx, fy, cx, cy;
+    float R[9];
+    float t[3];
+};
+
+struct VsFrame {
+    uint32_t width, height, tiles_x, tiles_y;
+    float near_plane, t_min;
+    float bg[3];
+};
+
+// counters[0] dropped, [1] degenerate, [2] tile refs
+enum { VS_CNT_DROPPED = 0, VS_CNT_DEGENERATE = 1, VS_CNT_REFS = 2, VS_CNT_N = 4 };
+
+// ---- triangle setup shared by the binning, raster and shading kernels ----------
+struct VsTri {
+    int X0, Y0, X1, Y1, X2, Y2;
+    float q0, q1, q2;
+    long long A2;
+    bool swapped;  // vertices 1 and 2 were exchanged to make A2 > 0
+};
+
+// vtx record = {X, Y, float_as_int(q), bad}
+__device__ __forceinline__ int vs_setup_tri(const int4& a, const int4& b, const int4& c, VsTri& t)
+{
+    if ((a.w | b.w | c.w) != 0) return 1;  // behind the near plane or off the guard band: dropped
+    long long A2 = (long long)(b.x - a.x) * (long long)(c.y - a.y) - (long long)(c.x - a.x) * (long long)(b.y - a.y);
+    if (A2 == 0) return 2;
+    t.X0 = a.x; t.Y0 = a.y; t.q0 = __int_as_float(a.z);
+    if (A2 < 0) {
+        t.X1 = c.x; t.Y1 = c.y; t.q1 = __int_as_float(c.z);
+        t.X2 = b.x; t.Y2 = b.y; t.q2 = __int_as_float(b.z);
+        t.A2 = -A2; t.swapped = true;
+    } else {
+        t.X1 = b.x; t.Y1 = b.y; t.q1 = __int_as_float(b.z);
+        t.X2 = c.x; t.Y2 = c.y; t.q2 = __int_as_float(c.z);
+        t.A2 = A2; t.swapped = false;
+    }
+    return 0;
+}
+
+// Pixel range whose sample points 256 i + 128 fall inside the triangle's bounding box, clipped to
+// [0, w-1] x [0, h-1].  Returns false if empty.
+__device__ __forceinline__ bool vs_tri_pixel_bbox(const VsTri& t, int w, int h, int& i0, int& i1, int& j0, int& j1)
+{
+    int minX = min(t.X0, min(t.X1, t.X2)), maxX = max(t.X0, max(t.X1, t.X2));
+    int minY = min(t.Y0, min(t.Y1, t.Y2)), maxY = max(t.Y0, max(t.Y1, t.Y2));
+    i0 = max((minX + 127) >> 8, 0);      // ceil((minX - 128) / 256)
+    i1 = min((maxX - 128) >> 8, w - 1);  // floor((maxX - 128) / 256)
+    j0 = max((minY + 127) >> 8, 0);
+    j1 = min((maxY - 128) >> 8, h - 1);
+    return i0 <= i1 && j0 <= j1;
+}
+
+// Edge functions at the sample point of pixel (i, j): e0 = 1->2 weights vertex 0,
+// e1 = 2->0 weights vertex 1, e2 = 0->1 weights vertex 2.
+struct VsEdges {
+    long long E0, E1, E2;
+};
+
+__device__ __forceinline__ long long vs_edge(int Xa, int Ya, int Xb, int Yb, int Sx, int Sy)
+{
+    return (long long)(Xb - Xa) * (long long)(Sy - Ya) - (long long)(Yb - Ya) * (long long)(Sx - Xa);
+}
+
+__device__ __forceinline__ bool vs_topleft(int Xa, int Ya, int Xb, int Yb)
+{
+    int dx = Xb - Xa, dy = Yb - Ya;
+    return (dy < 0) || (dy == 0 && dx > 0);
+}
+
+__device__ __forceinline__ void vs_edges_at(const VsTri& t, int i, int j, VsEdges& e)
+{
+    int Sx = 256 * i + 128, Sy = 256 * j + 128;
+    e.E0 = vs_edge(t.X1, t.Y1, t.X2, t.Y2, Sx, Sy);
+    e.E1 = vs_edge(t.X2, t.Y2, t.X0, t.Y0, Sx, Sy);
+    e.E2 = vs_edge(t.X0, t.Y0, t.X1, t.Y1, Sx, Sy);
+}
+
+// Top-left biases: covered <=> E_e + bias_e > 0 with bias = 0 for top/left edges, -1... expressed as
+// E_e >= min_e where min_e = 0 if the edge owns its samples, else 1.
+__device__ __forceinline__ void vs_edge_mins(const VsTri& t, int& m0, int& m1, int& m2)
+{
+    m0 = vs_topleft(t.X1, t.Y1, t.X2, t.Y2) ? 0 : 1;
+    m1 = vs_topleft(t.X2, t.Y2, t.X0, t.Y0) ? 0 : 1;
+    m2 = vs_topleft(t.X0, t.Y0, t.X1, t.Y1) ? 0 : 1;
+}
+
+// Depth key, fp32-exact: qp = fma(f2,q2, fma(f1,q1, f0*q0)) / fA
+__device__ __forceinline__ float vs_depth_q(const VsTri& t, long long E0, long long E1, long long E2)
+{
+    float f0 = __ll2float_rn(E0), f1 = __ll2float_rn(E1), f2 = __ll2float_rn(E2);
+    float fA = __ll2float_rn(t.A2);
+    float num = __fmaf_rn(f2, t.q2, __fmaf_rn(f1, t.q1, __fmul_rn(f0, t.q0)));
+    return __fdiv_rn(num, fA);
+}
+
+__device__ __forceinline__ unsigned long long vs_make_key(float qp, uint32_t local_tri)
+{
+    return ((unsigned long long)__float_as_uint(qp) << 32) | (unsigned long long)(0xFFFFFFFFu - local_tri);
+}
+
+// Real SH basis, fp32, tolerance domain.
+template <int DEG>
+__device__ __forceinline__ void vs_sh_basis(float x, float y, float z, float* Y)
+{
+    Y[0] = 0.28209479177387814f;
+    if (DEG >= 1) {
+        Y[1] = 0.4886025119029199f * y;
+        Y[2] = 0.4886025119029199f * z;
+        Y[3] = 0.4886025119029199f * x;
+    }
+    if (DEG >= 2) {
+        float xx = x * x, yy = y * y, zz = z * z;
+        Y[4] = 1.0925484305920792f * x * y;
+        Y[5] = 1.0925484305920792f * y * z;
+        Y[6] = 0.31539156525252005f * (3.0f * zz - 1.0f);
+        Y[7] = 1.0925484305920792f * x * z;
+        Y[8] = 0.5462742152960396f * (xx - yy);
+        if (DEG >= 3) {
+            Y[9] = 0.5900435899266435f * y * (3.0f * xx - yy);
+            Y[10] = 2.890611442640554f * x * y * z;
+            Y[11] = 0.4570457994644658f * y * (5.0f * zz - 1.0f);
+            Y[12] = 0.3731763325901154f * z * (5.0f * zz - 3.0f);
+            Y[13] = 0.4570457994644658f * x * (5.0f * zz - 1.0f);
+            Y[14] = 1.445305721320277f * z * (xx - yy);
+            Y[15] = 0.5900435899266435f * x * (xx - 3.0f * yy);
+        }
+    }
+}
+
+// Unit view direction of pixel (i, j), world frame (DESIGN.md §3.7 / reading Q4).
+__device__ __forceinline__ void vs_view_dir(const VsCamDev& c, int i, int j, float& x, float& y, float& z)
+{
+    float dx = ((float)i + 0.5f - c.cx) / c.fx;
+    float dy = ((float)j + 0.5f - c.cy) / c.fy;
+    float wx = c.R[0] * dx + c.R[3] * dy + c.R[6];
+    float wy = c.R[1] * dx + c.R[4] * dy + c.R[7];
+    float wz = c.R[2] * dx + c.R[5] * dy + c.R[8];
+    float inv = rsqrtf(wx * wx + wy * wy + wz * wz);
+    x = wx * inv; y = wy * inv; z = wz * inv;
+}
+
+__device__ __forceinline__ float vs_sigmoid(float s)
+{
+    return __fdividef(1.0f, 1.0f + __expf(-s));
+}
+
+// ---- host-side launchers (vs_kernels_*.cu) ------------------------------------------------------
+struct VsChunk {                 // one pass over `views` cameras
+    uint32_t views;
+    const VsCamDev* cams;        // DEVICE [views]
+    int4* vtx;                   // DEVICE [views][v_total]
+    uint32_t* tile_count;        // DEVICE [views * tiles]   (count pass output)
+    uint32_t* tile_off;          // DEVICE [views * tiles + 1] exclusive scan
+    uint32_t* tile_cursor;       // DEVICE [views * tiles]   scatter cursors
+    uint32_t* tile_tris;         // DEVICE [total refs]
+    unsigned long long* counters;  // DEVICE [VS_CNT_N]
+    float* out_rgba;             // DEVICE [views][H][W][4]
+    uint32_t* out_ids;           // DEVICE [views][k][H][W] or nullptr
+};
+
+cudaError_t vs_launch_transform(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_bin_count(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_bin_scan(const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_bin_scatter(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_raster_shade(const VsSceneDev& sc, int tex_f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_reference(const VsSceneDev& sc, int tex_f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
+
+// scene construction helpers
+cudaError_t vs_launch_pack_tris(const uint32_t* indices, uint32_t num_tris, uint32_t num_vertices, uint32_t vtx_off,
+                                uint32_t layer, uint4* out, uint32_t* error_flag, cudaStream_t st);
+cudaError_t vs_launch_check_finite(const float* v, size_t n, uint32_t* error_flag, cudaStream_t st);
+cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, uint32_t n_coef, uint32_t texel_vecs,
+                                   uint4* dst, cudaStream_t st);

@@ -1,0 +1,184 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the CPU oracle on the same seeded inputs.
+Bar (BASELINE.json north_star): coverage and per-layer triangle IDs BIT-EXACT, RGBA max abs error
+<= 1e-4.  Sizes here are ones the oracle finishes in seconds and that still span many tiles and a
+ragged tail; the full BASELINE.json sizes are in test_gpu_configs.py."""
+import types
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    import oracle
+    from paper_2409_02482_b200 import binding, synth
+    binding.load_library()
+    return types.SimpleNamespace(torch=torch, oracle=oracle, binding=binding, synth=synth)
+
+
+def gpu_render(env, sc, views, flags=0, t_min=None, background=None, views_per_chunk=0, want_ids=True):
+    b = env.binding
+    r = b.Renderer(sc)
+    p = b.make_params(sc.width, sc.height, sc.near_plane, sc.t_min if t_min is None else t_min,
+                      sc.background if background is None else background, flags, views_per_chunk)
+    rgba, ids = r.render(sc.cameras[list(views)], p, want_ids=want_ids)
+    env.torch.cuda.synchronize()
+    stats = r.stats()
+    out = rgba.cpu().numpy(), (ids.cpu().numpy().view(np.uint32) if want_ids else None), stats
+    r.close()
+    return out
+
+
+def check_against_oracle(env, sc, views, **kw):
+    rgba, ids, stats = gpu_render(env, sc, views, **kw)
+    okw = {}
+    if "t_min" in kw and kw["t_min"] is not None:
+        okw["t_min"] = kw["t_min"]
+    if "background" in kw and kw["background"] is not None:
+        okw["background"] = kw["background"]
+    worst = 0.0
+    for n, v in enumerate(views):
+        ref = env.oracle.render_scene(sc, [v], **okw)[0]
+        assert np.array_equal(ids[n], ref["ids"]), "triangle ids differ in view %d: %d pixels" % (
+            v, int((ids[n] != ref["ids"]).sum()))
+        err = float(np.abs(rgba[n].astype(np.float64) - ref["rgba"]).max())
+        worst = max(worst, err)
+        assert err <= TOL, "view %d: max abs rgba error %.3e" % (v, err)
+        assert stats["dropped_triangles"] == 0 or ref["stats"][0] > 0
+    return worst, rgba, ids
+
+
+def test_config1_all_views(env):
+    sc = env.synth.make_config(1)
+    worst, rgba, ids = check_against_oracle(env, sc, range(4))
+    assert (ids != env.binding.MISS).mean() > 0.5
+    print("C1 worst rgba err %.3e" % worst)
+
+
+def test_config1_reference_path_agrees(env):
+    sc = env.synth.make_config(1)
+    a = gpu_render(env, sc, [0, 2])
+    b = gpu_render(env, sc, [0, 2], flags=env.binding.VS_FLAG_REFERENCE_PATH)
+    assert np.array_equal(a[1], b[1])
+    assert np.abs(a[0] - b[0]).max() <= 2e-6
+    check_against_oracle(env, sc, [1], flags=env.binding.VS_FLAG_REFERENCE_PATH)
+
+
+@pytest.mark.parametrize("cfg,kw", [
+    (2, dict(mesh_n=40, width=333, height=250, tex_size=256, num_cameras=4)),          # fp16 deg 2, ragged tiles
+    (3, dict(mesh_n=48, width=400, height=225, tex_size=256, num_cameras=3, k=7)),     # fp16 deg 3, low alpha
+    (4, dict(mesh_n=64, width=480, height=270, tex_size=512, num_cameras=5, k=9)),     # fp16 deg 3, k = 9
+    (5, dict(mesh_n=120, width=384, height=216, tex_size=512, num_cameras=4, k=9)),    # sub-pixel tris + close-ups
+])
+def test_reduced_configs(env, cfg, kw):
+    sc = env.synth.make_config(cfg, **kw)
+    worst, _, ids = check_against_oracle(env, sc, range(len(sc.cameras)), views_per_chunk=2)
+    print("C%d reduced worst rgba err %.3e, coverage %.2f" % (cfg, worst, (ids != env.binding.MISS).mean()))
+
+
+def test_determinism_and_chunking(env):
+    sc = env.synth.make_config(2, mesh_n=30, width=200, height=150, tex_size=128, num_cameras=6)
+    a = gpu_render(env, sc, range(6), views_per_chunk=1)
+    b = gpu_render(env, sc, range(6), views_per_chunk=4)
+    c = gpu_render(env, sc, range(6))
+    for x in (b, c):
+        assert np.array_equal(a[0], x[0]) and np.array_equal(a[1], x[1])
+
+
+@pytest.mark.parametrize("dtype,deg", [(np.float32, 0), (np.float16, 0), (np.float16, 1), (np.float32, 2), (np.float32, 3)])
+def test_all_texture_formats(env, dtype, deg):
+    rng = np.random.default_rng(5)
+    sc = env.synth.make_config(1, width=96, height=80, num_cameras=2, tex_size=64)
+    n = (deg + 1) ** 2
+    for ly in sc.layers:
+        ly.texture = rng.normal(0, 0.5, size=(48, 64, n, 4)).astype(dtype)     # non-square texture too
+    sc.sh_degree = deg
+    check_against_oracle(env, sc, [0, 1])
+
+
+def test_edge_cases(env):
+    s = env.synth
+    # early exit with opaque-ish layers, non-zero background, t_min variants
+    sc = s.make_config(1, width=100, height=60, num_cameras=1, tex_size=64)
+    for ly in sc.layers:
+        ly.texture[:, :, 0, 3] += 12.0
+    check_against_oracle(env, sc, [0], t_min=2.0 ** -6, background=(0.2, 0.4, 0.6))
+    check_against_oracle(env, sc, [0], t_min=0.0)
+    # exactly opaque / exactly transparent layers (fp16 +-60000)
+    sc = s.make_config(2, mesh_n=16, width=90, height=70, tex_size=64, num_cameras=2, k=3)
+    sc.layers[0].texture[:, :, 0, 3] = -60000.0
+    sc.layers[1].texture[:, :, 0, 3] = 60000.0
+    worst, rgba, ids = check_against_oracle(env, sc, [0, 1])
+    assert np.all(rgba[..., 3][ids[:, 1] != env.binding.MISS] == 1.0)
+    # a shell with no triangles, a 1x1 texture, k = 1, 1x1 image, image not a multiple of the tile
+    sc = s.make_config(1, width=17, height=33, num_cameras=1, tex_size=16)
+    sc.layers[1].indices = np.zeros((0, 3), np.uint32)
+    sc.layers[2].texture = sc.layers[2].texture[:1, :1].copy()
+    check_against_oracle(env, sc, [0])
+    one = s.Scene("k1", sc.layers[:1], 1, sc.cameras, 1, 1)
+    check_against_oracle(env, one, [0])
+    # every triangle behind the camera: dropped, background everywhere
+    cam = s.look_at_camera((0, 0, 3.0), 64, 48, target=(0, 0, 6.0))
+    sc = s.make_config(1, width=64, height=48, num_cameras=1, tex_size=16)
+    sc.cameras = cam[None]
+    rgba, ids, stats = gpu_render(env, sc, [0], background=(0.1, 0.2, 0.3))
+    assert np.all(ids == env.binding.MISS) and stats["dropped_triangles"] == 3 * 1280
+    assert np.allclose(rgba, np.array([0.1, 0.2, 0.3, 0.0], np.float32))
+    # big triangles (warp-cooperative path) + degenerate + duplicate triangles, UVs outside [0,1]
+    rng = np.random.default_rng(3)
+    pos = np.array([[-2, -2, 4], [2, -2, 4], [2, 2, 4], [-2, 2, 4], [0, 0, 3.5]], np.float32)
+    uv = np.array([[-0.3, -0.2], [1.4, 0], [1.2, 1.3], [0, 1], [0.5, 0.5]], np.float32)
+    idx = np.array([[0, 1, 2], [0, 2, 3], [0, 1, 4], [0, 0, 1], [0, 1, 2]], np.uint32)
+    tex = rng.normal(0, 0.5, (32, 32, 4, 4)).astype(np.float32)
+    big = s.Scene("big", [s.Layer(pos, uv, idx, tex)], 1,
+                  np.stack([s.look_at_camera((0.3, 0.2, -1.0), 150, 100, target=(0, 0, 4.0))]), 150, 100)
+    check_against_oracle(env, big, [0])
+    rgba, ids, stats = gpu_render(env, big, [0])
+    assert stats["degenerate_triangles"] == 1
+
+
+def test_invalid_arguments_are_rejected(env):
+    b, torch = env.binding, env.torch
+    sc = env.synth.make_config(1, width=32, height=32, num_cameras=1, tex_size=16)
+    sc.layers[0].indices = sc.layers[0].indices.copy()
+    sc.layers[0].indices[5, 1] = 10 ** 6
+    with pytest.raises(b.VsError) as e:
+        b.Renderer(sc)
+    assert e.value.status == b.VS_ERR_INVALID_ARG
+    sc = env.synth.make_config(1, width=32, height=32, num_cameras=1, tex_size=16)
+    sc.layers[1].positions = sc.layers[1].positions.copy()
+    sc.layers[1].positions[7, 2] = np.nan
+    with pytest.raises(b.VsError):
+        b.Renderer(sc)
+    sc = env.synth.make_config(1, width=32, height=32, num_cameras=1, tex_size=16)
+    r = b.Renderer(sc)
+    out = torch.empty((1, 32, 32, 4), device="cuda")
+    with pytest.raises(b.VsError):
+        b.vs_render(r.handle, sc.cameras, b.make_params(32, 32, near_plane=0.0), out)
+    bad = sc.cameras.copy()
+    bad[0, 5] = np.inf
+    with pytest.raises(b.VsError):
+        b.vs_render(r.handle, bad, b.make_params(32, 32), out)
+    r.close()
+
+
+def test_host_path_matches_device_path(env):
+    b, torch = env.binding, env.torch
+    sc = env.synth.make_config(2, mesh_n=24, width=160, height=120, tex_size=64, num_cameras=5)
+    dev_rgba, dev_ids, _ = gpu_render(env, sc, range(5))
+    # host descriptors (numpy arrays) for scene creation + host outputs
+    h = b.vs_scene_create(sc.layers, sc.sh_degree)
+    out = torch.empty((5, 120, 160, 4), dtype=torch.float32).pin_memory()
+    ids = torch.empty((5, sc.k, 120, 160), dtype=torch.int32).pin_memory()
+    b.vs_render_host(h, sc.cameras, b.make_params(160, 120, views_per_chunk=2), out, ids)
+    assert np.array_equal(out.numpy(), dev_rgba) and np.array_equal(ids.numpy().view(np.uint32), dev_ids)
+    pageable = np.empty((5, 120, 160, 4), np.float32)
+    b.vs_render_host(h, sc.cameras, b.make_params(160, 120), pageable)
+    assert np.array_equal(pageable, dev_rgba)
+    b.vs_scene_destroy(h)
