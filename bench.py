@@ -1,0 +1,278 @@
+#!/usr/bin/env python
+"""bench.py -- headline measurement of the k-shell render path (BASELINE.json metric: megapixels/s and
+fps rendering k layers at 1080p; achieved HBM GB/s vs peak).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
+
+A "step" is one vs_render call = one pass of the whole hot path (S1-S7) over one batch of cameras of
+the chosen configuration (default C4, the headline roofline config: k=9, ~300k triangles per layer,
+1920x1080, 64 views per call, SH-3 fp16 2048^2 textures).  Prints ONE JSON line on rank 0.
+`--impl reference` times the CPU oracle (as it stands) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_2409_02482_b200 import dist as vsdist  # noqa: E402
+from paper_2409_02482_b200 import synth  # noqa: E402
+
+METRIC = "megapixels_per_sec_rendering_k_layers"
+UNIT = "MP/s"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
+# `ncu --set full` capture (profiles/), keyed by config; None until a capture exists.
+NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+def geometry_bytes_per_view(sc):
+    return sum(ly.positions.shape[0] * 20 + ly.indices.shape[0] * 12 for ly in sc.layers)
+
+
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.path = tempfile.mktemp(suffix=".csv")
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.FIELDS,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        try:
+            for line in open(self.path):
+                f = [x.strip() for x in line.split(",")]
+                if len(f) < 8:
+                    continue
+                try:
+                    sm.append(float(f[0])); mx.append(float(f[1])); power.append(float(f[2]))
+                except ValueError:
+                    continue
+                for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[4:8]):
+                    if val.lower().startswith("active"):
+                        reasons.add(name)
+            os.unlink(self.path)
+        except Exception:
+            pass
+        if sm:
+            out = {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+                   "samples": len(sm), "power_w_max": max(power) if power else None}
+        return out
+
+
+def build_scene(cfg, rank, world, args):
+    kw = {}
+    if args.views:
+        kw["num_cameras"] = args.views
+    return synth.make_config(cfg, camera_rotate=vsdist.rank_camera_rotation(rank, world), **kw)
+
+
+def time_oracle(sc, views, threads=0):
+    import oracle
+    t0 = time.perf_counter()
+    for v in views:
+        oracle.render_view(sc.layers, sc.sh_degree, sc.cameras[v], sc.width, sc.height, near_plane=sc.near_plane,
+                           t_min=sc.t_min, background=sc.background, num_threads=threads)
+    return time.perf_counter() - t0
+
+
+def run_reference(args):
+    rank, local, world = vsdist.env_rank()
+    if rank != 0:
+        return 0
+    import oracle
+    sc = build_scene(args.config, 0, 1, args)
+    sample_views = 1
+    px = sc.width * sc.height * sample_views
+    for _ in range(args.warmup):
+        time_oracle(sc, [0])
+    t = 0.0
+    for s in range(args.steps):
+        t += time_oracle(sc, [(s * sample_views + i) % len(sc.cameras) for i in range(sample_views)])
+    value = px * args.steps / t / 1e6
+    cores = oracle.max_threads()
+    sample = "%d view(s) per step of %s (bounded sample of the %d-view batch)" % (sample_views, sc.name, len(sc.cameras))
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "fps": sample_views * args.steps / t,
+            "config": {"workload": sc.name, "k": sc.k, "width": sc.width, "height": sc.height,
+                       "views_per_step": sample_views, "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+    return 0
+
+
+def run_ours(args):
+    import torch
+    from paper_2409_02482_b200 import binding
+    rank, local, world = vsdist.env_rank()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    vsdist.init_process_group("nccl")
+    binding.load_library()
+
+    sc = build_scene(args.config, rank, world, args)
+    B, W, H = len(sc.cameras), sc.width, sc.height
+    renderer = binding.Renderer(sc, dev)
+    flags = binding.VS_FLAG_KERNEL_TIMING
+    params = binding.make_params(W, H, sc.near_plane, sc.t_min, sc.background, flags, args.chunk)
+    out = torch.empty((B, H, W, 4), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+
+    # untimed: count the algorithmic texture bytes (unique texels per view) of this batch
+    cparams = binding.make_params(W, H, sc.near_plane, sc.t_min, sc.background, binding.VS_FLAG_COUNT_TEXELS, args.chunk)
+    binding.vs_render(renderer.handle, sc.cameras, cparams, out)
+    cstats = renderer.stats()
+    texel_bytes = 16 * ((sc.n_coef * 4 * sc.layers[0].texture.dtype.itemsize + 15) // 16)
+    b_tex = cstats["unique_texels"] * texel_bytes
+    b_geom = geometry_bytes_per_view(sc) * B
+    b_fb = W * H * 16 * B
+    alg_bytes_step = b_tex + b_geom + b_fb
+
+    for _ in range(max(args.warmup, 0)):
+        binding.vs_render(renderer.handle, sc.cameras, params, out)
+    torch.cuda.synchronize()
+
+    sampler = ClockSampler(local) if rank == 0 else None
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    raster_ms = bin_ms = xf_ms = 0.0
+    raster_launches = launches = 0
+    vsdist.barrier()
+    torch.cuda.synchronize()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        binding.vs_render(renderer.handle, sc.cameras, params, out)
+        st = renderer.stats()                      # syncs the stream; per-kernel CUDA-event times
+        raster_ms += st["ms_raster_shade"]; bin_ms += st["ms_binning"]; xf_ms += st["ms_transform"]
+        raster_launches += st["raster_launches"]; launches += st["kernel_launches"]
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    vsdist.barrier()
+    secs = ev0.elapsed_time(ev1) / 1e3
+    clocks = sampler.stop() if sampler else None
+    secs_max = vsdist.max_over_ranks(secs, dev)
+    pixels_all = vsdist.sum_over_ranks(float(B * W * H * args.steps), dev)
+    value = pixels_all / secs_max / 1e6
+    fps = vsdist.sum_over_ranks(float(B * args.steps), dev) / secs_max
+
+    # end to end through the C-ABI with HOST buffers: camera upload + image download every step
+    e2e_steps = max(1, min(args.steps, 5))
+    host_out = torch.empty((B, H, W, 4), dtype=torch.float32).pin_memory()
+    eparams = binding.make_params(W, H, sc.near_plane, sc.t_min, sc.background, 0, args.chunk)
+    binding.vs_render_host(renderer.handle, sc.cameras, eparams, host_out)
+    vsdist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        binding.vs_render_host(renderer.handle, sc.cameras, eparams, host_out)
+    torch.cuda.synchronize()
+    e2e_secs = vsdist.max_over_ranks(time.perf_counter() - t0, dev)
+    e2e_value = vsdist.sum_over_ranks(float(B * W * H * e2e_steps), dev) / e2e_secs / 1e6
+
+    if rank != 0:
+        renderer.close()
+        return 0
+
+    peak, peak_src = load_peaks()
+    per_launch_ms = raster_ms / max(raster_launches, 1)
+    bytes_per_launch = alg_bytes_step * args.steps / max(raster_launches, 1)
+    achieved = bytes_per_launch / (per_launch_ms * 1e-3) / 1e9 if per_launch_ms > 0 else 0.0
+    step_achieved = alg_bytes_step * world / (secs_max / args.steps) / 1e9
+    roofline = {"bound": "hbm", "kernel": "k_raster_shade", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config),
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_per_launch,
+                "launch_ms": per_launch_ms, "kernel_share_of_step": raster_ms / (secs * 1e3),
+                "bytes_per_view": {"texels_unique": b_tex / B, "geometry": b_geom / B, "framebuffer": b_fb / B},
+                "whole_step": {"achieved": step_achieved / world, "frac": step_achieved / world / peak},
+                "stage_ms_per_step": {"transform": xf_ms / args.steps, "binning": bin_ms / args.steps,
+                                      "raster_shade": raster_ms / args.steps}}
+
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu:
+        import oracle
+        nviews = args.cpu_views
+        t = time_oracle(sc, range(nviews))
+        cpu_baseline = {"value": nviews * W * H / t / 1e6, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
+                        "sample": "first %d of %d views of %s, %.1f s" % (nviews, B, sc.name, t)}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * secs_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic", "fps": fps,
+            "config": {"workload": sc.name, "k": sc.k, "triangles_per_layer": int(sc.layers[0].indices.shape[0]),
+                       "width": W, "height": H, "views_per_step": B, "sh_degree": sc.sh_degree,
+                       "texture": "%s %dx%d" % (sc.layers[0].texture.dtype, sc.layers[0].texture.shape[1], sc.layers[0].texture.shape[0]),
+                       "parallelism": "views sharded, scene replicated (dp%d)" % world,
+                       "l2": "no flush: %.1f GiB of textures streamed per step >> 126 MB L2" % (
+                           sum(ly.texture.nbytes for ly in sc.layers) / 2 ** 30),
+                       "shaded_fragments_per_view": cstats["shaded_fragments"] / B,
+                       "tile_refs_per_view": cstats["tile_refs"] / B},
+            "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu_baseline,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(sc.cameras.nbytes),
+                    "d2h_bytes_per_step": int(host_out.numel() * 4), "steps": e2e_steps},
+            "gpu_launches": int(launches)}
+    print(json.dumps(line))
+    renderer.close()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
+    ap.add_argument("--views", type=int, default=0, help="override the number of views per step")
+    ap.add_argument("--chunk", type=int, default=0, help="views per internal pass (0 = automatic)")
+    ap.add_argument("--cpu-views", type=int, default=2, help="views of the sample the oracle is timed on")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -82,8 +82,13 @@ typedef struct {
 } vs_camera;
 
 enum {
-    VS_FLAG_REFERENCE_PATH = 1u << 0 /* debugging aid: brute-force kernel (one thread per pixel, every
-                                        triangle tested), same arithmetic and outputs; small scenes only */
+    VS_FLAG_REFERENCE_PATH = 1u << 0, /* debugging aid: brute-force kernel (one thread per pixel, every
+                                         triangle tested), same arithmetic and outputs; small scenes only */
+    VS_FLAG_KERNEL_TIMING  = 1u << 1, /* bracket every kernel launch with CUDA events on the render stream
+                                         and report per-stage device time in vs_render_stats              */
+    VS_FLAG_COUNT_TEXELS   = 1u << 2  /* measurement aid: count shaded fragments and, per view, the UNIQUE
+                                         texels their 2x2 footprints reference (the algorithmic texture
+                                         bytes of DESIGN.md §8); slower, not for timed runs                */
 };
 
 typedef struct {
@@ -103,6 +108,13 @@ typedef struct {
     uint64_t degenerate_triangles; /* zero area after snapping                                             */
     uint64_t tile_refs;            /* (triangle, tile) pairs binned                                        */
     uint64_t scratch_bytes;        /* peak device scratch of the call                                      */
+    uint64_t kernel_launches;      /* kernels launched by the call (memsets / copies not counted)          */
+    uint64_t raster_launches;      /* of which fused raster+shade kernels (one per chunk of cameras)       */
+    uint64_t shaded_fragments;     /* VS_FLAG_COUNT_TEXELS: (pixel, layer) fragments shaded                */
+    uint64_t unique_texels;        /* VS_FLAG_COUNT_TEXELS: sum over views and layers of distinct texels   */
+    double   ms_transform;         /* VS_FLAG_KERNEL_TIMING: device time per stage, summed over the call   */
+    double   ms_binning;           /*   count + scan + scatter                                             */
+    double   ms_raster_shade;      /*   fused raster + shade + composite kernel                            */
 } vs_render_stats;
 
 /*

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libvs_b200.so")
 VS_OK, VS_ERR_INVALID_ARG, VS_ERR_OUT_OF_MEMORY, VS_ERR_CUDA, VS_ERR_UNSUPPORTED = range(5)
 VS_F32, VS_F16 = 0, 1
 VS_MEM_DEVICE, VS_MEM_HOST = 0, 1
-VS_FLAG_REFERENCE_PATH = 1
+VS_FLAG_REFERENCE_PATH, VS_FLAG_KERNEL_TIMING, VS_FLAG_COUNT_TEXELS = 1, 2, 4
 MISS = 0xFFFFFFFF
 
 EXPORTS = ["vs_scene_create", "vs_render", "vs_render_host", "vs_query_last_render", "vs_scene_destroy",
@@ -54,7 +54,9 @@ class vs_render_params(C.Structure):
 
 class vs_render_stats(C.Structure):
     _fields_ = [("dropped_triangles", C.c_uint64), ("degenerate_triangles", C.c_uint64),
-                ("tile_refs", C.c_uint64), ("scratch_bytes", C.c_uint64)]
+                ("tile_refs", C.c_uint64), ("scratch_bytes", C.c_uint64), ("kernel_launches", C.c_uint64),
+                ("raster_launches", C.c_uint64), ("shaded_fragments", C.c_uint64), ("unique_texels", C.c_uint64),
+                ("ms_transform", C.c_double), ("ms_binning", C.c_double), ("ms_raster_shade", C.c_double)]
 
 
 _lib = None
@@ -192,7 +194,7 @@ def vs_render_host(scene: int, cameras, params: vs_render_params, out_rgba, out_
 def vs_query_last_render(scene: int) -> dict:
     st = vs_render_stats()
     _check(load_library().vs_query_last_render(scene, C.byref(st)))
-    return {f: int(getattr(st, f)) for f, _ in vs_render_stats._fields_}
+    return {f: (float if t is C.c_double else int)(getattr(st, f)) for f, t in vs_render_stats._fields_}
 
 
 def vs_scene_destroy(scene: int):

@@ -52,7 +52,13 @@ struct vs_scene {
     int tex_f16 = 0;
     std::vector<void*> owned;
     // scratch, reused between calls
-    DevBuf cams, vtx, tile_count, tile_off, tile_cursor, tile_tris, counters, stage_rgba[2], stage_ids[2];
+    DevBuf cams, vtx, tile_count, tile_off, tile_cursor, tile_tris, counters, texel_bits, stage_rgba[2], stage_ids[2];
+    // per-call bookkeeping
+    uint64_t launches = 0, raster_launches = 0;
+    struct Span { cudaEvent_t a, b; int stage; };
+    std::vector<Span> spans;        // VS_FLAG_KERNEL_TIMING: event pairs recorded this call
+    std::vector<cudaEvent_t> event_pool;
+    size_t events_used = 0;
     uint32_t* host_total = nullptr;  // pinned
     cudaStream_t last_stream = nullptr;
     cudaStream_t copy_stream = nullptr;
@@ -61,8 +67,9 @@ struct vs_scene {
     ~vs_scene()
     {
         for (void* p : owned) cudaFree(p);
-        DevBuf* bufs[] = {&cams, &vtx, &tile_count, &tile_off, &tile_cursor, &tile_tris, &counters,
+        DevBuf* bufs[] = {&cams, &vtx, &tile_count, &tile_off, &tile_cursor, &tile_tris, &counters, &texel_bits,
                           &stage_rgba[0], &stage_rgba[1], &stage_ids[0], &stage_ids[1]};
+        for (cudaEvent_t e : event_pool) cudaEventDestroy(e);
         for (DevBuf* b : bufs) b->release();
         if (host_total) cudaFreeHost(host_total);
         if (copy_stream) cudaStreamDestroy(copy_stream);
@@ -127,6 +134,12 @@ static vs_status scene_create_impl(const vs_scene_desc* desc, cudaStream_t st, v
         if (vt >= (1ull << 31) || tt >= (1ull << 31)) return fail(VS_ERR_UNSUPPORTED, "scene too large");
     }
     for (uint32_t l = k; l <= VS_MAX_LAYERS; ++l) d.tri_off[l] = (uint32_t)tt;
+    uint64_t bits = 0;
+    for (uint32_t l = 0; l <= VS_MAX_LAYERS; ++l) {
+        d.tex_bit_off[l] = (uint32_t)bits;
+        if (l < k) bits += ((uint64_t)desc->layers[l].tex_w * desc->layers[l].tex_h + 31) / 32 * 32;
+        if (bits >= (1ull << 32)) return fail(VS_ERR_UNSUPPORTED, "textures too large");
+    }
     d.v_total = (uint32_t)vt; d.t_total = (uint32_t)tt;
 
     float* pos; float2* uvs; uint4* tris; uint32_t* flag;
@@ -219,7 +232,8 @@ static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, u
     if (p->width > 16384 || p->height > 16384) return fail(VS_ERR_UNSUPPORTED, "image larger than 16384 px");
     if (!(p->near_plane > 0.0f) || !std::isfinite(p->near_plane)) return fail(VS_ERR_INVALID_ARG, "near_plane must be > 0");
     if (!(p->t_min >= 0.0f) || !std::isfinite(p->t_min)) return fail(VS_ERR_INVALID_ARG, "t_min must be >= 0");
-    if (p->flags & ~(uint32_t)VS_FLAG_REFERENCE_PATH) return fail(VS_ERR_INVALID_ARG, "reserved flag bits set");
+    if (p->flags & ~(uint32_t)(VS_FLAG_REFERENCE_PATH | VS_FLAG_KERNEL_TIMING | VS_FLAG_COUNT_TEXELS))
+        return fail(VS_ERR_INVALID_ARG, "reserved flag bits set");
     for (int i = 0; i < 3; ++i)
         if (!std::isfinite(p->background[i])) return fail(VS_ERR_INVALID_ARG, "background not finite");
     for (uint32_t c = 0; c < n; ++c) {
@@ -240,6 +254,28 @@ static uint32_t pick_chunk(const vs_scene* s, const vs_render_params* p, uint32_
     if (c < 1) c = 1;
     if (c > 16) c = 16;
     return (uint32_t)(c < n ? c : n);
+}
+
+static vs_status span_begin(vs_scene* s, bool on, int stage, cudaStream_t st)
+{
+    if (!on) return VS_OK;
+    while (s->event_pool.size() < s->events_used + 2) {
+        cudaEvent_t e;
+        CU(cudaEventCreate(&e));
+        s->event_pool.push_back(e);
+    }
+    vs_scene::Span sp{s->event_pool[s->events_used], s->event_pool[s->events_used + 1], stage};
+    s->events_used += 2;
+    CU(cudaEventRecord(sp.a, st));
+    s->spans.push_back(sp);
+    return VS_OK;
+}
+
+static vs_status span_end(vs_scene* s, bool on, cudaStream_t st)
+{
+    if (!on) return VS_OK;
+    CU(cudaEventRecord(s->spans.back().b, st));
+    return VS_OK;
 }
 
 // Render `views` cameras starting at cams[0] into device outputs.  All work on `st`.
@@ -272,24 +308,48 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
     ch.out_ids = out_ids;
 
     static_assert(sizeof(VsCamDev) == sizeof(vs_camera), "camera layout");
+    const bool timing = (p->flags & VS_FLAG_KERNEL_TIMING) != 0;
+    vs_status r;
     CU(cudaMemcpyAsync(s->cams.p, cams, sizeof(VsCamDev) * views, cudaMemcpyHostToDevice, st));
+    if ((r = span_begin(s, timing, 0, st)) != VS_OK) return r;
     CU(vs_launch_transform(s->dev, fr, ch, st));
+    if ((r = span_end(s, timing, st)) != VS_OK) return r;
+    s->launches += 1;
     if (p->flags & VS_FLAG_REFERENCE_PATH) {
         CU(vs_launch_reference(s->dev, s->tex_f16, fr, ch, st));
+        s->launches += 1;
         return VS_OK;
     }
     CU(cudaMemsetAsync(ch.tile_count, 0, ntile * 4, st));
     CU(cudaMemsetAsync(ch.tile_cursor, 0, ntile * 4, st));
+    if ((r = span_begin(s, timing, 1, st)) != VS_OK) return r;
     CU(vs_launch_bin_count(s->dev, fr, ch, st));
     CU(vs_launch_bin_scan(fr, ch, st));
+    if ((r = span_end(s, timing, st)) != VS_OK) return r;
     // size the reference list from the count pass (one 4-byte read)
     CU(cudaMemcpyAsync(s->host_total, ch.tile_off + ntile, 4, cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
     const size_t total = *s->host_total;
     CU(s->tile_tris.reserve(total * 4 + 16));
     ch.tile_tris = (uint32_t*)s->tile_tris.p;
+    if (p->flags & VS_FLAG_COUNT_TEXELS) {
+        const size_t words = (size_t)views * (s->dev.tex_bit_off[s->dev.k] >> 5);
+        CU(s->texel_bits.reserve(words * 4 + 16));
+        CU(cudaMemsetAsync(s->texel_bits.p, 0, words * 4, st));
+        ch.texel_bits = (uint32_t*)s->texel_bits.p;
+    }
+    if ((r = span_begin(s, timing, 1, st)) != VS_OK) return r;
     CU(vs_launch_bin_scatter(s->dev, fr, ch, st));
+    if ((r = span_end(s, timing, st)) != VS_OK) return r;
+    if ((r = span_begin(s, timing, 2, st)) != VS_OK) return r;
     CU(vs_launch_raster_shade(s->dev, s->tex_f16, fr, ch, st));
+    if ((r = span_end(s, timing, st)) != VS_OK) return r;
+    s->launches += 4;
+    s->raster_launches += 1;
+    if (ch.texel_bits) {
+        CU(vs_launch_popcount(ch.texel_bits, (size_t)views * (s->dev.tex_bit_off[s->dev.k] >> 5),
+                              ch.counters + VS_CNT_TEXELS, st));
+    }
     const size_t scratch = s->cams.cap + s->vtx.cap + s->tile_count.cap + s->tile_off.cap + s->tile_cursor.cap + s->tile_tris.cap;
     if (scratch > s->scratch_peak) s->scratch_peak = scratch;
     return VS_OK;
@@ -302,6 +362,9 @@ static vs_status begin_render(vs_scene* s, cudaStream_t st)
     CU(cudaMemsetAsync(s->counters.p, 0, VS_CNT_N * 8, st));
     s->last_stream = st;
     s->scratch_peak = 0;
+    s->launches = s->raster_launches = 0;
+    s->spans.clear();
+    s->events_used = 0;
     return VS_OK;
 }
 
@@ -378,5 +441,14 @@ extern "C" vs_status vs_query_last_render(vs_scene* scene, vs_render_stats* out)
     out->degenerate_triangles = h[VS_CNT_DEGENERATE];
     out->tile_refs = h[VS_CNT_REFS];
     out->scratch_bytes = scene->scratch_peak;
+    out->kernel_launches = scene->launches;
+    out->raster_launches = scene->raster_launches;
+    out->shaded_fragments = h[VS_CNT_FRAGS];
+    out->unique_texels = h[VS_CNT_TEXELS];
+    for (const vs_scene::Span& sp : scene->spans) {
+        float ms = 0.0f;
+        CU(cudaEventElapsedTime(&ms, sp.a, sp.b));
+        (sp.stage == 0 ? out->ms_transform : sp.stage == 1 ? out->ms_binning : out->ms_raster_shade) += ms;
+    }
     return VS_OK;
 }

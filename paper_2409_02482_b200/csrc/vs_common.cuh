@@ -24,6 +24,7 @@ struct VsSceneDev {
     uint32_t tri_off[VS_MAX_LAYERS + 1];  // global triangle id of each layer's triangle 0
     const uint4* tex[VS_MAX_LAYERS];      // [tex_h][tex_w][texel_vecs] 16-byte vectors
     uint32_t tex_w[VS_MAX_LAYERS], tex_h[VS_MAX_LAYERS];
+    uint32_t tex_bit_off[VS_MAX_LAYERS + 1];  // VS_FLAG_COUNT_TEXELS: first bitmap bit of each layer (multiple of 32)
 };
 
 struct VsCamDev {  // == vs_camera
@@ -38,8 +39,8 @@ struct VsFrame {
     float bg[3];
 };
 
-// counters[0] dropped, [1] degenerate, [2] tile refs
-enum { VS_CNT_DROPPED = 0, VS_CNT_DEGENERATE = 1, VS_CNT_REFS = 2, VS_CNT_N = 4 };
+// counters[0] dropped, [1] degenerate, [2] tile refs, [3] shaded fragments, [4] unique texels
+enum { VS_CNT_DROPPED = 0, VS_CNT_DEGENERATE = 1, VS_CNT_REFS = 2, VS_CNT_FRAGS = 3, VS_CNT_TEXELS = 4, VS_CNT_N = 8 };
 
 // ---- triangle setup shared by the binning, raster and shading kernels ----------
 struct VsTri {
@@ -187,6 +188,7 @@ struct VsChunk {                 // one pass over `views` cameras
     unsigned long long* counters;  // DEVICE [VS_CNT_N]
     float* out_rgba;             // DEVICE [views][H][W][4]
     uint32_t* out_ids;           // DEVICE [views][k][H][W] or nullptr
+    uint32_t* texel_bits;        // DEVICE [views][tex_bit_off[k] / 32] or nullptr (VS_FLAG_COUNT_TEXELS)
 };
 
 cudaError_t vs_launch_transform(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
@@ -194,6 +196,7 @@ cudaError_t vs_launch_bin_count(const VsSceneDev& sc, const VsFrame& fr, const V
 cudaError_t vs_launch_bin_scan(const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_bin_scatter(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_raster_shade(const VsSceneDev& sc, int tex_f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_popcount(const uint32_t* words, size_t n, unsigned long long* counter, cudaStream_t st);
 cudaError_t vs_launch_reference(const VsSceneDev& sc, int tex_f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 
 // scene construction helpers

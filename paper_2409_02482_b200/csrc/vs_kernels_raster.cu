@@ -100,11 +100,12 @@ __device__ __forceinline__ void vs_accumulate_vec(const uint4& t00, const uint4&
     }
 }
 
-template <int F16, int DEG>
+template <int F16, int DEG, bool COUNT>
 __global__ void __launch_bounds__(256, 2)
 k_raster_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams, const int4* __restrict__ vtx,
                const uint32_t* __restrict__ tile_off, const uint32_t* __restrict__ tile_tris,
-               float* __restrict__ out_rgba, uint32_t* __restrict__ out_ids)
+               float* __restrict__ out_rgba, uint32_t* __restrict__ out_ids, uint32_t* __restrict__ texel_bits,
+               unsigned long long* __restrict__ counters)
 {
     constexpr int NCOEF = (DEG + 1) * (DEG + 1);
     constexpr int CPV = F16 ? 2 : 1;                 // coefficients per 16-byte vector
@@ -261,6 +262,17 @@ k_raster_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict
         VsFragRec r;
         r.o00 = r.o01 = r.o10 = r.o11 = 0; r.w00 = r.w01 = r.w10 = r.w11 = 0.0f;
         if (shade) vs_fragment_record(sc, vv, l, lid, px, py, r);
+        if (COUNT) {  // measurement aid: mark the 2x2 footprint in this view's texel bitmap
+            if (shade) {
+                uint32_t* bits = texel_bits + (size_t)view * (sc.tex_bit_off[sc.k] >> 5);
+                const uint32_t o4[4] = {r.o00, r.o01, r.o10, r.o11};
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t bit = sc.tex_bit_off[l] + o4[q] / sc.texel_vecs;
+                    atomicOr(&bits[bit >> 5], 1u << (bit & 31));
+                }
+            }
+            if (lane == 0) atomicAdd(&counters[VS_CNT_FRAGS], (unsigned long long)__popc(m));
+        }
         rec[lane] = r;
         __syncwarp();
         const uint4* __restrict__ tb = sc.tex[l];
@@ -304,16 +316,23 @@ k_raster_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict
             make_float4(Cr + Tr * fr.bg[0], Cg + Tr * fr.bg[1], Cb + Tr * fr.bg[2], 1.0f - Tr);
 }
 
-template <int F16, int DEG>
-static cudaError_t launch_rs(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
+template <int F16, int DEG, bool COUNT>
+static cudaError_t launch_rs2(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
 {
     const size_t smem = (size_t)sc.k * VS_TILE_PIX * 8 + 8 * 32 * sizeof(VsFragRec) + 8 * 32 * 8 * sizeof(float4);
-    auto kern = k_raster_shade<F16, DEG>;
+    auto kern = k_raster_shade<F16, DEG, COUNT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid(fr.tiles_x * fr.tiles_y, ch.views);
-    kern<<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_off, ch.tile_tris, ch.out_rgba, ch.out_ids);
+    kern<<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_off, ch.tile_tris, ch.out_rgba, ch.out_ids,
+                                  ch.texel_bits, ch.counters);
     return cudaGetLastError();
+}
+
+template <int F16, int DEG>
+static cudaError_t launch_rs(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
+{
+    return ch.texel_bits ? launch_rs2<F16, DEG, true>(sc, fr, ch, st) : launch_rs2<F16, DEG, false>(sc, fr, ch, st);
 }
 
 cudaError_t vs_launch_raster_shade(const VsSceneDev& sc, int f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
@@ -400,5 +419,21 @@ cudaError_t vs_launch_reference(const VsSceneDev& sc, int f16, const VsFrame& fr
     dim3 grid((fr.width + 15) / 16, (fr.height + 7) / 8, ch.views);
     if (f16) k_reference<1><<<grid, 128, 0, st>>>(sc, fr, ch.cams, ch.vtx, ch.out_rgba, ch.out_ids);
     else k_reference<0><<<grid, 128, 0, st>>>(sc, fr, ch.cams, ch.vtx, ch.out_rgba, ch.out_ids);
+    return cudaGetLastError();
+}
+
+// VS_FLAG_COUNT_TEXELS: population count of the texel bitmaps
+__global__ void k_popcount(const uint32_t* __restrict__ w, size_t n, unsigned long long* counter)
+{
+    unsigned long long c = 0;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) c += __popc(w[i]);
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xFFFFFFFFu, c, o);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(counter, c);
+}
+
+cudaError_t vs_launch_popcount(const uint32_t* words, size_t n, unsigned long long* counter, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    k_popcount<<<148 * 4, 256, 0, st>>>(words, n, counter);
     return cudaGetLastError();
 }
