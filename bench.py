@@ -176,16 +176,16 @@ def run_ours(args):
 
     sampler = ClockSampler(local) if rank == 0 else None
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    raster_ms = bin_ms = xf_ms = 0.0
-    raster_launches = launches = 0
+    shade_ms = raster_ms = bin_ms = xf_ms = 0.0
+    shade_launches = launches = 0
     vsdist.barrier()
     torch.cuda.synchronize()
     ev0.record(stream)
     for _ in range(args.steps):
         binding.vs_render(renderer.handle, sc.cameras, params, out)
-        st = renderer.stats()                      # syncs the stream; per-kernel CUDA-event times
-        raster_ms += st["ms_raster_shade"]; bin_ms += st["ms_binning"]; xf_ms += st["ms_transform"]
-        raster_launches += st["raster_launches"]; launches += st["kernel_launches"]
+        st = renderer.stats()                      # per-kernel CUDA-event times of the finished call
+        shade_ms += st["ms_shade"]; raster_ms += st["ms_raster"]; bin_ms += st["ms_binning"]; xf_ms += st["ms_transform"]
+        shade_launches += st["shade_launches"]; launches += st["kernel_launches"]
     ev1.record(stream)
     torch.cuda.synchronize()
     vsdist.barrier()
@@ -215,24 +215,31 @@ def run_ours(args):
         return 0
 
     peak, peak_src = load_peaks()
-    per_launch_ms = raster_ms / max(raster_launches, 1)
-    bytes_per_launch = alg_bytes_step * args.steps / max(raster_launches, 1)
+    # dominant kernel = k_shade: it moves the texture bytes and writes the framebuffer; its algorithmic
+    # bytes are B_tex + B_fb of the views one launch processes (B_geom belongs to the geometry kernels
+    # and is counted in `whole_step`, which divides ALL algorithmic bytes by the whole step's time).
+    per_launch_ms = shade_ms / max(shade_launches, 1)
+    bytes_per_launch = (b_tex + b_fb) * args.steps / max(shade_launches, 1)
     achieved = bytes_per_launch / (per_launch_ms * 1e-3) / 1e9 if per_launch_ms > 0 else 0.0
     step_achieved = alg_bytes_step * world / (secs_max / args.steps) / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_raster_shade", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"bound": "hbm", "kernel": "k_shade", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_per_launch,
-                "launch_ms": per_launch_ms, "kernel_share_of_step": raster_ms / (secs * 1e3),
+                "launch_ms": per_launch_ms, "views_per_launch": B * args.steps / max(shade_launches, 1),
+                "kernel_share_of_step": shade_ms / (secs * 1e3),
                 "bytes_per_view": {"texels_unique": b_tex / B, "geometry": b_geom / B, "framebuffer": b_fb / B},
-                "whole_step": {"achieved": step_achieved / world, "frac": step_achieved / world / peak},
+                "whole_step": {"achieved": step_achieved / world, "frac": step_achieved / world / peak,
+                               "algorithmic_bytes_per_step": alg_bytes_step},
                 "stage_ms_per_step": {"transform": xf_ms / args.steps, "binning": bin_ms / args.steps,
-                                      "raster_shade": raster_ms / args.steps}}
+                                      "raster": raster_ms / args.steps, "shade": shade_ms / args.steps}}
 
     cpu_baseline = None
     if world == 1 and not args.no_cpu:
         import oracle
-        nviews = args.cpu_views
-        t = time_oracle(sc, range(nviews))
+        nviews, t = 0, 0.0
+        while nviews < B and (t < args.cpu_seconds or nviews < 1):   # bounded sample: ~10 s of oracle work
+            t += time_oracle(sc, [nviews])
+            nviews += 1
         cpu_baseline = {"value": nviews * W * H / t / 1e6, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
                         "sample": "first %d of %d views of %s, %.1f s" % (nviews, B, sc.name, t)}
 
@@ -265,7 +272,7 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--views", type=int, default=0, help="override the number of views per step")
     ap.add_argument("--chunk", type=int, default=0, help="views per internal pass (0 = automatic)")
-    ap.add_argument("--cpu-views", type=int, default=2, help="views of the sample the oracle is timed on")
+    ap.add_argument("--cpu-seconds", type=float, default=10.0, help="oracle work of the cpu_baseline sample (whole views)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

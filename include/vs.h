@@ -109,12 +109,14 @@ typedef struct {
     uint64_t tile_refs;            /* (triangle, tile) pairs binned                                        */
     uint64_t scratch_bytes;        /* peak device scratch of the call                                      */
     uint64_t kernel_launches;      /* kernels launched by the call (memsets / copies not counted)          */
-    uint64_t raster_launches;      /* of which fused raster+shade kernels (one per chunk of cameras)       */
+    uint64_t raster_launches;      /* of which k_raster (one per chunk of cameras)                         */
+    uint64_t shade_launches;       /* of which k_shade  (one per chunk of cameras)                         */
     uint64_t shaded_fragments;     /* VS_FLAG_COUNT_TEXELS: (pixel, layer) fragments shaded                */
     uint64_t unique_texels;        /* VS_FLAG_COUNT_TEXELS: sum over views and layers of distinct texels   */
     double   ms_transform;         /* VS_FLAG_KERNEL_TIMING: device time per stage, summed over the call   */
     double   ms_binning;           /*   count + scan + scatter                                             */
-    double   ms_raster_shade;      /*   fused raster + shade + composite kernel                            */
+    double   ms_raster;            /*   coverage + nearest-fragment resolve kernel                         */
+    double   ms_shade;             /*   texel fetch + SH + composite kernel                                */
 } vs_render_stats;
 
 /*
@@ -138,10 +140,11 @@ vs_status vs_scene_create(const vs_scene_desc* desc, void* cuda_stream, vs_scene
  *   out_tri_ids  DEVICE [num_cameras][num_layers][height][width] uint32 or NULL: id of the nearest
  *                covering triangle of each layer, 0xFFFFFFFF = miss (the AOV the parity tests read).
  *
- *   All kernels are enqueued on `cuda_stream`; outputs are complete once that stream has drained.
- *   The call may block the host while it sizes scratch from the binning count pass (one small
- *   device->host read per chunk of cameras) but does not wait for the rendering itself.  Scratch is
- *   owned by the scene and reused between calls, so calls on one scene must not overlap in time.
+ *   All kernels are enqueued on `cuda_stream` without any host synchronisation in between; the call
+ *   then waits for that stream once, reads the counters back and returns with the outputs complete.
+ *   (The per-tile triangle-reference list is sized from earlier calls and checked on the device; if a
+ *   chunk of cameras needed more, the list is grown and the call renders again before returning.)
+ *   Scratch is owned by the scene and reused between calls, so calls on one scene must not overlap.
  */
 vs_status vs_render(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
                     const vs_render_params* params, float* out_rgba, uint32_t* out_tri_ids,
@@ -157,7 +160,7 @@ vs_status vs_render_host(vs_scene* scene, const vs_camera* cameras, uint32_t num
                          const vs_render_params* params, float* out_rgba, uint32_t* out_tri_ids,
                          void* cuda_stream);
 
-/* Counters of the last render on this scene; synchronises the stream that render used. */
+/* Counters of the last completed render on this scene. */
 vs_status vs_query_last_render(vs_scene* scene, vs_render_stats* out_stats);
 
 /* Frees all device memory of the scene after synchronising the device.  NULL is a no-op. */

@@ -55,8 +55,9 @@ class vs_render_params(C.Structure):
 class vs_render_stats(C.Structure):
     _fields_ = [("dropped_triangles", C.c_uint64), ("degenerate_triangles", C.c_uint64),
                 ("tile_refs", C.c_uint64), ("scratch_bytes", C.c_uint64), ("kernel_launches", C.c_uint64),
-                ("raster_launches", C.c_uint64), ("shaded_fragments", C.c_uint64), ("unique_texels", C.c_uint64),
-                ("ms_transform", C.c_double), ("ms_binning", C.c_double), ("ms_raster_shade", C.c_double)]
+                ("raster_launches", C.c_uint64), ("shade_launches", C.c_uint64), ("shaded_fragments", C.c_uint64),
+                ("unique_texels", C.c_uint64), ("ms_transform", C.c_double), ("ms_binning", C.c_double),
+                ("ms_raster", C.c_double), ("ms_shade", C.c_double)]
 
 
 _lib = None

@@ -52,26 +52,27 @@ struct vs_scene {
     int tex_f16 = 0;
     std::vector<void*> owned;
     // scratch, reused between calls
-    DevBuf cams, vtx, tile_count, tile_off, tile_cursor, tile_tris, counters, texel_bits, stage_rgba[2], stage_ids[2];
+    DevBuf cams, vtx, tri_tiles, tile_count, tile_off, tile_cursor, tile_tris, ids, counters, texel_bits, stage_rgba[2], stage_ids[2];
     // per-call bookkeeping
-    uint64_t launches = 0, raster_launches = 0;
+    uint64_t launches = 0, raster_launches = 0, shade_launches = 0;
     struct Span { cudaEvent_t a, b; int stage; };
     std::vector<Span> spans;        // VS_FLAG_KERNEL_TIMING: event pairs recorded this call
     std::vector<cudaEvent_t> event_pool;
     size_t events_used = 0;
-    uint32_t* host_total = nullptr;  // pinned
+    unsigned long long* host_counters = nullptr;  // pinned [VS_CNT_N]
     cudaStream_t last_stream = nullptr;
     cudaStream_t copy_stream = nullptr;
     cudaEvent_t ev_render[2] = {nullptr, nullptr}, ev_copy[2] = {nullptr, nullptr};
     size_t scratch_peak = 0;
+    size_t ref_capacity_wanted = 0;  // entries of tile_tris the next chunk asks for
     ~vs_scene()
     {
         for (void* p : owned) cudaFree(p);
-        DevBuf* bufs[] = {&cams, &vtx, &tile_count, &tile_off, &tile_cursor, &tile_tris, &counters, &texel_bits,
+        DevBuf* bufs[] = {&cams, &vtx, &tri_tiles, &tile_count, &tile_off, &tile_cursor, &tile_tris, &ids, &counters, &texel_bits,
                           &stage_rgba[0], &stage_rgba[1], &stage_ids[0], &stage_ids[1]};
         for (cudaEvent_t e : event_pool) cudaEventDestroy(e);
         for (DevBuf* b : bufs) b->release();
-        if (host_total) cudaFreeHost(host_total);
+        if (host_counters) cudaFreeHost(host_counters);
         if (copy_stream) cudaStreamDestroy(copy_stream);
         for (int i = 0; i < 2; ++i) {
             if (ev_render[i]) cudaEventDestroy(ev_render[i]);
@@ -184,7 +185,7 @@ static vs_status scene_create_impl(const vs_scene_desc* desc, cudaStream_t st, v
     if (hflag & 1u) return fail(VS_ERR_INVALID_ARG, "a triangle index is >= num_vertices of its layer");
     if (hflag & 2u) return fail(VS_ERR_INVALID_ARG, "a vertex position or uv is not finite");
     d.positions = pos; d.uvs = uvs; d.tris = tris;
-    CU(cudaHostAlloc((void**)&s->host_total, 64, cudaHostAllocDefault));
+    CU(cudaHostAlloc((void**)&s->host_counters, VS_CNT_N * 8, cudaHostAllocDefault));
     CU(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
     for (int i = 0; i < 2; ++i) {
         CU(cudaEventCreateWithFlags(&s->ev_render[i], cudaEventDisableTiming));
@@ -248,9 +249,10 @@ static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, u
 static uint32_t pick_chunk(const vs_scene* s, const vs_render_params* p, uint32_t n)
 {
     if (p->views_per_chunk) return p->views_per_chunk < n ? p->views_per_chunk : n;
-    // keep the per-chunk transformed vertices + outputs within a few hundred MB
-    const size_t per_view = (size_t)s->dev.v_total * 16 + (size_t)p->width * p->height * 4;
-    size_t c = (size_t)(256u << 20) / (per_view ? per_view : 1);
+    // keep the per-chunk scratch (transformed vertices, packed tile ranges, id planes) near 1 GB
+    const size_t per_view = (size_t)s->dev.v_total * 16 + (size_t)s->dev.t_total * 8 +
+                            (size_t)p->width * p->height * 4 * s->dev.k;
+    size_t c = ((size_t)1 << 30) / (per_view ? per_view : 1);
     if (c < 1) c = 1;
     if (c > 16) c = 16;
     return (uint32_t)(c < n ? c : n);
@@ -278,7 +280,7 @@ static vs_status span_end(vs_scene* s, bool on, cudaStream_t st)
     return VS_OK;
 }
 
-// Render `views` cameras starting at cams[0] into device outputs.  All work on `st`.
+// Render `views` cameras starting at cams[0] into device outputs.  All work on `st`, no host sync.
 static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views, const vs_render_params* p,
                               float* out_rgba, uint32_t* out_ids, cudaStream_t st)
 {
@@ -289,23 +291,38 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
     for (int i = 0; i < 3; ++i) fr.bg[i] = p->background[i];
     const size_t ntile = (size_t)views * fr.tiles_x * fr.tiles_y;
     if (ntile >= (1ull << 31)) return fail(VS_ERR_UNSUPPORTED, "too many tiles in one chunk");
+    const bool reference = (p->flags & VS_FLAG_REFERENCE_PATH) != 0;
+    const size_t id_words = (size_t)views * s->dev.k * p->width * p->height;
 
     CU(s->cams.reserve(sizeof(VsCamDev) * views));
     CU(s->vtx.reserve((size_t)s->dev.v_total * views * 16 + 16));
-    CU(s->tile_count.reserve(ntile * 4));
-    CU(s->tile_off.reserve((ntile + 1) * 4));
-    CU(s->tile_cursor.reserve(ntile * 4));
+    if (!reference) {
+        CU(s->tri_tiles.reserve((size_t)s->dev.t_total * views * 4 + 16));
+        CU(s->tile_count.reserve(ntile * 4));
+        CU(s->tile_off.reserve((ntile + 1) * 4));
+        CU(s->tile_cursor.reserve(ntile * 4));
+        // the reference list is sized from what earlier calls needed (or a first guess) and CHECKED:
+        // k_scan records the chunk's need when it exceeds the capacity and vs_render then retries
+        if (s->ref_capacity_wanted < 1024) s->ref_capacity_wanted = 1024;
+        CU(s->tile_tris.reserve(s->ref_capacity_wanted * 4));
+        if (!out_ids) CU(s->ids.reserve(id_words * 4 + 16));
+    }
 
     VsChunk ch{};
     ch.views = views;
     ch.cams = (const VsCamDev*)s->cams.p;
     ch.vtx = (int4*)s->vtx.p;
+    ch.tri_tiles = (uint32_t*)s->tri_tiles.p;
     ch.tile_count = (uint32_t*)s->tile_count.p;
     ch.tile_off = (uint32_t*)s->tile_off.p;
     ch.tile_cursor = (uint32_t*)s->tile_cursor.p;
+    ch.tile_tris = (uint32_t*)s->tile_tris.p;
+    const size_t cap = s->tile_tris.cap / 4;
+    ch.ref_capacity = cap > 0xFFFFFFFFull ? 0xFFFFFFFFu : (uint32_t)cap;
     ch.counters = (unsigned long long*)s->counters.p;
     ch.out_rgba = out_rgba;
-    ch.out_ids = out_ids;
+    ch.ids = out_ids ? out_ids : (uint32_t*)s->ids.p;
+    ch.ids_is_output = out_ids != nullptr;
 
     static_assert(sizeof(VsCamDev) == sizeof(vs_camera), "camera layout");
     const bool timing = (p->flags & VS_FLAG_KERNEL_TIMING) != 0;
@@ -315,23 +332,13 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
     CU(vs_launch_transform(s->dev, fr, ch, st));
     if ((r = span_end(s, timing, st)) != VS_OK) return r;
     s->launches += 1;
-    if (p->flags & VS_FLAG_REFERENCE_PATH) {
+    if (reference) {
         CU(vs_launch_reference(s->dev, s->tex_f16, fr, ch, st));
         s->launches += 1;
         return VS_OK;
     }
     CU(cudaMemsetAsync(ch.tile_count, 0, ntile * 4, st));
     CU(cudaMemsetAsync(ch.tile_cursor, 0, ntile * 4, st));
-    if ((r = span_begin(s, timing, 1, st)) != VS_OK) return r;
-    CU(vs_launch_bin_count(s->dev, fr, ch, st));
-    CU(vs_launch_bin_scan(fr, ch, st));
-    if ((r = span_end(s, timing, st)) != VS_OK) return r;
-    // size the reference list from the count pass (one 4-byte read)
-    CU(cudaMemcpyAsync(s->host_total, ch.tile_off + ntile, 4, cudaMemcpyDeviceToHost, st));
-    CU(cudaStreamSynchronize(st));
-    const size_t total = *s->host_total;
-    CU(s->tile_tris.reserve(total * 4 + 16));
-    ch.tile_tris = (uint32_t*)s->tile_tris.p;
     if (p->flags & VS_FLAG_COUNT_TEXELS) {
         const size_t words = (size_t)views * (s->dev.tex_bit_off[s->dev.k] >> 5);
         CU(s->texel_bits.reserve(words * 4 + 16));
@@ -339,18 +346,26 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
         ch.texel_bits = (uint32_t*)s->texel_bits.p;
     }
     if ((r = span_begin(s, timing, 1, st)) != VS_OK) return r;
+    CU(vs_launch_bin_count(s->dev, fr, ch, st));
+    CU(vs_launch_bin_scan(fr, ch, st));
     CU(vs_launch_bin_scatter(s->dev, fr, ch, st));
     if ((r = span_end(s, timing, st)) != VS_OK) return r;
     if ((r = span_begin(s, timing, 2, st)) != VS_OK) return r;
-    CU(vs_launch_raster_shade(s->dev, s->tex_f16, fr, ch, st));
+    CU(vs_launch_raster(s->dev, fr, ch, st));
     if ((r = span_end(s, timing, st)) != VS_OK) return r;
-    s->launches += 4;
+    if ((r = span_begin(s, timing, 3, st)) != VS_OK) return r;
+    CU(vs_launch_shade(s->dev, s->tex_f16, fr, ch, st));
+    if ((r = span_end(s, timing, st)) != VS_OK) return r;
+    s->launches += (s->dev.t_total ? 3 : 1) + 2;
     s->raster_launches += 1;
+    s->shade_launches += 1;
     if (ch.texel_bits) {
         CU(vs_launch_popcount(ch.texel_bits, (size_t)views * (s->dev.tex_bit_off[s->dev.k] >> 5),
                               ch.counters + VS_CNT_TEXELS, st));
+        s->launches += 1;
     }
-    const size_t scratch = s->cams.cap + s->vtx.cap + s->tile_count.cap + s->tile_off.cap + s->tile_cursor.cap + s->tile_tris.cap;
+    const size_t scratch = s->cams.cap + s->vtx.cap + s->tri_tiles.cap + s->tile_count.cap + s->tile_off.cap +
+                           s->tile_cursor.cap + s->tile_tris.cap + s->ids.cap;
     if (scratch > s->scratch_peak) s->scratch_peak = scratch;
     return VS_OK;
 }
@@ -362,10 +377,28 @@ static vs_status begin_render(vs_scene* s, cudaStream_t st)
     CU(cudaMemsetAsync(s->counters.p, 0, VS_CNT_N * 8, st));
     s->last_stream = st;
     s->scratch_peak = 0;
-    s->launches = s->raster_launches = 0;
+    s->launches = s->raster_launches = s->shade_launches = 0;
     s->spans.clear();
     s->events_used = 0;
     return VS_OK;
+}
+
+// Waits for the call's kernels and reads the counters back.  *retry is set when a chunk needed more
+// triangle references than the list could hold (the images are then incomplete): the capacity is
+// raised to what was needed and the caller renders again.
+static vs_status finish_render(vs_scene* s, cudaStream_t st, bool* retry)
+{
+    CU(cudaMemcpyAsync(s->host_counters, s->counters.p, VS_CNT_N * 8, cudaMemcpyDeviceToHost, st));
+    CU(cudaStreamSynchronize(st));
+    const unsigned long long need = s->host_counters[VS_CNT_OVERFLOW];
+    *retry = need != 0;
+    if (need) s->ref_capacity_wanted = (size_t)(need + need / 4 + 1024);
+    return VS_OK;
+}
+
+static void first_capacity_guess(vs_scene* s, uint32_t chunk)
+{
+    if (s->ref_capacity_wanted == 0) s->ref_capacity_wanted = (size_t)2 * s->dev.t_total * chunk + 65536;
 }
 
 extern "C" vs_status vs_render(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
@@ -376,17 +409,23 @@ extern "C" vs_status vs_render(vs_scene* scene, const vs_camera* cameras, uint32
     vs_status r = validate_render(scene, cameras, num_cameras, params, out_rgba);
     if (r != VS_OK) return r;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if ((r = begin_render(scene, st)) != VS_OK) return r;
-    if (num_cameras == 0) return VS_OK;
     const uint32_t chunk = pick_chunk(scene, params, num_cameras);
     const size_t px = (size_t)params->width * params->height;
-    for (uint32_t v0 = 0; v0 < num_cameras; v0 += chunk) {
-        const uint32_t nv = num_cameras - v0 < chunk ? num_cameras - v0 : chunk;
-        r = render_chunk(scene, cameras + v0, nv, params, out_rgba + (size_t)v0 * px * 4,
-                         out_tri_ids ? out_tri_ids + (size_t)v0 * scene->dev.k * px : nullptr, st);
-        if (r != VS_OK) return r;
+    first_capacity_guess(scene, chunk);
+    for (int attempt = 0; attempt < 4; ++attempt) {
+        if ((r = begin_render(scene, st)) != VS_OK) return r;
+        if (num_cameras == 0) return VS_OK;
+        for (uint32_t v0 = 0; v0 < num_cameras; v0 += chunk) {
+            const uint32_t nv = num_cameras - v0 < chunk ? num_cameras - v0 : chunk;
+            r = render_chunk(scene, cameras + v0, nv, params, out_rgba + (size_t)v0 * px * 4,
+                             out_tri_ids ? out_tri_ids + (size_t)v0 * scene->dev.k * px : nullptr, st);
+            if (r != VS_OK) return r;
+        }
+        bool retry = false;
+        if ((r = finish_render(scene, st, &retry)) != VS_OK) return r;
+        if (!retry) return VS_OK;
     }
-    return VS_OK;
+    return fail(VS_ERR_CUDA, "triangle reference list kept overflowing");
 }
 
 extern "C" vs_status vs_render_host(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
@@ -397,34 +436,39 @@ extern "C" vs_status vs_render_host(vs_scene* scene, const vs_camera* cameras, u
     vs_status r = validate_render(scene, cameras, num_cameras, params, out_rgba);
     if (r != VS_OK) return r;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if ((r = begin_render(scene, st)) != VS_OK) return r;
-    if (num_cameras == 0) return VS_OK;
     const uint32_t chunk = pick_chunk(scene, params, num_cameras);
     const size_t px = (size_t)params->width * params->height;
     const size_t rgba_bytes = px * 16, ids_bytes = px * 4 * scene->dev.k;
-    uint32_t b = 0;
-    bool used[2] = {false, false};
-    for (uint32_t v0 = 0; v0 < num_cameras; v0 += chunk, b ^= 1u) {
-        const uint32_t nv = num_cameras - v0 < chunk ? num_cameras - v0 : chunk;
-        CU(scene->stage_rgba[b].reserve(rgba_bytes * chunk));
-        if (out_tri_ids) CU(scene->stage_ids[b].reserve(ids_bytes * chunk));
-        if (used[b]) CU(cudaStreamWaitEvent(st, scene->ev_copy[b], 0));  // staging buffer b is free again
-        r = render_chunk(scene, cameras + v0, nv, params, (float*)scene->stage_rgba[b].p,
-                         out_tri_ids ? (uint32_t*)scene->stage_ids[b].p : nullptr, st);
-        if (r != VS_OK) return r;
-        CU(cudaEventRecord(scene->ev_render[b], st));
-        CU(cudaStreamWaitEvent(scene->copy_stream, scene->ev_render[b], 0));
-        CU(cudaMemcpyAsync(out_rgba + (size_t)v0 * px * 4, scene->stage_rgba[b].p, rgba_bytes * nv, cudaMemcpyDeviceToHost,
-                           scene->copy_stream));
-        if (out_tri_ids)
-            CU(cudaMemcpyAsync(out_tri_ids + (size_t)v0 * scene->dev.k * px, scene->stage_ids[b].p, ids_bytes * nv,
-                               cudaMemcpyDeviceToHost, scene->copy_stream));
-        CU(cudaEventRecord(scene->ev_copy[b], scene->copy_stream));
-        used[b] = true;
+    first_capacity_guess(scene, chunk);
+    for (int attempt = 0; attempt < 4; ++attempt) {
+        if ((r = begin_render(scene, st)) != VS_OK) return r;
+        if (num_cameras == 0) return VS_OK;
+        uint32_t b = 0;
+        bool used[2] = {false, false};
+        for (uint32_t v0 = 0; v0 < num_cameras; v0 += chunk, b ^= 1u) {
+            const uint32_t nv = num_cameras - v0 < chunk ? num_cameras - v0 : chunk;
+            CU(scene->stage_rgba[b].reserve(rgba_bytes * chunk));
+            if (out_tri_ids) CU(scene->stage_ids[b].reserve(ids_bytes * chunk));
+            if (used[b]) CU(cudaStreamWaitEvent(st, scene->ev_copy[b], 0));  // staging buffer b is free again
+            r = render_chunk(scene, cameras + v0, nv, params, (float*)scene->stage_rgba[b].p,
+                             out_tri_ids ? (uint32_t*)scene->stage_ids[b].p : nullptr, st);
+            if (r != VS_OK) return r;
+            CU(cudaEventRecord(scene->ev_render[b], st));
+            CU(cudaStreamWaitEvent(scene->copy_stream, scene->ev_render[b], 0));
+            CU(cudaMemcpyAsync(out_rgba + (size_t)v0 * px * 4, scene->stage_rgba[b].p, rgba_bytes * nv, cudaMemcpyDeviceToHost,
+                               scene->copy_stream));
+            if (out_tri_ids)
+                CU(cudaMemcpyAsync(out_tri_ids + (size_t)v0 * scene->dev.k * px, scene->stage_ids[b].p, ids_bytes * nv,
+                                   cudaMemcpyDeviceToHost, scene->copy_stream));
+            CU(cudaEventRecord(scene->ev_copy[b], scene->copy_stream));
+            used[b] = true;
+        }
+        bool retry = false;
+        if ((r = finish_render(scene, st, &retry)) != VS_OK) return r;
+        CU(cudaStreamSynchronize(scene->copy_stream));
+        if (!retry) return VS_OK;
     }
-    CU(cudaStreamSynchronize(scene->copy_stream));
-    CU(cudaStreamSynchronize(st));
-    return VS_OK;
+    return fail(VS_ERR_CUDA, "triangle reference list kept overflowing");
 }
 
 extern "C" vs_status vs_query_last_render(vs_scene* scene, vs_render_stats* out)
@@ -435,20 +479,20 @@ extern "C" vs_status vs_query_last_render(vs_scene* scene, vs_render_stats* out)
     if (!scene->counters.p) return VS_OK;
     CU(cudaSetDevice(scene->device));
     CU(cudaStreamSynchronize(scene->last_stream));
-    unsigned long long h[VS_CNT_N];
-    CU(cudaMemcpy(h, scene->counters.p, sizeof(h), cudaMemcpyDeviceToHost));
+    const unsigned long long* h = scene->host_counters;  // read back by finish_render
     out->dropped_triangles = h[VS_CNT_DROPPED];
     out->degenerate_triangles = h[VS_CNT_DEGENERATE];
     out->tile_refs = h[VS_CNT_REFS];
     out->scratch_bytes = scene->scratch_peak;
     out->kernel_launches = scene->launches;
     out->raster_launches = scene->raster_launches;
+    out->shade_launches = scene->shade_launches;
     out->shaded_fragments = h[VS_CNT_FRAGS];
     out->unique_texels = h[VS_CNT_TEXELS];
     for (const vs_scene::Span& sp : scene->spans) {
         float ms = 0.0f;
         CU(cudaEventElapsedTime(&ms, sp.a, sp.b));
-        (sp.stage == 0 ? out->ms_transform : sp.stage == 1 ? out->ms_binning : out->ms_raster_shade) += ms;
+        (sp.stage == 0 ? out->ms_transform : sp.stage == 1 ? out->ms_binning : sp.stage == 2 ? out->ms_raster : out->ms_shade) += ms;
     }
     return VS_OK;
 }

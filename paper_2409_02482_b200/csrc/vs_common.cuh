@@ -39,8 +39,9 @@ struct VsFrame {
     float bg[3];
 };
 
-// counters[0] dropped, [1] degenerate, [2] tile refs, [3] shaded fragments, [4] unique texels
-enum { VS_CNT_DROPPED = 0, VS_CNT_DEGENERATE = 1, VS_CNT_REFS = 2, VS_CNT_FRAGS = 3, VS_CNT_TEXELS = 4, VS_CNT_N = 8 };
+// counters[0] dropped, [1] degenerate, [2] tile refs, [3] shaded fragments, [4] unique texels,
+// [5] max over chunks of the references a chunk needed when that exceeded ref_capacity (0 = no overflow)
+enum { VS_CNT_DROPPED = 0, VS_CNT_DEGENERATE = 1, VS_CNT_REFS = 2, VS_CNT_FRAGS = 3, VS_CNT_TEXELS = 4, VS_CNT_OVERFLOW = 5, VS_CNT_N = 8 };
 
 // ---- triangle setup shared by the binning, raster and shading kernels ----------
 struct VsTri {
@@ -176,18 +177,63 @@ __device__ __forceinline__ float vs_sigmoid(float s)
     return __fdividef(1.0f, 1.0f + __expf(-s));
 }
 
+// ---- fragment setup (S5 addressing): winning triangle of a layer at pixel
+// (px, py) -> clamped texel columns / rows of the 2x2 footprint and the bilinear fractions.
+struct VsFrag {
+    uint32_t cx0, cx1, cy0, cy1;
+    float a, b;
+};
+
+__device__ __forceinline__ void vs_texel_coord(float u0, float du, float fW, int Wt, uint32_t& c0, uint32_t& c1, float& frac)
+{
+    // texel coordinate = (u0 W - 0.5) + du W, carried as integer + fraction so that the fraction
+    // keeps full fp32 resolution at 4096^2 (u0 W is split into its rounded product and the FMA residual)
+    const float ph = __fmul_rn(u0, fW), pl = __fmaf_rn(u0, fW, -ph);
+    const float x0 = fminf(fmaxf(ph - 0.5f, -1048576.0f), 1048576.0f);
+    const float fl = floorf(x0);
+    const float t = ((x0 - fl) + pl) + du * fW;
+    const float ft = floorf(t);
+    frac = t - ft;
+    const int i0 = __float2int_rd(fl) + __float2int_rd(ft);
+    c0 = (uint32_t)min(max(i0, 0), Wt - 1);
+    c1 = (uint32_t)min(max(i0 + 1, 0), Wt - 1);
+}
+
+__device__ __forceinline__ void vs_fragment_setup(const VsSceneDev& sc, const int4* __restrict__ vv, uint32_t l,
+                                                  uint32_t local_tri, int px, int py, VsFrag& f)
+{
+    const uint4 tri = __ldg(&sc.tris[sc.tri_off[l] + local_tri]);
+    const int4 a = __ldg(&vv[tri.x]), b = __ldg(&vv[tri.y]), c = __ldg(&vv[tri.z]);
+    const float2 uva = __ldg(&sc.uvs[tri.x]), uvb = __ldg(&sc.uvs[tri.y]), uvc = __ldg(&sc.uvs[tri.z]);
+    VsTri T;
+    vs_setup_tri(a, b, c, T);
+    const float2 uv0 = uva, uv1 = T.swapped ? uvc : uvb, uv2 = T.swapped ? uvb : uvc;
+    VsEdges e;
+    vs_edges_at(T, px, py, e);
+    // perspective-correct barycentrics b'_i ~ E_i q_i
+    const float g0 = __ll2float_rn(e.E0) * T.q0, g1 = __ll2float_rn(e.E1) * T.q1, g2 = __ll2float_rn(e.E2) * T.q2;
+    const float inv = __fdividef(1.0f, g0 + g1 + g2);
+    const float b1 = g1 * inv, b2 = g2 * inv;
+    const int Wt = (int)sc.tex_w[l], Ht = (int)sc.tex_h[l];
+    vs_texel_coord(uv0.x, b1 * (uv1.x - uv0.x) + b2 * (uv2.x - uv0.x), (float)Wt, Wt, f.cx0, f.cx1, f.a);
+    vs_texel_coord(uv0.y, b1 * (uv1.y - uv0.y) + b2 * (uv2.y - uv0.y), (float)Ht, Ht, f.cy0, f.cy1, f.b);
+}
+
 // ---- host-side launchers (vs_kernels_*.cu) ------------------------------------------------------
 struct VsChunk {                 // one pass over `views` cameras
     uint32_t views;
     const VsCamDev* cams;        // DEVICE [views]
     int4* vtx;                   // DEVICE [views][v_total]
+    uint32_t* tri_tiles;         // DEVICE [views][t_total] packed tile range of each triangle (count pass output)
     uint32_t* tile_count;        // DEVICE [views * tiles]   (count pass output)
-    uint32_t* tile_off;          // DEVICE [views * tiles + 1] exclusive scan
+    uint32_t* tile_off;          // DEVICE [views * tiles + 1] exclusive scan; [views*tiles] = total references
     uint32_t* tile_cursor;       // DEVICE [views * tiles]   scatter cursors
-    uint32_t* tile_tris;         // DEVICE [total refs]
+    uint32_t* tile_tris;         // DEVICE [ref_capacity]
+    uint32_t ref_capacity;       // entries of tile_tris; references past it are dropped and flagged
     unsigned long long* counters;  // DEVICE [VS_CNT_N]
+    uint32_t* ids;               // DEVICE [views][k][H][W] nearest triangle per (pixel, layer)
+    int ids_is_output;           // ids is the caller's AOV: empty tiles must be filled with MISS too
     float* out_rgba;             // DEVICE [views][H][W][4]
-    uint32_t* out_ids;           // DEVICE [views][k][H][W] or nullptr
     uint32_t* texel_bits;        // DEVICE [views][tex_bit_off[k] / 32] or nullptr (VS_FLAG_COUNT_TEXELS)
 };
 
@@ -195,7 +241,8 @@ cudaError_t vs_launch_transform(const VsSceneDev& sc, const VsFrame& fr, const V
 cudaError_t vs_launch_bin_count(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_bin_scan(const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_bin_scatter(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
-cudaError_t vs_launch_raster_shade(const VsSceneDev& sc, int tex_f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_raster(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_shade(const VsSceneDev& sc, int tex_f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_popcount(const uint32_t* words, size_t n, unsigned long long* counter, cudaStream_t st);
 cudaError_t vs_launch_reference(const VsSceneDev& sc, int tex_f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 

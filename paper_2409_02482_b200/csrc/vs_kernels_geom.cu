@@ -100,49 +100,110 @@ cudaError_t vs_launch_transform(const VsSceneDev& sc, const VsFrame& fr, const V
 }
 
 // ------------------------------------------------------------------------------------------------
-// S2 + S3: triangle setup and tile binning.  One thread per (view, triangle); the same code runs
-// twice: COUNT (atomicAdd on the tile counters) and SCATTER (claim a slot, write the triangle id).
-// A triangle is referenced by every tile its sample-point bounding box touches.
+// S2 + S3: triangle setup and tile binning.  One thread per (view, triangle).
+//   k_bin_count  : setup, sample bounding box -> tile range; remembers the packed range per
+//                  (view, triangle) and counts references per (view, tile).
+//   k_scan       : exclusive prefix sum of the counters of the whole chunk.
+//   k_bin_scatter: re-reads the packed range (no vertex gathers) and writes the triangle id into
+//                  the tile's list.
+// A triangle is referenced by every tile its sample-point bounding box touches.  Consecutive
+// triangles of a mesh mostly fall into the same tile, so the tile atomics are warp-aggregated:
+// lanes that target the same tile elect a leader (match.any) which adds the group's size once.
 // ------------------------------------------------------------------------------------------------
-template <bool SCATTER>
-__global__ void __launch_bounds__(256) k_bin(VsSceneDev sc, VsFrame fr, const int4* __restrict__ vtx,
-                                             uint32_t* __restrict__ tile_counter, const uint32_t* __restrict__ tile_off,
-                                             uint32_t* __restrict__ tile_tris, unsigned long long* counters)
+#define VS_RANGE_NONE 0xFFFFFFFFu   // triangle references no tile
+#define VS_RANGE_WIDE 0xFFFFFFFEu   // more than 64 tiles in one direction: the scatter pass recomputes the range
+
+__device__ __forceinline__ bool vs_tile_range(const VsSceneDev& sc, const VsFrame& fr, const int4* __restrict__ vv, uint32_t t,
+                                              int& tx0, int& tx1, int& ty0, int& ty1, int& status)
 {
-    uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
+    const uint4 tri = __ldg(&sc.tris[t]);
+    const int4 a = __ldg(&vv[tri.x]), b = __ldg(&vv[tri.y]), c = __ldg(&vv[tri.z]);
+    VsTri T;
+    status = vs_setup_tri(a, b, c, T);
+    int i0, i1, j0, j1;
+    if (status != 0 || !vs_tri_pixel_bbox(T, (int)fr.width, (int)fr.height, i0, i1, j0, j1)) return false;
+    tx0 = i0 / VS_TILE_W; tx1 = i1 / VS_TILE_W; ty0 = j0 / VS_TILE_H; ty1 = j1 / VS_TILE_H;
+    return true;
+}
+
+// Adds 1 to counter[tile] for every lane with `single` set, one atomic per distinct tile of the warp.
+// Returns the lane's slot (value of the counter before its own increment).  All 32 lanes must call.
+__device__ __forceinline__ uint32_t vs_warp_tile_add(uint32_t* __restrict__ counter, bool single, uint32_t tile, uint32_t lane)
+{
+    const uint32_t key = single ? tile : (0x80000000u | lane);
+    const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key);
+    const int leader = __ffs(peers) - 1;
+    uint32_t base = 0;
+    if (single && (int)lane == leader) base = atomicAdd(&counter[tile], (uint32_t)__popc(peers));
+    base = __shfl_sync(0xFFFFFFFFu, base, leader);
+    return base + (uint32_t)__popc(peers & ((1u << lane) - 1u));
+}
+
+__global__ void __launch_bounds__(256) k_bin_count(VsSceneDev sc, VsFrame fr, const int4* __restrict__ vtx,
+                                                   uint32_t* __restrict__ tri_tiles, uint32_t* __restrict__ tile_count,
+                                                   unsigned long long* counters)
+{
+    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
     const uint32_t view = blockIdx.y;
-    int status = -1;
-    uint32_t refs = 0;
-    if (t < sc.t_total) {
-        const uint4 tri = __ldg(&sc.tris[t]);
-        const int4* vv = vtx + (size_t)view * sc.v_total;
-        const int4 a = __ldg(&vv[tri.x]), b = __ldg(&vv[tri.y]), c = __ldg(&vv[tri.z]);
-        VsTri T;
-        status = vs_setup_tri(a, b, c, T);
-        int i0, i1, j0, j1;
-        if (status == 0 && vs_tri_pixel_bbox(T, (int)fr.width, (int)fr.height, i0, i1, j0, j1)) {
-            const int tx0 = i0 / VS_TILE_W, tx1 = i1 / VS_TILE_W, ty0 = j0 / VS_TILE_H, ty1 = j1 / VS_TILE_H;
-            const uint32_t tiles = fr.tiles_x * fr.tiles_y;
-            for (int ty = ty0; ty <= ty1; ++ty)
-                for (int tx = tx0; tx <= tx1; ++tx) {
-                    const uint32_t tile = view * tiles + (uint32_t)ty * fr.tiles_x + (uint32_t)tx;
-                    const uint32_t slot = atomicAdd(&tile_counter[tile], 1u);
-                    if (SCATTER) tile_tris[tile_off[tile] + slot] = t;
-                    ++refs;
-                }
-        }
+    const uint32_t tiles = fr.tiles_x * fr.tiles_y;
+    int status = -1, tx0 = 0, tx1 = -1, ty0 = 0, ty1 = -1;
+    bool any = false;
+    if (t < sc.t_total) any = vs_tile_range(sc, fr, vtx + (size_t)view * sc.v_total, t, tx0, tx1, ty0, ty1, status);
+    const int nx = tx1 - tx0 + 1, ny = ty1 - ty0 + 1;
+    uint32_t packed = VS_RANGE_NONE, refs = 0;
+    if (any) {
+        packed = (nx > 64 || ny > 64) ? VS_RANGE_WIDE
+                                      : ((uint32_t)tx0 | ((uint32_t)ty0 << 10) | ((uint32_t)(nx - 1) << 20) | ((uint32_t)(ny - 1) << 26));
+        refs = (uint32_t)(nx * ny);
     }
-    if (!SCATTER) {
-        // warp-aggregated statistics
-        const unsigned full = 0xFFFFFFFFu;
-        unsigned dropped = __popc(__ballot_sync(full, status == 1));
-        unsigned degen = __popc(__ballot_sync(full, status == 2));
-        for (int o = 16; o > 0; o >>= 1) refs += __shfl_xor_sync(full, refs, o);
-        if ((threadIdx.x & 31) == 0) {
-            if (dropped) atomicAdd(&counters[VS_CNT_DROPPED], (unsigned long long)dropped);
-            if (degen) atomicAdd(&counters[VS_CNT_DEGENERATE], (unsigned long long)degen);
-            if (refs) atomicAdd(&counters[VS_CNT_REFS], (unsigned long long)refs);
-        }
+    if (t < sc.t_total) tri_tiles[(size_t)view * sc.t_total + t] = packed;
+    const bool single = any && refs == 1;
+    vs_warp_tile_add(tile_count, single, view * tiles + (uint32_t)ty0 * fr.tiles_x + (uint32_t)tx0, lane);
+    if (any && !single)
+        for (int ty = ty0; ty <= ty1; ++ty)
+            for (int tx = tx0; tx <= tx1; ++tx) atomicAdd(&tile_count[view * tiles + (uint32_t)ty * fr.tiles_x + (uint32_t)tx], 1u);
+    // warp-aggregated statistics
+    const unsigned full = 0xFFFFFFFFu;
+    const unsigned dropped = __popc(__ballot_sync(full, status == 1));
+    const unsigned degen = __popc(__ballot_sync(full, status == 2));
+    refs = __reduce_add_sync(full, refs);
+    if (lane == 0) {
+        if (dropped) atomicAdd(&counters[VS_CNT_DROPPED], (unsigned long long)dropped);
+        if (degen) atomicAdd(&counters[VS_CNT_DEGENERATE], (unsigned long long)degen);
+        if (refs) atomicAdd(&counters[VS_CNT_REFS], (unsigned long long)refs);
+    }
+}
+
+__global__ void __launch_bounds__(256) k_bin_scatter(VsSceneDev sc, VsFrame fr, const int4* __restrict__ vtx,
+                                                     const uint32_t* __restrict__ tri_tiles, uint32_t* __restrict__ tile_cursor,
+                                                     const uint32_t* __restrict__ tile_off, uint32_t* __restrict__ tile_tris,
+                                                     uint32_t ref_capacity)
+{
+    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    const uint32_t view = blockIdx.y;
+    const uint32_t tiles = fr.tiles_x * fr.tiles_y;
+    const uint32_t packed = t < sc.t_total ? __ldg(&tri_tiles[(size_t)view * sc.t_total + t]) : VS_RANGE_NONE;
+    int tx0 = 0, tx1 = -1, ty0 = 0, ty1 = -1;
+    if (packed == VS_RANGE_WIDE) {
+        int status;
+        vs_tile_range(sc, fr, vtx + (size_t)view * sc.v_total, t, tx0, tx1, ty0, ty1, status);
+    } else if (packed != VS_RANGE_NONE) {
+        tx0 = (int)(packed & 1023u); ty0 = (int)((packed >> 10) & 1023u);
+        tx1 = tx0 + (int)((packed >> 20) & 63u); ty1 = ty0 + (int)(packed >> 26);
+    }
+    const bool any = tx1 >= tx0, single = any && tx0 == tx1 && ty0 == ty1;
+    const uint32_t tile0 = view * tiles + (uint32_t)ty0 * fr.tiles_x + (uint32_t)tx0;
+    const uint32_t slot = vs_warp_tile_add(tile_cursor, single, tile0, lane);
+    if (single) {
+        const uint32_t pos = __ldg(&tile_off[tile0]) + slot;
+        if (pos < ref_capacity) tile_tris[pos] = t;
+    } else if (any) {
+        for (int ty = ty0; ty <= ty1; ++ty)
+            for (int tx = tx0; tx <= tx1; ++tx) {
+                const uint32_t tile = view * tiles + (uint32_t)ty * fr.tiles_x + (uint32_t)tx;
+                const uint32_t pos = __ldg(&tile_off[tile]) + atomicAdd(&tile_cursor[tile], 1u);
+                if (pos < ref_capacity) tile_tris[pos] = t;
+            }
     }
 }
 
@@ -150,7 +211,7 @@ cudaError_t vs_launch_bin_count(const VsSceneDev& sc, const VsFrame& fr, const V
 {
     if (sc.t_total == 0) return cudaSuccess;
     dim3 grid((sc.t_total + 255) / 256, ch.views);
-    k_bin<false><<<grid, 256, 0, st>>>(sc, fr, ch.vtx, ch.tile_count, nullptr, nullptr, ch.counters);
+    k_bin_count<<<grid, 256, 0, st>>>(sc, fr, ch.vtx, ch.tri_tiles, ch.tile_count, ch.counters);
     return cudaGetLastError();
 }
 
@@ -158,47 +219,61 @@ cudaError_t vs_launch_bin_scatter(const VsSceneDev& sc, const VsFrame& fr, const
 {
     if (sc.t_total == 0) return cudaSuccess;
     dim3 grid((sc.t_total + 255) / 256, ch.views);
-    k_bin<true><<<grid, 256, 0, st>>>(sc, fr, ch.vtx, ch.tile_cursor, ch.tile_off, ch.tile_tris, ch.counters);
+    k_bin_scatter<<<grid, 256, 0, st>>>(sc, fr, ch.vtx, ch.tri_tiles, ch.tile_cursor, ch.tile_off, ch.tile_tris, ch.ref_capacity);
     return cudaGetLastError();
 }
 
-// Exclusive prefix sum of the tile counters of the whole chunk: one 1024-thread block, each thread
-// scans a contiguous run serially, warp-shuffle scan across the threads.  off[n] = total.
-__global__ void __launch_bounds__(1024) k_scan(const uint32_t* __restrict__ count, uint32_t n, uint32_t* __restrict__ off)
+// Exclusive prefix sum of the tile counters of the whole chunk, off[n] = total.  One 1024-thread
+// block per view: the block first sums the counters of all earlier views (its base; no block waits
+// on another), then scans its own view in coalesced 1024-element pieces with warp-shuffle scans.
+__device__ __forceinline__ uint32_t vs_block_scan_1024(uint32_t v, uint32_t* warp_sums, uint32_t& total)
 {
-    __shared__ uint32_t warp_sums[32];
-    const uint32_t tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const uint32_t per = (n + 1023) / 1024;
-    const uint32_t begin = min(tid * per, n), end = min(begin + per, n);
-    uint32_t sum = 0;
-    for (uint32_t i = begin; i < end; ++i) sum += count[i];
-    uint32_t incl = sum;
+    const uint32_t lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    uint32_t incl = v;
     for (int o = 1; o < 32; o <<= 1) {
-        uint32_t v = __shfl_up_sync(0xFFFFFFFFu, incl, o);
-        if (lane >= (uint32_t)o) incl += v;
+        const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (lane >= (uint32_t)o) incl += u;
     }
+    __syncthreads();  // warp_sums may still be read from the previous call
     if (lane == 31) warp_sums[wid] = incl;
     __syncthreads();
-    if (wid == 0) {
-        uint32_t w = warp_sums[lane], wi = w;
-        for (int o = 1; o < 32; o <<= 1) {
-            uint32_t v = __shfl_up_sync(0xFFFFFFFFu, wi, o);
-            if (lane >= (uint32_t)o) wi += v;
-        }
-        warp_sums[lane] = wi - w;  // exclusive
+    uint32_t w = warp_sums[lane], wi = w;
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, wi, o);
+        if (lane >= (uint32_t)o) wi += u;
     }
-    __syncthreads();
-    uint32_t run = warp_sums[wid] + incl - sum;
-    for (uint32_t i = begin; i < end; ++i) {
-        off[i] = run;
-        run += count[i];
+    total = __shfl_sync(0xFFFFFFFFu, wi, 31);
+    const uint32_t wbase = __shfl_sync(0xFFFFFFFFu, wi - w, wid);
+    return wbase + incl - v;  // exclusive
+}
+
+__global__ void __launch_bounds__(1024) k_scan(const uint32_t* __restrict__ count, uint32_t tiles, uint32_t views,
+                                               uint32_t* __restrict__ off, uint32_t ref_capacity, unsigned long long* counters)
+{
+    __shared__ uint32_t warp_sums[32];
+    const uint32_t view = blockIdx.x, tid = threadIdx.x;
+    uint32_t mine = 0;
+    for (uint32_t i = tid; i < view * tiles; i += 1024) mine += __ldg(&count[i]);
+    uint32_t base;
+    vs_block_scan_1024(mine, warp_sums, base);
+    const uint32_t* c = count + (size_t)view * tiles;
+    uint32_t* o = off + (size_t)view * tiles;
+    for (uint32_t i0 = 0; i0 < tiles; i0 += 1024) {
+        const uint32_t i = i0 + tid;
+        const uint32_t v = i < tiles ? __ldg(&c[i]) : 0u;
+        uint32_t total;
+        const uint32_t ex = vs_block_scan_1024(v, warp_sums, total);
+        if (i < tiles) o[i] = base + ex;
+        base += total;
     }
-    if (tid == 1023) off[n] = run;
+    if (view == views - 1 && tid == 0) {
+        off[(size_t)views * tiles] = base;
+        if (base > ref_capacity) atomicMax(&counters[VS_CNT_OVERFLOW], (unsigned long long)base);
+    }
 }
 
 cudaError_t vs_launch_bin_scan(const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
 {
-    const uint32_t n = ch.views * fr.tiles_x * fr.tiles_y;
-    k_scan<<<1, 1024, 0, st>>>(ch.tile_count, n, ch.tile_off);
+    k_scan<<<ch.views, 1024, 0, st>>>(ch.tile_count, fr.tiles_x * fr.tiles_y, ch.views, ch.tile_off, ch.ref_capacity, ch.counters);
     return cudaGetLastError();
 }

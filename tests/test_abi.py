@@ -28,7 +28,7 @@ def test_struct_layouts_match_header():
     assert C.sizeof(binding.vs_render_params) == 36
     assert C.sizeof(binding.vs_layer_desc) == 56
     assert C.sizeof(binding.vs_scene_desc) == 24
-    assert C.sizeof(binding.vs_render_stats) == 88
+    assert C.sizeof(binding.vs_render_stats) == 104
 
 
 def test_argument_validation_happens_before_any_cuda_work():
