@@ -1,0 +1,87 @@
+"""GPU parity at BASELINE.json's FULL sizes (configs C2..C5; C1 is already full size in
+test_gpu_parity.py), in the launch configuration bench.py times (whole camera batch in one vs_render
+call, automatic chunking, no AOV in the timed call).
+
+For each configuration the whole batch is rendered once; a sample of views (chosen to include the
+first, the last and -- for C5 -- a far and a close-up camera) is compared against the CPU oracle pixel
+by pixel: triangle ids BIT-EXACT, RGBA max abs error <= 1e-4.  Every view is additionally checked
+through properties that hold at any size (the AOV-less timed call and the AOV call give the same
+image bit for bit; alpha in [0,1]; pixels no layer hits are exactly the background; ids in range;
+no dropped triangles)."""
+import types
+
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = 1e-4
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    assert torch.cuda.is_available(), "these tests need the B200"
+    import oracle
+    from paper_2409_02482_b200 import binding, synth
+    binding.load_library()
+    return types.SimpleNamespace(torch=torch, oracle=oracle, binding=binding, synth=synth)
+
+
+def _check_config(env, cfg, sample_views, id_views):
+    b, torch = env.binding, env.torch
+    sc = env.synth.make_config(cfg)
+    B, W, H, k = len(sc.cameras), sc.width, sc.height, sc.k
+    r = b.Renderer(sc)
+    p = b.make_params(W, H, sc.near_plane, sc.t_min, sc.background)
+    # (1) the timed launch configuration: whole batch, no AOV
+    out = torch.empty((B, H, W, 4), dtype=torch.float32, device="cuda")
+    b.vs_render(r.handle, sc.cameras, p, out)
+    torch.cuda.synchronize()
+    stats = r.stats()
+    assert stats["dropped_triangles"] == 0, "cameras are outside the shells: nothing may be dropped"
+    rgba_all = out.cpu().numpy()
+    del out
+    assert np.isfinite(rgba_all).all()
+    assert rgba_all[..., 3].min() >= 0.0 and rgba_all[..., 3].max() <= 1.0
+    # (2) the AOV call on the sampled views must give the same image and ids that match the oracle
+    worst = 0.0
+    for v in sample_views:
+        rgba, ids = r.render(sc.cameras[[v]], p, want_ids=True)
+        torch.cuda.synchronize()
+        rgba = rgba.cpu().numpy()[0]
+        ids = ids.cpu().numpy().view(np.uint32)[0]
+        assert np.array_equal(rgba, rgba_all[v]), "AOV call and timed call differ in view %d" % v
+        ntri = np.array([ly.indices.shape[0] for ly in sc.layers], np.uint32)[:, None, None]
+        hit = ids != b.MISS
+        assert np.all(ids[hit] < np.broadcast_to(ntri, ids.shape)[hit])
+        nohit = ~hit.any(axis=0)
+        bg = np.array(list(sc.background) + [0.0], np.float32)
+        assert np.array_equal(rgba[nohit], np.broadcast_to(bg, rgba[nohit].shape))
+        if v in id_views:
+            ref = env.oracle.render_scene(sc, [v])[0]
+            nbad = int((ids != ref["ids"]).sum())
+            assert nbad == 0, "C%d view %d: %d triangle ids differ from the oracle" % (cfg, v, nbad)
+            err = float(np.abs(rgba.astype(np.float64) - ref["rgba"]).max())
+            worst = max(worst, err)
+            assert err <= TOL, "C%d view %d: max abs rgba error %.3e" % (cfg, v, err)
+    r.close()
+    print("C%d full size: %d views rendered, %d compared with the oracle, worst rgba err %.3e, coverage of view %d = %.3f"
+          % (cfg, B, len(id_views), worst, sample_views[0], float(hit.any(axis=0).mean())))
+
+
+def test_config2_full(env):
+    _check_config(env, 2, [0, 7, 15], [0, 15])
+
+
+def test_config3_full(env):
+    _check_config(env, 3, [0, 13, 31], [0, 31])
+
+
+def test_config4_full(env):
+    _check_config(env, 4, [0, 29, 63], [0, 63])
+
+
+def test_config5_full(env):
+    # even views are far cameras (r = 3), odd views close-ups (r = 1.6) that fill the frame
+    _check_config(env, 5, [0, 1, 15], [0, 1])
