@@ -117,9 +117,10 @@ static vs_status scene_create_impl(const vs_scene_desc* desc, cudaStream_t st, v
     const uint32_t k = desc->num_layers;
     const uint32_t n = (desc->sh_degree + 1) * (desc->sh_degree + 1);
     const int f16 = desc->tex_dtype == VS_F16;
-    const uint32_t cpv = f16 ? 2 : 1;
     VsSceneDev& d = s->dev;
-    d.k = k; d.sh_degree = desc->sh_degree; d.n_coef = n; d.texel_vecs = (n + cpv - 1) / cpv;
+    d.k = k; d.sh_degree = desc->sh_degree; d.n_coef = n;
+    d.texel_vecs = 4 * vs_vecs_per_channel(f16, n);
+    d.np_pad = vs_vecs_per_channel(f16, n) * (f16 ? 8u : 4u);
     s->tex_f16 = f16;
     uint64_t vt = 0, tt = 0;
     for (uint32_t l = 0; l < k; ++l) {
@@ -167,12 +168,10 @@ static vs_status scene_create_impl(const vs_scene_desc* desc, cudaStream_t st, v
         const size_t src_bytes = texels * n * 4 * (f16 ? 2 : 4);
         uint4* tex;
         if ((r = dev_alloc(s, (void**)&tex, texels * d.texel_vecs * 16)) != VS_OK) return r;
-        if (d.texel_vecs * 16 == n * 4 * (f16 ? 2u : 4u)) {
-            CU(cudaMemcpyAsync(tex, L.texture, src_bytes, kind, st));
-        } else {
+        {
             const void* tsrc = nullptr;
             if ((r = stage_in(L.texture, src_bytes, desc->memory, st, temps, &tsrc)) != VS_OK) return r;
-            CU(vs_launch_pack_texture(tsrc, f16, (uint32_t)texels, n, d.texel_vecs, tex, st));
+            CU(vs_launch_pack_texture(tsrc, f16, (uint32_t)texels, n, d.np_pad, tex, st));
         }
         d.tex[l] = tex; d.tex_w[l] = L.tex_w; d.tex_h[l] = L.tex_h;
         voff += L.num_vertices;

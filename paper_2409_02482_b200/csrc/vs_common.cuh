@@ -20,7 +20,8 @@ struct VsSceneDev {
     const uint4* tris;        // [t_total] {i0, i1, i2 : global vertex index, w : layer}
     uint32_t v_total, t_total;
     uint32_t k, sh_degree, n_coef;
-    uint32_t texel_vecs;                  // 16-byte vectors per texel in the internal layout
+    uint32_t texel_vecs;                  // 16-byte vectors per texel in the internal layout (= 4 * np_pad * elem / 16)
+    uint32_t np_pad;                      // coefficients per channel row of the internal layout [texel][ch][np_pad]
     uint32_t tri_off[VS_MAX_LAYERS + 1];  // global triangle id of each layer's triangle 0
     const uint4* tex[VS_MAX_LAYERS];      // [tex_h][tex_w][texel_vecs] 16-byte vectors
     uint32_t tex_w[VS_MAX_LAYERS], tex_h[VS_MAX_LAYERS];
@@ -250,5 +251,14 @@ cudaError_t vs_launch_reference(const VsSceneDev& sc, int tex_f16, const VsFrame
 cudaError_t vs_launch_pack_tris(const uint32_t* indices, uint32_t num_tris, uint32_t num_vertices, uint32_t vtx_off,
                                 uint32_t layer, uint4* out, uint32_t* error_flag, cudaStream_t st);
 cudaError_t vs_launch_check_finite(const float* v, size_t n, uint32_t* error_flag, cudaStream_t st);
-cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, uint32_t n_coef, uint32_t texel_vecs,
+cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, uint32_t n_coef, uint32_t np_pad,
                                    uint4* dst, cudaStream_t st);
+
+// Internal texel layout: [texel][ch = 0..3][np_pad] elements, channel-major, every channel row
+// padded to np_pad = 16-byte vectors-per-channel (1, 2 or 4) * elements per vector coefficients.
+__host__ __device__ inline uint32_t vs_vecs_per_channel(int f16, uint32_t n_coef)
+{
+    const uint32_t epv = f16 ? 8u : 4u;
+    const uint32_t v = (n_coef + epv - 1u) / epv;
+    return v <= 1u ? 1u : (v == 2u ? 2u : 4u);
+}

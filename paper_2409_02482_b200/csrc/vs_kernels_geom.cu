@@ -21,19 +21,19 @@ __global__ void k_check_finite(const float* __restrict__ v, size_t n, uint32_t* 
     if (i < n && !isfinite(v[i])) atomicOr(err, 2u);
 }
 
-// API layout [texel][n][4] (float or half) -> internal [texel][texel_vecs] 16-byte vectors:
-// the same element order, zero-padded to a multiple of 16 bytes per texel.
+// API layout [texel][c][ch] (float or half) -> internal [texel][ch][np_pad]: channel-major so that a
+// 16-byte vector holds consecutive coefficients of ONE channel; rows zero-padded to np_pad.
 template <typename T>
-__global__ void k_pack_texture(const T* __restrict__ src, uint32_t n_texels, uint32_t n_coef, uint32_t texel_vecs,
+__global__ void k_pack_texture(const T* __restrict__ src, uint32_t n_texels, uint32_t n_coef, uint32_t np_pad,
                                T* __restrict__ dst)
 {
-    const uint32_t per_vec = 16 / sizeof(T);
-    const uint32_t dst_elems = texel_vecs * per_vec, src_elems = n_coef * 4;
+    const uint32_t dst_elems = 4 * np_pad, src_elems = n_coef * 4;
     size_t total = (size_t)n_texels * dst_elems;
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
         size_t texel = i / dst_elems;
         uint32_t e = (uint32_t)(i - texel * dst_elems);
-        dst[i] = e < src_elems ? src[texel * src_elems + e] : T(0);
+        uint32_t ch = e / np_pad, c = e - ch * np_pad;
+        dst[i] = c < n_coef ? src[texel * src_elems + 4 * c + ch] : T(0);
     }
 }
 
@@ -52,14 +52,14 @@ cudaError_t vs_launch_check_finite(const float* v, size_t n, uint32_t* error_fla
     return cudaGetLastError();
 }
 
-cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, uint32_t n_coef, uint32_t texel_vecs,
+cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, uint32_t n_coef, uint32_t np_pad,
                                    uint4* dst, cudaStream_t st)
 {
     const int blocks = 148 * 16;
     if (f16)
-        k_pack_texture<__half><<<blocks, 256, 0, st>>>((const __half*)src, n_texels, n_coef, texel_vecs, (__half*)dst);
+        k_pack_texture<__half><<<blocks, 256, 0, st>>>((const __half*)src, n_texels, n_coef, np_pad, (__half*)dst);
     else
-        k_pack_texture<float><<<blocks, 256, 0, st>>>((const float*)src, n_texels, n_coef, texel_vecs, (float*)dst);
+        k_pack_texture<float><<<blocks, 256, 0, st>>>((const float*)src, n_texels, n_coef, np_pad, (float*)dst);
     return cudaGetLastError();
 }
 

@@ -187,8 +187,8 @@ k_reference(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ 
                 float v = 0.0f;
                 for (int q = 0; q < 4; ++q) {
                     float tv;
-                    if (F16) tv = __half2float(reinterpret_cast<const __half*>(sc.tex[l] + offs[q])[4 * c + ch]);
-                    else tv = reinterpret_cast<const float*>(sc.tex[l] + offs[q])[4 * c + ch];
+                    if (F16) tv = __half2float(reinterpret_cast<const __half*>(sc.tex[l] + offs[q])[ch * sc.np_pad + c]);
+                    else tv = reinterpret_cast<const float*>(sc.tex[l] + offs[q])[ch * sc.np_pad + c];
                     v += ws[q] * tv;
                 }
                 s[ch] += Y[c] * v;

@@ -1,51 +1,64 @@
 // vs_kernels_shade.cu -- S5 perspective-correct UV + bilinear texel fetch, S6 SH evaluation + sigmoid,
-// S7 fixed-order front-to-back compositing.  DESIGN.md §1, §3.5-3.8, §7.
+// S7 fixed-order front-to-back compositing.  DESIGN.md §1, §3.5-3.8, §6, §7.
 //
 // One CTA per (view, 16x16 tile), a warp owns an 8x4 pixel block, lane = pixel ("owner").
 // Phase A: every owner turns the winning triangle of each layer (the id planes k_raster wrote) into
 //   a packed fragment record (clamped texel column/row of the 2x2 footprint + the two bilinear
 //   fractions) in shared memory.  The gather chain id -> triangle -> 3 vertices + 3 uvs is paid once
 //   per tile, three layers at a time, instead of once per layer inside the shading loop.
-// Phase B: per layer the warp re-maps itself to 4 fragments x 8 lanes: octet `o` streams the four
-//   texels of the fragment of pixel row `o`, column `j`, as 16-byte vectors (one full 128-byte line
-//   per octet per texel at SH degree 3 / fp16), blends them with the bilinear weights, dots with
-//   the pixel's SH basis (kept in registers for all layers) and hands 4 partial channel sums back
-//   through shared memory.  Owners add the partials, apply the sigmoid and composite front to back.
+// Phase B: per layer the warp re-maps itself to 4 fragments x 8 lanes.  Octet `o` streams the four
+//   texels of the fragment of pixel row `o`, column `j`, as 16-byte vectors: the internal texel layout
+//   is channel-major ([ch][coefficient]), so a lane's vector holds 8 (fp16) / 4 (fp32)
+//   consecutive coefficients of ONE channel and an octet reads one full 128-byte line per texel at SH
+//   degree 3 / fp16.  The loads of column j+1 are issued before the arithmetic of column j (software
+//   pipeline).  A lane blends its coefficients with the bilinear weights and dots them with the pixel's
+//   SH basis (staged once per pixel in shared memory, shared by all layers) using packed fp32 FMAs
+//   (fma.rn.f32x2 -> FFMA2); the one or two lanes of a channel are summed with one shuffle and the
+//   four channel logits go back to the owner through shared memory.  Owners apply the sigmoid and
+//   composite front to back in registers.
 #include "vs_common.cuh"
 
 struct __align__(16) VsFragRec {
     uint32_t o00, o01, o10, o11;  // 16-byte-vector offsets of the four texels inside the layer texture
-    float w00, w01, w10, w11;     // bilinear weights
+    float w00, w01, w10, w11;     // bilinear weights (all 0: no fragment)
 };
 
+// ---- packed fp32 pairs (sm_100: FFMA2 / FMUL2) -------------------------------------------------
+typedef unsigned long long f32x2;
+
+__device__ __forceinline__ f32x2 vs_pack2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void vs_unpack2(f32x2 v, float& lo, float& hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 vs_fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2 vs_mul2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+
+// element pair q (0..3 for fp16, 0..1 for fp32) of a 16-byte texel vector as packed fp32
 template <int F16>
-__device__ __forceinline__ void vs_accumulate_vec(const uint4& t00, const uint4& t01, const uint4& t10, const uint4& t11,
-                                                  const float4& w, const float* Y, float4& acc)
+__device__ __forceinline__ f32x2 vs_pair(const uint4& t, int q)
 {
     if (F16) {
-        const __half2* h00 = reinterpret_cast<const __half2*>(&t00);
-        const __half2* h01 = reinterpret_cast<const __half2*>(&t01);
-        const __half2* h10 = reinterpret_cast<const __half2*>(&t10);
-        const __half2* h11 = reinterpret_cast<const __half2*>(&t11);
-        float v[8];
-#pragma unroll
-        for (int q = 0; q < 4; ++q) {
-            const float2 a = __half22float2(h00[q]), b = __half22float2(h01[q]);
-            const float2 c = __half22float2(h10[q]), d = __half22float2(h11[q]);
-            v[2 * q] = w.x * a.x + w.y * b.x + w.z * c.x + w.w * d.x;
-            v[2 * q + 1] = w.x * a.y + w.y * b.y + w.z * c.y + w.w * d.y;
-        }
-        acc.x += Y[0] * v[0] + Y[1] * v[4];
-        acc.y += Y[0] * v[1] + Y[1] * v[5];
-        acc.z += Y[0] * v[2] + Y[1] * v[6];
-        acc.w += Y[0] * v[3] + Y[1] * v[7];
+        const uint32_t w = q == 0 ? t.x : q == 1 ? t.y : q == 2 ? t.z : t.w;
+        const float2 f = __half22float2(*reinterpret_cast<const __half2*>(&w));
+        return vs_pack2(f.x, f.y);
     } else {
-        const float4 a = *reinterpret_cast<const float4*>(&t00), b = *reinterpret_cast<const float4*>(&t01);
-        const float4 c = *reinterpret_cast<const float4*>(&t10), d = *reinterpret_cast<const float4*>(&t11);
-        acc.x += Y[0] * (w.x * a.x + w.y * b.x + w.z * c.x + w.w * d.x);
-        acc.y += Y[0] * (w.x * a.y + w.y * b.y + w.z * c.y + w.w * d.y);
-        acc.z += Y[0] * (w.x * a.z + w.y * b.z + w.z * c.z + w.w * d.z);
-        acc.w += Y[0] * (w.x * a.w + w.y * b.w + w.z * c.w + w.w * d.w);
+        return q == 0 ? vs_pack2(__uint_as_float(t.x), __uint_as_float(t.y)) : vs_pack2(__uint_as_float(t.z), __uint_as_float(t.w));
     }
 }
 
@@ -55,24 +68,35 @@ __device__ __forceinline__ uint32_t vs_pack_frag(const VsFrag& f)
     return f.cx0 | ((f.cx1 != f.cx0) ? 0x8000u : 0u) | (f.cy0 << 16) | ((f.cy1 != f.cy0) ? 0x80000000u : 0u);
 }
 
+// compile-time shape of the octet mapping for a texture format (must agree with vs_vecs_per_channel)
+template <int F16, int DEG>
+struct VsShadeShape {
+    static constexpr int NCOEF = (DEG + 1) * (DEG + 1);
+    static constexpr int EPV = F16 ? 8 : 4;                            // elements per 16-byte vector
+    static constexpr int VPC0 = (NCOEF + EPV - 1) / EPV;
+    static constexpr int VPC = VPC0 <= 1 ? 1 : (VPC0 == 2 ? 2 : 4);     // vectors per channel row
+    static constexpr int NVEC = 4 * VPC;                               // vectors per texel (== sc.texel_vecs)
+    static constexpr int SLOTS = NVEC > 8 ? NVEC / 8 : 1;              // vectors per octet lane
+    static constexpr int LPC = VPC / SLOTS;                            // lanes per channel (1 or 2)
+    static constexpr int NACT = NVEC / SLOTS;                          // octet lanes that hold data (4 or 8)
+    static constexpr int NE = SLOTS * EPV;                             // coefficients per lane (4 or 8)
+    static constexpr int PPV = EPV / 2;                                // fp32 pairs per vector
+};
+
 template <int F16, int DEG, bool COUNT>
-__global__ void __launch_bounds__(256, 2)
+__global__ void __launch_bounds__(256, 3)
 k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams, const int4* __restrict__ vtx,
         const uint32_t* __restrict__ tile_off, const uint32_t* __restrict__ ids, float* __restrict__ out_rgba,
         uint32_t* __restrict__ texel_bits, unsigned long long* __restrict__ counters)
 {
-    constexpr int NCOEF = (DEG + 1) * (DEG + 1);
-    constexpr int CPV = F16 ? 2 : 1;                 // coefficients per 16-byte vector
-    constexpr int NVEC = (NCOEF + CPV - 1) / CPV;    // vectors per texel (== sc.texel_vecs)
-    constexpr int SLOTS = (NVEC + 7) / 8;            // vectors per octet lane
-    constexpr int NACT = NVEC < 8 ? NVEC : 8;        // octet lanes that hold data
-    constexpr int YROW = SLOTS * 8 * CPV;            // floats per pixel in the Y staging buffer
+    typedef VsShadeShape<F16, DEG> S;
+    constexpr int SLOTS = S::SLOTS, LPC = S::LPC, NACT = S::NACT, NE = S::NE, PPV = S::PPV;
 
     extern __shared__ __align__(16) unsigned char smem[];
     // [k][256] packed texel coordinates, then [k][256] float2 fractions (a < 0: no fragment)
     uint32_t* rec_xy = reinterpret_cast<uint32_t*>(smem);
     float2* rec_ab = reinterpret_cast<float2*>(smem + (size_t)sc.k * VS_TILE_PIX * 4);
-    unsigned char* per_warp = smem + (size_t)sc.k * VS_TILE_PIX * 12;  // 8 x (1 KB records + 4 KB partial sums)
+    unsigned char* per_warp = smem + (size_t)sc.k * VS_TILE_PIX * 12;  // 8 x (2 KB basis + 1 KB records + 512 B logits)
 
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t tile = blockIdx.x, view = blockIdx.y;
@@ -117,35 +141,31 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     }
     // each thread reads back only its own records: no barrier needed
 
-    // ---------------- phase B: shade + composite ----------------
-    const uint32_t oct = lane >> 3, oi = lane & 7;  // octet index (= pixel row) / lane within octet
-    VsFragRec* rec = reinterpret_cast<VsFragRec*>(per_warp + warp * 5120);
-    float4* part = reinterpret_cast<float4*>(per_warp + warp * 5120 + 1024);
-    float* ysm = reinterpret_cast<float*>(part);    // Y staging aliases the partial-sum buffer
-
     if (!__any_sync(0xFFFFFFFFu, any_hit)) {
         if (inimg) reinterpret_cast<float4*>(out_rgba)[pix] = make_float4(fr.bg[0], fr.bg[1], fr.bg[2], 0.0f);
         return;
     }
-    float Yr[8][SLOTS][CPV];
+
+    // ---------------- phase B: shade + composite ----------------
+    const uint32_t oct = lane >> 3, oi = lane & 7;  // octet index (= pixel row) / lane within octet
+    float4* ysm = reinterpret_cast<float4*>(per_warp + warp * 3584);                // [j][oct][4 chunks of 4 floats], swizzled
+    VsFragRec* rec = reinterpret_cast<VsFragRec*>(per_warp + warp * 3584 + 2048);   // [pixel]
+    float4* part = reinterpret_cast<float4*>(per_warp + warp * 3584 + 3072);        // [pixel] 4 channel logits
     {
-        float Y[YROW];
+        // SH basis of the owner's pixel -> row (j = column, oct = row); chunk q stored at q ^ (row >> 1) so that
+        // the four octets' reads of one chunk fall into distinct banks
+        float Y[16];
 #pragma unroll
-        for (int c = 0; c < YROW; ++c) Y[c] = 0.0f;
+        for (int c = 0; c < 16; ++c) Y[c] = 0.0f;
         float vx, vy, vz;
         vs_view_dir(cams[view], px, py, vx, vy, vz);
         vs_sh_basis<DEG>(vx, vy, vz, Y);
+        float4* row = ysm + ((lane & 7) * 4 + (lane >> 3)) * 4;
 #pragma unroll
-        for (int c = 0; c < YROW; ++c) ysm[lane * YROW + c] = Y[c];
-        __syncwarp();
-#pragma unroll
-        for (int j = 0; j < 8; ++j)
-#pragma unroll
-            for (int s = 0; s < SLOTS; ++s)
-#pragma unroll
-                for (int c = 0; c < CPV; ++c) Yr[j][s][c] = ysm[(8 * oct + j) * YROW + (oi + 8 * s) * CPV + c];
-        __syncwarp();
+        for (int q = 0; q < 4; ++q) row[q ^ (int)(lane >> 4)] = make_float4(Y[4 * q], Y[4 * q + 1], Y[4 * q + 2], Y[4 * q + 3]);
     }
+    const uint32_t ychunk0 = ((oi % LPC) * NE) >> 2;   // first 16-byte chunk of this lane's coefficients
+    const bool lane_on = oi < (uint32_t)NACT;
 
     float Tr = 1.0f, Cr = 0.0f, Cg = 0.0f, Cb = 0.0f;
     bool alive = true;
@@ -159,7 +179,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
         if (shade) {
             const uint32_t xy = rec_xy[l * VS_TILE_PIX + tid];
             const uint32_t cx0 = xy & 0x7FFFu, cy0 = (xy >> 16) & 0x7FFFu;
-            const uint32_t Wt = sc.tex_w[l], nv = (uint32_t)NVEC;
+            const uint32_t Wt = sc.tex_w[l], nv = (uint32_t)S::NVEC;
             const uint32_t row0 = cy0 * Wt, row1 = row0 + ((xy >> 31) ? Wt : 0u);
             const uint32_t cx1 = cx0 + ((xy >> 15) & 1u);
             r.o00 = (row0 + cx0) * nv; r.o01 = (row0 + cx1) * nv;
@@ -178,41 +198,62 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
         if (COUNT && lane == 0) atomicAdd(&counters[VS_CNT_FRAGS], (unsigned long long)__popc(m));
         rec[lane] = r;
         __syncwarp();
-        const uint4* __restrict__ tb = sc.tex[l];
+        const uint4* __restrict__ tb = sc.tex[l] + SLOTS * oi;
+
+        uint4 tv[2][SLOTS][4];
+        auto issue = [&](int j, int b) {
+            const uint4 o = *reinterpret_cast<const uint4*>(&rec[8 * oct + j]);
+#pragma unroll
+            for (int s = 0; s < SLOTS; ++s) {
+                if (lane_on) {
+                    tv[b][s][0] = __ldg(tb + o.x + s); tv[b][s][1] = __ldg(tb + o.y + s);
+                    tv[b][s][2] = __ldg(tb + o.z + s); tv[b][s][3] = __ldg(tb + o.w + s);
+                } else {
+                    tv[b][s][0] = tv[b][s][1] = tv[b][s][2] = tv[b][s][3] = make_uint4(0, 0, 0, 0);
+                }
+            }
+        };
+        issue(0, 0);
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-            if (m & (0x01010101u << j)) {  // some pixel of column j is shaded
-                const VsFragRec* rp = &rec[8 * oct + j];
-                const uint4 o = *reinterpret_cast<const uint4*>(rp);
-                const float4 w = *(reinterpret_cast<const float4*>(rp) + 1);
-                float4 acc = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+            if (j + 1 < 8) issue(j + 1, (j + 1) & 1);
+            const int b = j & 1;
+            const float4 w = *(reinterpret_cast<const float4*>(&rec[8 * oct + j]) + 1);
+            const f32x2 W00 = vs_pack2(w.x, w.x), W01 = vs_pack2(w.y, w.y), W10 = vs_pack2(w.z, w.z), W11 = vs_pack2(w.w, w.w);
+            const float4* yrow = ysm + (j * 4 + oct) * 4;
+            f32x2 acc2 = 0ull;
 #pragma unroll
-                for (int s = 0; s < SLOTS; ++s) {
-                    const uint32_t vi = oi + 8 * s;
-                    if (vi < (uint32_t)NVEC) {
-                        const uint4 t00 = __ldg(tb + o.x + vi), t01 = __ldg(tb + o.y + vi);
-                        const uint4 t10 = __ldg(tb + o.z + vi), t11 = __ldg(tb + o.w + vi);
-                        vs_accumulate_vec<F16>(t00, t01, t10, t11, w, Yr[j][s], acc);
+            for (int s = 0; s < SLOTS; ++s) {
+#pragma unroll
+                for (int h = 0; h < PPV / 2; ++h) {   // 16-byte chunk of 4 basis values <-> 2 element pairs
+                    const int e = s * PPV + 2 * h;    // element pair index within the lane's coefficients
+                    const float4 y = yrow[(ychunk0 + (e >> 1)) ^ (oct >> 1)];
+#pragma unroll
+                    for (int g = 0; g < 2; ++g) {
+                        const int q = 2 * h + g;
+                        f32x2 v = vs_mul2(W00, vs_pair<F16>(tv[b][s][0], q));
+                        v = vs_fma2(W01, vs_pair<F16>(tv[b][s][1], q), v);
+                        v = vs_fma2(W10, vs_pair<F16>(tv[b][s][2], q), v);
+                        v = vs_fma2(W11, vs_pair<F16>(tv[b][s][3], q), v);
+                        acc2 = vs_fma2(g == 0 ? vs_pack2(y.x, y.y) : vs_pack2(y.z, y.w), v, acc2);
                     }
                 }
-                if (oi < (uint32_t)NACT) part[(8 * oct + j) * 8 + oi] = acc;
             }
+            float a0, a1;
+            vs_unpack2(acc2, a0, a1);
+            float acc = a0 + a1;
+            if (LPC == 2) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, 1);
+            if (lane_on && (oi % LPC) == 0) reinterpret_cast<float*>(part)[(8 * oct + j) * 4 + oi / LPC] = acc;
         }
         __syncwarp();
         if (shade) {
-            float4 s4 = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-#pragma unroll
-            for (int s = 0; s < NACT; ++s) {
-                const float4 p = part[lane * 8 + ((s + lane) % NACT)];
-                s4.x += p.x; s4.y += p.y; s4.z += p.z; s4.w += p.w;
-            }
+            const float4 s4 = part[lane];
             const float A = vs_sigmoid(s4.w);
             const float TA = Tr * A;
             Cr += TA * vs_sigmoid(s4.x); Cg += TA * vs_sigmoid(s4.y); Cb += TA * vs_sigmoid(s4.z);
             Tr *= (1.0f - A);
             if (Tr < fr.t_min) alive = false;
         }
-        __syncwarp();
     }
     if (inimg)
         reinterpret_cast<float4*>(out_rgba)[pix] = make_float4(Cr + Tr * fr.bg[0], Cg + Tr * fr.bg[1], Cb + Tr * fr.bg[2], 1.0f - Tr);
@@ -221,7 +262,8 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
 template <int F16, int DEG, bool COUNT>
 static cudaError_t launch_sh2(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
 {
-    const size_t smem = (size_t)sc.k * VS_TILE_PIX * 12 + 8 * 5120;
+    if (sc.texel_vecs != (uint32_t)VsShadeShape<F16, DEG>::NVEC) return cudaErrorInvalidValue;
+    const size_t smem = (size_t)sc.k * VS_TILE_PIX * 12 + 8 * 3584;
     auto kern = k_shade<F16, DEG, COUNT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
