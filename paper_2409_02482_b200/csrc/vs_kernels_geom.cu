@@ -107,11 +107,15 @@ cudaError_t vs_launch_transform(const VsSceneDev& sc, const VsFrame& fr, const V
 //   k_bin_scatter: re-reads the packed range (no vertex gathers) and writes the triangle id into
 //                  the tile's list.
 // A triangle is referenced by every tile its sample-point bounding box touches.  Consecutive
-// triangles of a mesh mostly fall into the same tile, so the tile atomics are warp-aggregated:
-// lanes that target the same tile elect a leader (match.any) which adds the group's size once.
+// triangles of a mesh mostly fall into a handful of tiles, so the tile atomics are CTA-aggregated in
+// a small shared-memory table and every distinct global counter is touched once per CTA.
 // ------------------------------------------------------------------------------------------------
 #define VS_RANGE_NONE 0xFFFFFFFFu   // triangle references no tile
 #define VS_RANGE_WIDE 0xFFFFFFFEu   // more than 64 tiles in one direction: the scatter pass recomputes the range
+#define VS_BIN_THREADS 512
+#define VS_BIN_SLOTS 256            // per-CTA tile table (open addressing, <= VS_BIN_PROBES probes)
+#define VS_BIN_PROBES 8
+#define VS_BIN_EMPTY 0xFFFFFFFFu
 
 __device__ __forceinline__ bool vs_tile_range(const VsSceneDev& sc, const VsFrame& fr, const int4* __restrict__ vv, uint32_t t,
                                               int& tx0, int& tx1, int& ty0, int& ty1, int& status)
@@ -126,62 +130,84 @@ __device__ __forceinline__ bool vs_tile_range(const VsSceneDev& sc, const VsFram
     return true;
 }
 
-// Adds 1 to counter[tile] for every lane with `single` set, one atomic per distinct tile of the warp.
-// Returns the lane's slot (value of the counter before its own increment).  All 32 lanes must call.
-__device__ __forceinline__ uint32_t vs_warp_tile_add(uint32_t* __restrict__ counter, bool single, uint32_t tile, uint32_t lane)
+__device__ __forceinline__ uint32_t vs_pack_range(int tx0, int tx1, int ty0, int ty1)
 {
-    const uint32_t key = single ? tile : (0x80000000u | lane);
-    const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key);
-    const int leader = __ffs(peers) - 1;
-    uint32_t base = 0;
-    if (single && (int)lane == leader) base = atomicAdd(&counter[tile], (uint32_t)__popc(peers));
-    base = __shfl_sync(0xFFFFFFFFu, base, leader);
-    return base + (uint32_t)__popc(peers & ((1u << lane) - 1u));
+    const int nx = tx1 - tx0 + 1, ny = ty1 - ty0 + 1;
+    return (nx > 64 || ny > 64) ? VS_RANGE_WIDE
+                                : ((uint32_t)tx0 | ((uint32_t)ty0 << 10) | ((uint32_t)(nx - 1) << 20) | ((uint32_t)(ny - 1) << 26));
 }
 
-__global__ void __launch_bounds__(256) k_bin_count(VsSceneDev sc, VsFrame fr, const int4* __restrict__ vtx,
-                                                   uint32_t* __restrict__ tri_tiles, uint32_t* __restrict__ tile_count,
-                                                   unsigned long long* counters)
+// Per-CTA tile table.  Consecutive triangles of a mesh mostly fall into a handful of tiles, so a CTA
+// first sums its references per tile in shared memory and then touches every distinct global
+// counter once.  vs_bin_find returns the slot of `tile` (inserting it) or -1 when the probe sequence
+// is exhausted (the caller then falls back to a global atomic of its own).
+__device__ __forceinline__ int vs_bin_find(uint32_t* __restrict__ keys, uint32_t tile)
 {
+    uint32_t h = (tile * 2654435761u) >> 24;  // 8 bits
+#pragma unroll 1
+    for (int p = 0; p < VS_BIN_PROBES; ++p) {
+        const uint32_t s = (h + (uint32_t)p) & (VS_BIN_SLOTS - 1);
+        const uint32_t k = keys[s];
+        if (k == tile) return (int)s;
+        if (k == VS_BIN_EMPTY) {
+            const uint32_t old = atomicCAS(&keys[s], VS_BIN_EMPTY, tile);
+            if (old == VS_BIN_EMPTY || old == tile) return (int)s;
+        }
+    }
+    return -1;
+}
+
+// Pass 1: setup + sample bounding box -> tile range per (view, triangle) and reference counts per
+// (view, tile).  The chunk's total is read off the prefix sum afterwards (no counter traffic here).
+__global__ void __launch_bounds__(VS_BIN_THREADS) k_bin_count(VsSceneDev sc, VsFrame fr, const int4* __restrict__ vtx,
+                                                              uint32_t* __restrict__ tri_tiles, uint32_t* __restrict__ tile_count,
+                                                              unsigned long long* counters)
+{
+    __shared__ uint32_t skey[VS_BIN_SLOTS], scnt[VS_BIN_SLOTS];
     const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
     const uint32_t view = blockIdx.y;
     const uint32_t tiles = fr.tiles_x * fr.tiles_y;
+    for (uint32_t i = threadIdx.x; i < VS_BIN_SLOTS; i += blockDim.x) { skey[i] = VS_BIN_EMPTY; scnt[i] = 0; }
+    __syncthreads();
     int status = -1, tx0 = 0, tx1 = -1, ty0 = 0, ty1 = -1;
     bool any = false;
-    if (t < sc.t_total) any = vs_tile_range(sc, fr, vtx + (size_t)view * sc.v_total, t, tx0, tx1, ty0, ty1, status);
-    const int nx = tx1 - tx0 + 1, ny = ty1 - ty0 + 1;
-    uint32_t packed = VS_RANGE_NONE, refs = 0;
-    if (any) {
-        packed = (nx > 64 || ny > 64) ? VS_RANGE_WIDE
-                                      : ((uint32_t)tx0 | ((uint32_t)ty0 << 10) | ((uint32_t)(nx - 1) << 20) | ((uint32_t)(ny - 1) << 26));
-        refs = (uint32_t)(nx * ny);
+    if (t < sc.t_total) {
+        any = vs_tile_range(sc, fr, vtx + (size_t)view * sc.v_total, t, tx0, tx1, ty0, ty1, status);
+        tri_tiles[(size_t)view * sc.t_total + t] = any ? vs_pack_range(tx0, tx1, ty0, ty1) : VS_RANGE_NONE;
     }
-    if (t < sc.t_total) tri_tiles[(size_t)view * sc.t_total + t] = packed;
-    const bool single = any && refs == 1;
-    vs_warp_tile_add(tile_count, single, view * tiles + (uint32_t)ty0 * fr.tiles_x + (uint32_t)tx0, lane);
-    if (any && !single)
+    if (any)
         for (int ty = ty0; ty <= ty1; ++ty)
-            for (int tx = tx0; tx <= tx1; ++tx) atomicAdd(&tile_count[view * tiles + (uint32_t)ty * fr.tiles_x + (uint32_t)tx], 1u);
-    // warp-aggregated statistics
+            for (int tx = tx0; tx <= tx1; ++tx) {
+                const uint32_t tile = (uint32_t)ty * fr.tiles_x + (uint32_t)tx;
+                const int s = vs_bin_find(skey, tile);
+                if (s >= 0) atomicAdd(&scnt[s], 1u);
+                else atomicAdd(&tile_count[view * tiles + tile], 1u);
+            }
     const unsigned full = 0xFFFFFFFFu;
     const unsigned dropped = __popc(__ballot_sync(full, status == 1));
     const unsigned degen = __popc(__ballot_sync(full, status == 2));
-    refs = __reduce_add_sync(full, refs);
     if (lane == 0) {
         if (dropped) atomicAdd(&counters[VS_CNT_DROPPED], (unsigned long long)dropped);
         if (degen) atomicAdd(&counters[VS_CNT_DEGENERATE], (unsigned long long)degen);
-        if (refs) atomicAdd(&counters[VS_CNT_REFS], (unsigned long long)refs);
     }
+    __syncthreads();
+    for (uint32_t i = threadIdx.x; i < VS_BIN_SLOTS; i += blockDim.x)
+        if (skey[i] != VS_BIN_EMPTY) atomicAdd(&tile_count[view * tiles + skey[i]], scnt[i]);
 }
 
-__global__ void __launch_bounds__(256) k_bin_scatter(VsSceneDev sc, VsFrame fr, const int4* __restrict__ vtx,
-                                                     const uint32_t* __restrict__ tri_tiles, uint32_t* __restrict__ tile_cursor,
-                                                     const uint32_t* __restrict__ tile_off, uint32_t* __restrict__ tile_tris,
-                                                     uint32_t ref_capacity)
+// Pass 2: re-reads the packed range (no vertex gathers), reserves the CTA's references of every
+// distinct tile with one global atomic, and writes the triangle ids into the tiles' lists.
+__global__ void __launch_bounds__(VS_BIN_THREADS) k_bin_scatter(VsSceneDev sc, VsFrame fr, const int4* __restrict__ vtx,
+                                                                const uint32_t* __restrict__ tri_tiles, uint32_t* __restrict__ tile_cursor,
+                                                                const uint32_t* __restrict__ tile_off, uint32_t* __restrict__ tile_tris,
+                                                                uint32_t ref_capacity)
 {
-    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x, lane = threadIdx.x & 31;
+    __shared__ uint32_t skey[VS_BIN_SLOTS], scnt[VS_BIN_SLOTS];
+    const uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
     const uint32_t view = blockIdx.y;
     const uint32_t tiles = fr.tiles_x * fr.tiles_y;
+    for (uint32_t i = threadIdx.x; i < VS_BIN_SLOTS; i += blockDim.x) { skey[i] = VS_BIN_EMPTY; scnt[i] = 0; }
+    __syncthreads();
     const uint32_t packed = t < sc.t_total ? __ldg(&tri_tiles[(size_t)view * sc.t_total + t]) : VS_RANGE_NONE;
     int tx0 = 0, tx1 = -1, ty0 = 0, ty1 = -1;
     if (packed == VS_RANGE_WIDE) {
@@ -191,35 +217,57 @@ __global__ void __launch_bounds__(256) k_bin_scatter(VsSceneDev sc, VsFrame fr, 
         tx0 = (int)(packed & 1023u); ty0 = (int)((packed >> 10) & 1023u);
         tx1 = tx0 + (int)((packed >> 20) & 63u); ty1 = ty0 + (int)(packed >> 26);
     }
-    const bool any = tx1 >= tx0, single = any && tx0 == tx1 && ty0 == ty1;
-    const uint32_t tile0 = view * tiles + (uint32_t)ty0 * fr.tiles_x + (uint32_t)tx0;
-    const uint32_t slot = vs_warp_tile_add(tile_cursor, single, tile0, lane);
-    if (single) {
-        const uint32_t pos = __ldg(&tile_off[tile0]) + slot;
-        if (pos < ref_capacity) tile_tris[pos] = t;
-    } else if (any) {
-        for (int ty = ty0; ty <= ty1; ++ty)
-            for (int tx = tx0; tx <= tx1; ++tx) {
-                const uint32_t tile = view * tiles + (uint32_t)ty * fr.tiles_x + (uint32_t)tx;
-                const uint32_t pos = __ldg(&tile_off[tile]) + atomicAdd(&tile_cursor[tile], 1u);
+    // phase 1: count per tile inside the CTA; references that miss the table go out directly
+    for (int ty = ty0; ty <= ty1; ++ty)
+        for (int tx = tx0; tx <= tx1; ++tx) {
+            const uint32_t tile = (uint32_t)ty * fr.tiles_x + (uint32_t)tx;
+            const int s = vs_bin_find(skey, tile);
+            if (s >= 0) atomicAdd(&scnt[s], 1u);
+            else {
+                const uint32_t g = view * tiles + tile;
+                const uint32_t pos = __ldg(&tile_off[g]) + atomicAdd(&tile_cursor[g], 1u);
                 if (pos < ref_capacity) tile_tris[pos] = t;
             }
-    }
+        }
+    __syncthreads();
+    // phase 2: one reservation per distinct tile; scnt becomes the next free position of the CTA's run
+    for (uint32_t i = threadIdx.x; i < VS_BIN_SLOTS; i += blockDim.x)
+        if (skey[i] != VS_BIN_EMPTY) {
+            const uint32_t g = view * tiles + skey[i];
+            scnt[i] = __ldg(&tile_off[g]) + atomicAdd(&tile_cursor[g], scnt[i]);
+        }
+    __syncthreads();
+    // phase 3: write the references (the table is read-only now, so lookups cannot insert)
+    for (int ty = ty0; ty <= ty1; ++ty)
+        for (int tx = tx0; tx <= tx1; ++tx) {
+            const uint32_t tile = (uint32_t)ty * fr.tiles_x + (uint32_t)tx;
+            const uint32_t h = (tile * 2654435761u) >> 24;
+            for (int p = 0; p < VS_BIN_PROBES; ++p) {
+                const uint32_t s = (h + (uint32_t)p) & (VS_BIN_SLOTS - 1);
+                const uint32_t k = skey[s];
+                if (k == tile) {
+                    const uint32_t pos = atomicAdd(&scnt[s], 1u);
+                    if (pos < ref_capacity) tile_tris[pos] = t;
+                    break;
+                }
+                if (k == VS_BIN_EMPTY) break;  // went out directly in phase 1
+            }
+        }
 }
 
 cudaError_t vs_launch_bin_count(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
 {
     if (sc.t_total == 0) return cudaSuccess;
-    dim3 grid((sc.t_total + 255) / 256, ch.views);
-    k_bin_count<<<grid, 256, 0, st>>>(sc, fr, ch.vtx, ch.tri_tiles, ch.tile_count, ch.counters);
+    dim3 grid((sc.t_total + VS_BIN_THREADS - 1) / VS_BIN_THREADS, ch.views);
+    k_bin_count<<<grid, VS_BIN_THREADS, 0, st>>>(sc, fr, ch.vtx, ch.tri_tiles, ch.tile_count, ch.counters);
     return cudaGetLastError();
 }
 
 cudaError_t vs_launch_bin_scatter(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
 {
     if (sc.t_total == 0) return cudaSuccess;
-    dim3 grid((sc.t_total + 255) / 256, ch.views);
-    k_bin_scatter<<<grid, 256, 0, st>>>(sc, fr, ch.vtx, ch.tri_tiles, ch.tile_cursor, ch.tile_off, ch.tile_tris, ch.ref_capacity);
+    dim3 grid((sc.t_total + VS_BIN_THREADS - 1) / VS_BIN_THREADS, ch.views);
+    k_bin_scatter<<<grid, VS_BIN_THREADS, 0, st>>>(sc, fr, ch.vtx, ch.tri_tiles, ch.tile_cursor, ch.tile_off, ch.tile_tris, ch.ref_capacity);
     return cudaGetLastError();
 }
 
@@ -268,6 +316,7 @@ __global__ void __launch_bounds__(1024) k_scan(const uint32_t* __restrict__ coun
     }
     if (view == views - 1 && tid == 0) {
         off[(size_t)views * tiles] = base;
+        atomicAdd(&counters[VS_CNT_REFS], (unsigned long long)base);
         if (base > ref_capacity) atomicMax(&counters[VS_CNT_OVERFLOW], (unsigned long long)base);
     }
 }
