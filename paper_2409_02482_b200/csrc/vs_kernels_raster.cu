@@ -23,7 +23,13 @@
 
 __device__ __forceinline__ void vs_key_max(unsigned long long* slot, unsigned long long key)
 {
-    if (key > *slot) atomicMax(slot, key);
+    // 64-bit shared-memory max: the plain read doubles as the expected value of the first compare-and-swap
+    unsigned long long old = *slot;
+    while (key > old) {
+        const unsigned long long assumed = old;
+        old = atomicCAS(slot, assumed, key);
+        if (old == assumed) break;
+    }
 }
 
 __device__ __forceinline__ float vs_to_float(int v) { return __int2float_rn(v); }
@@ -80,7 +86,11 @@ k_raster(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, co
             for (uint32_t l = 0; l < sc.k; ++l) ids[(((size_t)view * sc.k + l) * H + py) * W + px] = VS_MISS;
         return;
     }
+    // the list is handed out 32 references at a time: the first two batches of a warp are fixed, the later ones
+    // come from a shared counter so that the warps finish together
+    __shared__ uint32_t s_next;
     for (uint32_t i = tid; i < sc.k * VS_TILE_PIX; i += 256) keys[i] = 0ull;
+    if (tid == 0) s_next = begin + 512u;
     __syncthreads();
 
     int* rec = reinterpret_cast<int*>(keys + sc.k * VS_TILE_PIX) + warp * VS_RS_WARP_WORDS;  // [field][lane]
@@ -88,8 +98,19 @@ k_raster(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, co
     const int4* __restrict__ vv = vtx + (size_t)view * sc.v_total;
     const int tx1 = min(px0 + VS_TILE_W, W) - 1, ty1 = min(py0 + VS_TILE_H, H) - 1;
 
-    for (uint32_t base = begin + warp * 32; base < end; base += 256) {  // warp-uniform
+    // software pipeline over the gather chain tile_tris -> tris -> vertices: the reference of batch n+2 and the
+    // index record of batch n+1 are in flight while batch n is rasterised
+    uint32_t base = begin + warp * 32, base1 = base + 256u;
+    uint32_t gt = base + lane < end ? __ldg(&tile_tris[base + lane]) : 0u;
+    uint32_t gt1 = base1 + lane < end ? __ldg(&tile_tris[base1 + lane]) : 0u;
+    uint4 tri = __ldg(&sc.tris[gt]);
+    for (; base < end; ) {  // warp-uniform
         const uint32_t idx = base + lane;
+        uint32_t base2 = 0;
+        if (lane == 0) base2 = atomicAdd(&s_next, 32u);
+        base2 = __shfl_sync(0xFFFFFFFFu, base2, 0);
+        const uint32_t gt2 = base2 + lane < end ? __ldg(&tile_tris[base2 + lane]) : 0u;
+        const uint4 tri1 = __ldg(&sc.tris[gt1]);
         // ---------------- phase 1: lane = triangle ----------------
         bool large = false;
         VsTri T;
@@ -97,8 +118,6 @@ k_raster(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, co
         uint32_t layer = 0, lid = 0;
         bool narrow = false, valid = false;
         if (idx < end) {
-            const uint32_t gt = __ldg(&tile_tris[idx]);
-            const uint4 tri = __ldg(&sc.tris[gt]);
             const int4 a = __ldg(&vv[tri.x]), b = __ldg(&vv[tri.y]), c = __ldg(&vv[tri.z]);
             if (vs_setup_tri(a, b, c, T) == 0) {
                 const int minX = min(T.X0, min(T.X1, T.X2)), maxX = max(T.X0, max(T.X1, T.X2));
@@ -139,10 +158,11 @@ k_raster(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, co
         }
         const int nr = small ? j1 - j0 + 1 : 0, nc = small ? i1 - i0 + 1 : 0;
         {
-            // rows of 8 samples, the row count uniform over the warp (the lanes' boxes are alike); samples
-            // of a row are visited from column 7 down to 0 so that each funnel shift pushes the next lower bit
+            // rows of up to 8 samples, row and column counts uniform over the warp (the lanes' boxes are alike);
+            // samples of a row are visited from column cols-1 down to 0 so that each funnel shift pushes the next lower bit
             const int rows = __reduce_max_sync(0xFFFFFFFFu, nr);
-            int a0 = E0 + 7 * sx0, a1 = E1 + 7 * sx1, a2 = E2 + 7 * sx2;
+            const int cols = __reduce_max_sync(0xFFFFFFFFu, nc);  // columns >= cols are masked off below for every lane
+            int a0 = E0 + (cols - 1) * sx0, a1 = E1 + (cols - 1) * sx1, a2 = E2 + (cols - 1) * sx2;
 #pragma unroll
             for (int r = 0; r < 8; ++r) {
                 if (r < rows) {
@@ -150,8 +170,10 @@ k_raster(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, co
                     int c0 = a0, c1 = a1, c2 = a2;
 #pragma unroll
                     for (int c = 7; c >= 0; --c) {
-                        bits = __funnelshift_l((uint32_t)(c0 | c1 | c2), bits, 1);
-                        c0 -= sx0; c1 -= sx1; c2 -= sx2;
+                        if (c < cols) {  // warp-uniform
+                            bits = __funnelshift_l((uint32_t)(c0 | c1 | c2), bits, 1);
+                            c0 -= sx0; c1 -= sx1; c2 -= sx2;
+                        }
                     }
                     bits = ~bits & 0xFFu;
                     if (r < 4) mlo |= bits << (8 * r); else mhi |= bits << (8 * (r - 4));
@@ -227,6 +249,8 @@ k_raster(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, co
             else vs_raster_large<long long>(X0, Y0, X1, Y1, X2, Y2, q0, q1, q2, __ll2float_rn(A2), bi0, bi1, bj0, bj1, px0, py0, kl, blid, lane);
         }
         __syncwarp();  // the slab is rewritten by the next batch
+        base = base1; gt = gt1; tri = tri1;
+        base1 = base2; gt1 = gt2;
     }
     __syncthreads();
 

@@ -149,8 +149,12 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     // ---------------- phase B: shade + composite ----------------
     const uint32_t oct = lane >> 3, oi = lane & 7;  // octet index (= pixel row) / lane within octet
     float4* ysm = reinterpret_cast<float4*>(per_warp + warp * 3584);                // [j][oct][4 chunks of 4 floats], swizzled
-    VsFragRec* rec = reinterpret_cast<VsFragRec*>(per_warp + warp * 3584 + 2048);   // [pixel]
-    float4* part = reinterpret_cast<float4*>(per_warp + warp * 3584 + 3072);        // [pixel] 4 channel logits
+    // record / logit slabs, one 16-byte chunk per pixel, pixel (row o, column j) at chunk 8 o + ((j + 2 o) & 7):
+    // the owners' stores (8 columns of one row) and the octets' accesses (4 rows of one column) are both conflict free
+    uint4* rec_o = reinterpret_cast<uint4*>(per_warp + warp * 3584 + 2048);         // texel offsets
+    float4* rec_w = reinterpret_cast<float4*>(per_warp + warp * 3584 + 2560);       // bilinear weights
+    float4* part = reinterpret_cast<float4*>(per_warp + warp * 3584 + 3072);        // 4 channel logits
+    const uint32_t own_slot = (lane & 24u) + (((lane & 7u) + 2u * (lane >> 3)) & 7u);
     {
         // SH basis of the owner's pixel -> row (j = column, oct = row); chunk q stored at q ^ (row >> 1) so that
         // the four octets' reads of one chunk fall into distinct banks
@@ -196,13 +200,14 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             }
         }
         if (COUNT && lane == 0) atomicAdd(&counters[VS_CNT_FRAGS], (unsigned long long)__popc(m));
-        rec[lane] = r;
+        rec_o[own_slot] = make_uint4(r.o00, r.o01, r.o10, r.o11);
+        rec_w[own_slot] = make_float4(r.w00, r.w01, r.w10, r.w11);
         __syncwarp();
         const uint4* __restrict__ tb = sc.tex[l] + SLOTS * oi;
 
         uint4 tv[2][SLOTS][4];
         auto issue = [&](int j, int b) {
-            const uint4 o = *reinterpret_cast<const uint4*>(&rec[8 * oct + j]);
+            const uint4 o = rec_o[8 * oct + ((j + 2 * oct) & 7)];
 #pragma unroll
             for (int s = 0; s < SLOTS; ++s) {
                 if (lane_on) {
@@ -218,7 +223,8 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
         for (int j = 0; j < 8; ++j) {
             if (j + 1 < 8) issue(j + 1, (j + 1) & 1);
             const int b = j & 1;
-            const float4 w = *(reinterpret_cast<const float4*>(&rec[8 * oct + j]) + 1);
+            const uint32_t slot = 8 * oct + ((j + 2 * oct) & 7);
+            const float4 w = rec_w[slot];
             const f32x2 W00 = vs_pack2(w.x, w.x), W01 = vs_pack2(w.y, w.y), W10 = vs_pack2(w.z, w.z), W11 = vs_pack2(w.w, w.w);
             const float4* yrow = ysm + (j * 4 + oct) * 4;
             f32x2 acc2 = 0ull;
@@ -243,11 +249,11 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             vs_unpack2(acc2, a0, a1);
             float acc = a0 + a1;
             if (LPC == 2) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, 1);
-            if (lane_on && (oi % LPC) == 0) reinterpret_cast<float*>(part)[(8 * oct + j) * 4 + oi / LPC] = acc;
+            if (lane_on && (oi % LPC) == 0) reinterpret_cast<float*>(part)[slot * 4 + oi / LPC] = acc;
         }
         __syncwarp();
         if (shade) {
-            const float4 s4 = part[lane];
+            const float4 s4 = part[own_slot];
             const float A = vs_sigmoid(s4.w);
             const float TA = Tr * A;
             Cr += TA * vs_sigmoid(s4.x); Cg += TA * vs_sigmoid(s4.y); Cb += TA * vs_sigmoid(s4.z);
