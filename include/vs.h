@@ -86,6 +86,10 @@ enum {
                                          triangle tested), same arithmetic and outputs; small scenes only */
     VS_FLAG_KERNEL_TIMING  = 1u << 1, /* bracket every kernel launch with CUDA events on the render stream
                                          and report per-stage device time in vs_render_stats              */
+    VS_FLAG_TILED_PATH     = 1u << 3, /* rasterise through per-tile triangle lists (count / scan / scatter binning
+                                         + one CTA per 16x16 tile with shared-memory keys) instead of the
+                                         default triangle-parallel path (64-bit max keys in HBM/L2); same
+                                         outputs bit for bit                                                */
     VS_FLAG_COUNT_TEXELS   = 1u << 2  /* measurement aid: count shaded fragments and, per view, the UNIQUE
                                          texels their 2x2 footprints reference (the algorithmic texture
                                          bytes of DESIGN.md §8); slower, not for timed runs                */

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libvs_b200.so")
 VS_OK, VS_ERR_INVALID_ARG, VS_ERR_OUT_OF_MEMORY, VS_ERR_CUDA, VS_ERR_UNSUPPORTED = range(5)
 VS_F32, VS_F16 = 0, 1
 VS_MEM_DEVICE, VS_MEM_HOST = 0, 1
-VS_FLAG_REFERENCE_PATH, VS_FLAG_KERNEL_TIMING, VS_FLAG_COUNT_TEXELS = 1, 2, 4
+VS_FLAG_REFERENCE_PATH, VS_FLAG_KERNEL_TIMING, VS_FLAG_COUNT_TEXELS, VS_FLAG_TILED_PATH = 1, 2, 4, 8
 MISS = 0xFFFFFFFF
 
 EXPORTS = ["vs_scene_create", "vs_render", "vs_render_host", "vs_query_last_render", "vs_scene_destroy",

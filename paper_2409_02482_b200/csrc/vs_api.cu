@@ -53,6 +53,8 @@ struct vs_scene {
     std::vector<void*> owned;
     // scratch, reused between calls
     DevBuf cams, vtx, tri_tiles, tile_count, tile_off, tile_cursor, tile_tris, ids, counters, texel_bits, stage_rgba[2], stage_ids[2];
+    DevBuf keys, big_list, big_count;  // direct path
+    bool keys_dirty = true;            // the key image holds something other than zeros (fresh allocation or an aborted pass)
     // per-call bookkeeping
     uint64_t launches = 0, raster_launches = 0, shade_launches = 0;
     struct Span { cudaEvent_t a, b; int stage; };
@@ -69,7 +71,7 @@ struct vs_scene {
     {
         for (void* p : owned) cudaFree(p);
         DevBuf* bufs[] = {&cams, &vtx, &tri_tiles, &tile_count, &tile_off, &tile_cursor, &tile_tris, &ids, &counters, &texel_bits,
-                          &stage_rgba[0], &stage_rgba[1], &stage_ids[0], &stage_ids[1]};
+                          &stage_rgba[0], &stage_rgba[1], &stage_ids[0], &stage_ids[1], &keys, &big_list, &big_count};
         for (cudaEvent_t e : event_pool) cudaEventDestroy(e);
         for (DevBuf* b : bufs) b->release();
         if (host_counters) cudaFreeHost(host_counters);
@@ -232,7 +234,7 @@ static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, u
     if (p->width > 16384 || p->height > 16384) return fail(VS_ERR_UNSUPPORTED, "image larger than 16384 px");
     if (!(p->near_plane > 0.0f) || !std::isfinite(p->near_plane)) return fail(VS_ERR_INVALID_ARG, "near_plane must be > 0");
     if (!(p->t_min >= 0.0f) || !std::isfinite(p->t_min)) return fail(VS_ERR_INVALID_ARG, "t_min must be >= 0");
-    if (p->flags & ~(uint32_t)(VS_FLAG_REFERENCE_PATH | VS_FLAG_KERNEL_TIMING | VS_FLAG_COUNT_TEXELS))
+    if (p->flags & ~(uint32_t)(VS_FLAG_REFERENCE_PATH | VS_FLAG_KERNEL_TIMING | VS_FLAG_COUNT_TEXELS | VS_FLAG_TILED_PATH))
         return fail(VS_ERR_INVALID_ARG, "reserved flag bits set");
     for (int i = 0; i < 3; ++i)
         if (!std::isfinite(p->background[i])) return fail(VS_ERR_INVALID_ARG, "background not finite");
@@ -248,10 +250,11 @@ static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, u
 static uint32_t pick_chunk(const vs_scene* s, const vs_render_params* p, uint32_t n)
 {
     if (p->views_per_chunk) return p->views_per_chunk < n ? p->views_per_chunk : n;
-    // keep the per-chunk scratch (transformed vertices, packed tile ranges, id planes) near 1 GB
-    const size_t per_view = (size_t)s->dev.v_total * 16 + (size_t)s->dev.t_total * 8 +
-                            (size_t)p->width * p->height * 4 * s->dev.k;
-    size_t c = ((size_t)1 << 30) / (per_view ? per_view : 1);
+    // keep the per-chunk scratch (transformed vertices, key image or packed tile ranges + id planes) near 1.5 GB
+    const bool tiled = (p->flags & VS_FLAG_TILED_PATH) != 0;
+    const size_t per_view = (size_t)s->dev.v_total * 16 + (tiled ? (size_t)s->dev.t_total * 8 : 0) +
+                            (size_t)p->width * p->height * (tiled ? 4 : 8) * s->dev.k;
+    size_t c = ((size_t)3 << 29) / (per_view ? per_view : 1);
     if (c < 1) c = 1;
     if (c > 16) c = 16;
     return (uint32_t)(c < n ? c : n);
@@ -291,11 +294,19 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
     const size_t ntile = (size_t)views * fr.tiles_x * fr.tiles_y;
     if (ntile >= (1ull << 31)) return fail(VS_ERR_UNSUPPORTED, "too many tiles in one chunk");
     const bool reference = (p->flags & VS_FLAG_REFERENCE_PATH) != 0;
+    const bool tiled = (p->flags & VS_FLAG_TILED_PATH) != 0;
     const size_t id_words = (size_t)views * s->dev.k * p->width * p->height;
 
     CU(s->cams.reserve(sizeof(VsCamDev) * views));
     CU(s->vtx.reserve((size_t)s->dev.v_total * views * 16 + 16));
-    if (!reference) {
+    if (!reference && !tiled) {
+        const size_t had = s->keys.cap;
+        CU(s->keys.reserve(id_words * 8 + 16));
+        if (s->keys.cap != had) s->keys_dirty = true;
+        CU(s->big_list.reserve((size_t)65536 * 8));
+        CU(s->big_count.reserve(16));
+    }
+    if (!reference && tiled) {
         CU(s->tri_tiles.reserve((size_t)s->dev.t_total * views * 4 + 16));
         CU(s->tile_count.reserve(ntile * 4));
         CU(s->tile_off.reserve((ntile + 1) * 4));
@@ -336,13 +347,43 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
         s->launches += 1;
         return VS_OK;
     }
-    CU(cudaMemsetAsync(ch.tile_count, 0, ntile * 4, st));
-    CU(cudaMemsetAsync(ch.tile_cursor, 0, ntile * 4, st));
+    if (tiled) {
+        CU(cudaMemsetAsync(ch.tile_count, 0, ntile * 4, st));
+        CU(cudaMemsetAsync(ch.tile_cursor, 0, ntile * 4, st));
+    }
     if (p->flags & VS_FLAG_COUNT_TEXELS) {
         const size_t words = (size_t)views * (s->dev.tex_bit_off[s->dev.k] >> 5);
         CU(s->texel_bits.reserve(words * 4 + 16));
         CU(cudaMemsetAsync(s->texel_bits.p, 0, words * 4, st));
         ch.texel_bits = (uint32_t*)s->texel_bits.p;
+    }
+    if (!tiled) {
+        // direct path: triangle-parallel raster into the key image, which k_shade reads and clears
+        ch.keys = (unsigned long long*)s->keys.p;
+        ch.big_list = (uint2*)s->big_list.p;
+        ch.big_count = (uint32_t*)s->big_count.p;
+        ch.big_capacity = 65536;
+        if (s->keys_dirty) CU(cudaMemsetAsync(s->keys.p, 0, s->keys.cap, st));
+        s->keys_dirty = true;
+        CU(cudaMemsetAsync(ch.big_count, 0, 4, st));
+        if ((r = span_begin(s, timing, 2, st)) != VS_OK) return r;
+        CU(vs_launch_raster_direct(s->dev, fr, ch, st));
+        if ((r = span_end(s, timing, st)) != VS_OK) return r;
+        if ((r = span_begin(s, timing, 3, st)) != VS_OK) return r;
+        CU(vs_launch_shade(s->dev, s->tex_f16, fr, ch, st));
+        if ((r = span_end(s, timing, st)) != VS_OK) return r;
+        s->keys_dirty = false;
+        s->launches += (s->dev.t_total ? 2 : 0) + 1;
+        s->raster_launches += 1;
+        s->shade_launches += 1;
+        if (ch.texel_bits) {
+            CU(vs_launch_popcount(ch.texel_bits, (size_t)views * (s->dev.tex_bit_off[s->dev.k] >> 5),
+                                  ch.counters + VS_CNT_TEXELS, st));
+            s->launches += 1;
+        }
+        const size_t scratch = s->cams.cap + s->vtx.cap + s->keys.cap + s->big_list.cap + s->big_count.cap;
+        if (scratch > s->scratch_peak) s->scratch_peak = scratch;
+        return VS_OK;
     }
     if ((r = span_begin(s, timing, 1, st)) != VS_OK) return r;
     CU(vs_launch_bin_count(s->dev, fr, ch, st));

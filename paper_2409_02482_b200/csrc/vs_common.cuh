@@ -236,12 +236,18 @@ struct VsChunk {                 // one pass over `views` cameras
     int ids_is_output;           // ids is the caller's AOV: empty tiles must be filled with MISS too
     float* out_rgba;             // DEVICE [views][H][W][4]
     uint32_t* texel_bits;        // DEVICE [views][tex_bit_off[k] / 32] or nullptr (VS_FLAG_COUNT_TEXELS)
+    // direct (untiled) path: non-null keys selects it in vs_launch_shade
+    unsigned long long* keys;    // DEVICE [views][k][H][W] max keys, zero between passes
+    uint2* big_list;             // DEVICE [big_capacity] {view, global triangle} with very large boxes
+    uint32_t* big_count;         // DEVICE entries appended this chunk (may exceed big_capacity: the rest was done in place)
+    uint32_t big_capacity;
 };
 
 cudaError_t vs_launch_transform(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_bin_count(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_bin_scan(const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_bin_scatter(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_raster_direct(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_raster(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_shade(const VsSceneDev& sc, int tex_f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_popcount(const uint32_t* words, size_t n, unsigned long long* counter, cudaStream_t st);

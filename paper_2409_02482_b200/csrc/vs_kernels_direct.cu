@@ -1,0 +1,278 @@
+// vs_kernels_direct.cu -- S2 + S4 without screen tiles: triangle-parallel coverage and per-layer
+// nearest-fragment resolve straight into a 64-bit key image in HBM/L2.  DESIGN.md §1, §3.2-3.4, §7.
+//
+// The paper-shaped scenes consist of triangles of a few pixels (C4: ~6 px each, 2.7 M per view).  For
+// those, binning every triangle into 16x16 tiles and re-gathering it per tile costs more than the
+// rasterisation itself, so this path visits every triangle exactly once:
+//   phase 1, lane = triangle: coalesced index record, three vertex gathers, integer setup, sample
+//     bounding box clipped to the screen.  A triangle whose box fits 8x8 samples gets its coverage mask
+//     from three biased int32 edge functions stepped with exact adds (same arithmetic as k_raster) and
+//     leaves a 12-word record in the warp's shared-memory slab.
+//   phase 2, lane = covered sample: the warp's masks are compacted into a queue of (lane, sample) codes so
+//     that all 32 lanes evaluate one covered sample each: fp32-exact depth key (IEEE division) and one
+//     fire-and-forget 64-bit max (RED.MAX.U64) on keys[view][layer][y][x].  The maximum is order
+//     independent, so the key image is the same whatever the scheduling (reading Q18).
+//   larger triangles are broadcast one at a time and the warp maps its lanes to 8x4 pixel chunks of the
+//     box; triangles whose box exceeds VS_BIG_SAMPLES samples are appended to a list that k_raster_big
+//     spreads over the whole grid.
+// The key image must be zero on entry; k_shade reads it (id = ~low word) and clears what it read.
+#include "vs_common.cuh"
+
+#define VS_RD_FIELDS 12
+#define VS_RD_QUEUE 512u
+#define VS_RD_WARP_WORDS (VS_RD_FIELDS * 32 + 256)
+#define VS_BIG_SAMPLES 4096   // clipped-box samples above which a triangle goes to the big list
+
+__device__ __forceinline__ void vs_key_red(unsigned long long* slot, unsigned long long key)
+{
+    asm volatile("red.global.max.u64 [%0], %1;" ::"l"(slot), "l"(key) : "memory");
+}
+
+__device__ __forceinline__ float vs_depth_div(float f0, float f1, float f2, float q0, float q1, float q2, float fA)
+{
+    const float num = __fmaf_rn(f2, q2, __fmaf_rn(f1, q1, __fmul_rn(f0, q0)));
+    return __fdiv_rn(num, fA);
+}
+
+// Whole warp, lane = pixel of an 8x4 chunk of the box [i0,i1] x [j0,j1]; chunks c = first, first+stride, ...
+template <typename I>
+__device__ __forceinline__ void vs_direct_large(int X0, int Y0, int X1, int Y1, int X2, int Y2, float q0, float q1, float q2,
+                                                float fA, int i0, int i1, int j0, int j1, int W,
+                                                unsigned long long* __restrict__ plane, uint32_t lid, uint32_t lane,
+                                                uint32_t first, uint32_t stride)
+{
+    const int dx0 = X2 - X1, dy0 = Y2 - Y1, dx1 = X0 - X2, dy1 = Y0 - Y2, dx2 = X1 - X0, dy2 = Y1 - Y0;
+    const int m0 = ((dy0 < 0) || (dy0 == 0 && dx0 > 0)) ? 0 : 1;
+    const int m1 = ((dy1 < 0) || (dy1 == 0 && dx1 > 0)) ? 0 : 1;
+    const int m2 = ((dy2 < 0) || (dy2 == 0 && dx2 > 0)) ? 0 : 1;
+    const uint32_t ncx = (uint32_t)(i1 - i0 + 8) >> 3, ncy = (uint32_t)(j1 - j0 + 4) >> 2;
+    for (uint32_t c = first; c < ncx * ncy; c += stride) {
+        const int i = i0 + (int)(c % ncx) * 8 + (int)(lane & 7), j = j0 + (int)(c / ncx) * 4 + (int)(lane >> 3);
+        if (i > i1 || j > j1) continue;
+        const int Sx = 256 * i + 128, Sy = 256 * j + 128;
+        const I e0 = (I)dx0 * (I)(Sy - Y1) - (I)dy0 * (I)(Sx - X1);
+        const I e1 = (I)dx1 * (I)(Sy - Y2) - (I)dy1 * (I)(Sx - X2);
+        const I e2 = (I)dx2 * (I)(Sy - Y0) - (I)dy2 * (I)(Sx - X0);
+        if (e0 >= (I)m0 && e1 >= (I)m1 && e2 >= (I)m2) {
+            float f0, f1, f2;
+            if (sizeof(I) == 4) { f0 = __int2float_rn((int)e0); f1 = __int2float_rn((int)e1); f2 = __int2float_rn((int)e2); }
+            else { f0 = __ll2float_rn((long long)e0); f1 = __ll2float_rn((long long)e1); f2 = __ll2float_rn((long long)e2); }
+            const float qp = vs_depth_div(f0, f1, f2, q0, q1, q2, fA);
+            vs_key_red(&plane[(size_t)j * W + i], vs_make_key(qp, lid));
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256)
+k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, unsigned long long* __restrict__ keys,
+                uint2* __restrict__ big_list, uint32_t* __restrict__ big_count, uint32_t big_capacity,
+                unsigned long long* __restrict__ counters)
+{
+    __shared__ int slab[8 * VS_RD_WARP_WORDS];
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t view = blockIdx.y;
+    const uint32_t gt = blockIdx.x * 256u + tid;
+    const int W = (int)fr.width, H = (int)fr.height;
+    const size_t plane_px = (size_t)W * H;
+    int* rec = slab + warp * VS_RD_WARP_WORDS;                                            // [field][lane]
+    unsigned short* queue = reinterpret_cast<unsigned short*>(rec + VS_RD_FIELDS * 32);   // [512]
+    const int4* __restrict__ vv = vtx + (size_t)view * sc.v_total;
+    unsigned long long* __restrict__ vkeys = keys + (size_t)view * sc.k * plane_px;
+
+    // ---------------- phase 1: lane = triangle ----------------
+    VsTri T;
+    int i0 = 0, i1 = -1, j0 = 0, j1 = -1, status = -1;
+    uint32_t layer = 0, lid = 0;
+    bool narrow = false, valid = false, large = false;
+    if (gt < sc.t_total) {
+        const uint4 tri = __ldg(&sc.tris[gt]);
+        const int4 a = __ldg(&vv[tri.x]), b = __ldg(&vv[tri.y]), c = __ldg(&vv[tri.z]);
+        status = vs_setup_tri(a, b, c, T);
+        if (status == 0) {
+            const int minX = min(T.X0, min(T.X1, T.X2)), maxX = max(T.X0, max(T.X1, T.X2));
+            const int minY = min(T.Y0, min(T.Y1, T.Y2)), maxY = max(T.Y0, max(T.Y1, T.Y2));
+            i0 = max((minX + 127) >> 8, 0); i1 = min((maxX - 128) >> 8, W - 1);
+            j0 = max((minY + 127) >> 8, 0); j1 = min((maxY - 128) >> 8, H - 1);
+            layer = tri.w; lid = gt - sc.tri_off[layer];
+            narrow = maxX - minX < 8192 && maxY - minY < 8192;  // every int32 intermediate < 2^28
+            valid = i0 <= i1 && j0 <= j1;
+            large = valid && !(narrow && i1 - i0 < 8 && j1 - j0 < 8);
+        }
+    }
+    {
+        const unsigned dropped = __popc(__ballot_sync(0xFFFFFFFFu, status == 1));
+        const unsigned degen = __popc(__ballot_sync(0xFFFFFFFFu, status == 2));
+        if (lane == 0) {
+            if (dropped) atomicAdd(&counters[VS_CNT_DROPPED], (unsigned long long)dropped);
+            if (degen) atomicAdd(&counters[VS_CNT_DEGENERATE], (unsigned long long)degen);
+        }
+    }
+    uint32_t mlo = 0, mhi = 0;  // coverage of the clipped box, sample (r, c) -> bit 8r + c of mhi:mlo
+    int E0 = 0, E1 = 0, E2 = 0, sx0 = 0, sx1 = 0, sx2 = 0, sy0 = 0, sy1 = 0, sy2 = 0;
+    const bool small = valid && !large;
+    if (small) {
+        // edge e_i runs (i+1) -> (i+2) and weights vertex i; sample (i0, j0)
+        const int dx0 = T.X2 - T.X1, dy0 = T.Y2 - T.Y1, dx1 = T.X0 - T.X2, dy1 = T.Y0 - T.Y2;
+        const int dx2 = T.X1 - T.X0, dy2 = T.Y1 - T.Y0;
+        const int Sx = 256 * i0 + 128, Sy = 256 * j0 + 128;
+        E0 = dx0 * (Sy - T.Y1) - dy0 * (Sx - T.X1);
+        E1 = dx1 * (Sy - T.Y2) - dy1 * (Sx - T.X2);
+        E2 = dx2 * (Sy - T.Y0) - dy2 * (Sx - T.X0);
+        sx0 = -256 * dy0; sx1 = -256 * dy1; sx2 = -256 * dy2;  // one pixel in +x
+        sy0 = 256 * dx0; sy1 = 256 * dx1; sy2 = 256 * dx2;     // one pixel in +y
+        rec[0 * 32 + lane] = E0; rec[1 * 32 + lane] = E1;
+        rec[2 * 32 + lane] = sx0; rec[3 * 32 + lane] = sx1;
+        rec[4 * 32 + lane] = sy0; rec[5 * 32 + lane] = sy1;
+        rec[6 * 32 + lane] = (int)T.A2;
+        rec[7 * 32 + lane] = __float_as_int(T.q0); rec[8 * 32 + lane] = __float_as_int(T.q1);
+        rec[9 * 32 + lane] = __float_as_int(T.q2);
+        rec[10 * 32 + lane] = (int)lid;
+        rec[11 * 32 + lane] = (int)((uint32_t)(layer * plane_px) + (uint32_t)(j0 * W + i0));  // < 2^32: checked by the launcher
+        // covered <=> E_e > 0 || (E_e == 0 && topleft_e) <=> F_e := E_e - (topleft_e ? 0 : 1) >= 0
+        E0 -= ((dy0 < 0) || (dy0 == 0 && dx0 > 0)) ? 0 : 1;
+        E1 -= ((dy1 < 0) || (dy1 == 0 && dx1 > 0)) ? 0 : 1;
+        E2 -= ((dy2 < 0) || (dy2 == 0 && dx2 > 0)) ? 0 : 1;
+    }
+    const int nr = small ? j1 - j0 + 1 : 0, nc = small ? i1 - i0 + 1 : 0;
+    {
+        // rows of up to 8 samples, row and column counts uniform over the warp (the lanes' boxes are alike);
+        // samples of a row are visited from column cols-1 down to 0 so that each funnel shift pushes the next lower bit
+        const int rows = __reduce_max_sync(0xFFFFFFFFu, nr);
+        const int cols = __reduce_max_sync(0xFFFFFFFFu, nc);
+        int a0 = E0 + (cols - 1) * sx0, a1 = E1 + (cols - 1) * sx1, a2 = E2 + (cols - 1) * sx2;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) {
+            if (r < rows) {
+                uint32_t bits = 0;
+                int c0 = a0, c1 = a1, c2 = a2;
+#pragma unroll
+                for (int c = 7; c >= 0; --c) {
+                    if (c < cols) {  // warp-uniform
+                        bits = __funnelshift_l((uint32_t)(c0 | c1 | c2), bits, 1);
+                        c0 -= sx0; c1 -= sx1; c2 -= sx2;
+                    }
+                }
+                bits = ~bits & 0xFFu;
+                if (r < 4) mlo |= bits << (8 * r); else mhi |= bits << (8 * (r - 4));
+                a0 += sy0; a1 += sy1; a2 += sy2;
+            }
+        }
+        const uint32_t colm = 0x01010101u * ((1u << nc) - 1u);
+        mlo &= colm & (nr >= 4 ? 0xFFFFFFFFu : ((1u << (8 * nr)) - 1u));
+        mhi &= colm & (nr >= 8 ? 0xFFFFFFFFu : (nr > 4 ? ((1u << (8 * (nr - 4))) - 1u) : 0u));
+    }
+    // ---------------- compaction: (lane, bit) codes of the covered samples ----------------
+    const uint32_t cnt = (uint32_t)(__popc(mlo) + __popc(mhi));
+    uint32_t incl = cnt;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+        if (lane >= (uint32_t)o) incl += u;
+    }
+    const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
+    for (uint32_t win = 0; win < total; win += VS_RD_QUEUE) {  // one round unless the warp covers > 512 samples
+        {
+            uint32_t off = incl - cnt - win;  // wraps for codes in front of the window: fails the bound test
+            uint32_t m = mlo;
+            while (m) {
+                const int bit = __ffs(m) - 1;
+                m &= m - 1;
+                if (off < VS_RD_QUEUE) queue[off] = (unsigned short)((lane << 6) | (uint32_t)bit);
+                ++off;
+            }
+            m = mhi;
+            while (m) {
+                const int bit = __ffs(m) - 1;
+                m &= m - 1;
+                if (off < VS_RD_QUEUE) queue[off] = (unsigned short)((lane << 6) | 32u | (uint32_t)bit);
+                ++off;
+            }
+        }
+        __syncwarp();
+        // ---------------- phase 2: lane = covered sample ----------------
+        const uint32_t n = min(total - win, (uint32_t)VS_RD_QUEUE);
+        for (uint32_t s = lane; s < n; s += 32) {
+            const uint32_t code = queue[s];
+            const uint32_t src = code >> 6;
+            const int r = (int)((code >> 3) & 7u), c = (int)(code & 7u);
+            const int e0 = rec[0 * 32 + src] + r * rec[4 * 32 + src] + c * rec[2 * 32 + src];
+            const int e1 = rec[1 * 32 + src] + r * rec[5 * 32 + src] + c * rec[3 * 32 + src];
+            const int A2 = rec[6 * 32 + src];
+            const int e2 = A2 - e0 - e1;  // E0 + E1 + E2 == A2 at every point
+            const float qp = vs_depth_div(__int2float_rn(e0), __int2float_rn(e1), __int2float_rn(e2),
+                                          __int_as_float(rec[7 * 32 + src]), __int_as_float(rec[8 * 32 + src]),
+                                          __int_as_float(rec[9 * 32 + src]), __int2float_rn(A2));
+            vs_key_red(&vkeys[(uint32_t)rec[11 * 32 + src] + (uint32_t)(r * W + c)], vs_make_key(qp, (uint32_t)rec[10 * 32 + src]));
+        }
+        __syncwarp();
+    }
+    // ---------------- large triangles ----------------
+    bool big = false;
+    if (large) {
+        const unsigned long long samples = (unsigned long long)(i1 - i0 + 1) * (unsigned long long)(j1 - j0 + 1);
+        if (samples > VS_BIG_SAMPLES) {
+            const uint32_t slot = atomicAdd(big_count, 1u);
+            if (slot < big_capacity) { big_list[slot] = make_uint2(view, gt); big = true; }
+        }
+    }
+    uint32_t lm = __ballot_sync(0xFFFFFFFFu, large && !big);
+    while (lm) {
+        const int src = __ffs(lm) - 1;
+        lm &= lm - 1;
+        const int X0 = __shfl_sync(0xFFFFFFFFu, T.X0, src), Y0 = __shfl_sync(0xFFFFFFFFu, T.Y0, src);
+        const int X1 = __shfl_sync(0xFFFFFFFFu, T.X1, src), Y1 = __shfl_sync(0xFFFFFFFFu, T.Y1, src);
+        const int X2 = __shfl_sync(0xFFFFFFFFu, T.X2, src), Y2 = __shfl_sync(0xFFFFFFFFu, T.Y2, src);
+        const float q0 = __shfl_sync(0xFFFFFFFFu, T.q0, src), q1 = __shfl_sync(0xFFFFFFFFu, T.q1, src);
+        const float q2 = __shfl_sync(0xFFFFFFFFu, T.q2, src);
+        const long long A2 = __shfl_sync(0xFFFFFFFFu, T.A2, src);
+        const int bi0 = __shfl_sync(0xFFFFFFFFu, i0, src), bi1 = __shfl_sync(0xFFFFFFFFu, i1, src);
+        const int bj0 = __shfl_sync(0xFFFFFFFFu, j0, src), bj1 = __shfl_sync(0xFFFFFFFFu, j1, src);
+        const uint32_t blid = __shfl_sync(0xFFFFFFFFu, lid, src), blayer = __shfl_sync(0xFFFFFFFFu, layer, src);
+        const bool bnarrow = __shfl_sync(0xFFFFFFFFu, (int)narrow, src) != 0;
+        unsigned long long* plane = vkeys + blayer * plane_px;
+        if (bnarrow) vs_direct_large<int>(X0, Y0, X1, Y1, X2, Y2, q0, q1, q2, __ll2float_rn(A2), bi0, bi1, bj0, bj1, W, plane, blid, lane, 0u, 1u);
+        else vs_direct_large<long long>(X0, Y0, X1, Y1, X2, Y2, q0, q1, q2, __ll2float_rn(A2), bi0, bi1, bj0, bj1, W, plane, blid, lane, 0u, 1u);
+    }
+}
+
+// Triangles with very large clipped boxes (full-screen quads, close-ups of coarse meshes): every entry of
+// the list is rasterised by ALL warps of the grid, warp w taking the 8x4 chunks w, w + warps, ...
+__global__ void __launch_bounds__(256)
+k_raster_big(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, unsigned long long* __restrict__ keys,
+             const uint2* __restrict__ big_list, const uint32_t* __restrict__ big_count, uint32_t big_capacity)
+{
+    const uint32_t lane = threadIdx.x & 31;
+    const uint32_t gw = blockIdx.x * 8u + (threadIdx.x >> 5), warps = gridDim.x * 8u;
+    const uint32_t n = min(*big_count, big_capacity);
+    const int W = (int)fr.width, H = (int)fr.height;
+    const size_t plane_px = (size_t)W * H;
+    for (uint32_t e = 0; e < n; ++e) {
+        const uint2 ent = __ldg(&big_list[e]);
+        const uint4 tri = __ldg(&sc.tris[ent.y]);
+        const int4* __restrict__ vv = vtx + (size_t)ent.x * sc.v_total;
+        VsTri T;
+        if (vs_setup_tri(__ldg(&vv[tri.x]), __ldg(&vv[tri.y]), __ldg(&vv[tri.z]), T) != 0) continue;
+        int i0, i1, j0, j1;
+        if (!vs_tri_pixel_bbox(T, W, H, i0, i1, j0, j1)) continue;
+        const int minX = min(T.X0, min(T.X1, T.X2)), maxX = max(T.X0, max(T.X1, T.X2));
+        const int minY = min(T.Y0, min(T.Y1, T.Y2)), maxY = max(T.Y0, max(T.Y1, T.Y2));
+        const bool narrow = maxX - minX < 8192 && maxY - minY < 8192;
+        unsigned long long* plane = keys + ((size_t)ent.x * sc.k + tri.w) * plane_px;
+        const uint32_t lid = ent.y - sc.tri_off[tri.w];
+        if (narrow) vs_direct_large<int>(T.X0, T.Y0, T.X1, T.Y1, T.X2, T.Y2, T.q0, T.q1, T.q2, __ll2float_rn(T.A2), i0, i1, j0, j1, W, plane, lid, lane, gw, warps);
+        else vs_direct_large<long long>(T.X0, T.Y0, T.X1, T.Y1, T.X2, T.Y2, T.q0, T.q1, T.q2, __ll2float_rn(T.A2), i0, i1, j0, j1, W, plane, lid, lane, gw, warps);
+    }
+}
+
+cudaError_t vs_launch_raster_direct(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
+{
+    if (sc.t_total == 0) return cudaSuccess;
+    // key offsets inside one view are carried as uint32
+    if ((unsigned long long)sc.k * fr.width * fr.height >= (1ull << 32)) return cudaErrorInvalidValue;
+    dim3 grid((sc.t_total + 255) / 256, ch.views);
+    k_raster_direct<<<grid, 256, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.big_list, ch.big_count, ch.big_capacity, ch.counters);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    k_raster_big<<<148 * 4, 256, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.big_list, ch.big_count, ch.big_capacity);
+    return cudaGetLastError();
+}

@@ -23,6 +23,17 @@ struct __align__(16) VsFragRec {
     float w00, w01, w10, w11;     // bilinear weights (all 0: no fragment)
 };
 
+#ifndef VS_SHADE_PREFETCH
+#define VS_SHADE_PREFETCH 2   // 0: off, 1: left column of the footprint, 2: all four texels
+#endif
+#ifndef VS_SHADE_PF_DIST
+#define VS_SHADE_PF_DIST 1    // layers between the prefetch of a footprint and its use
+#endif
+__device__ __forceinline__ void vs_prefetch_l2(const void* p)
+{
+    asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
+}
+
 // ---- packed fp32 pairs (sm_100: FFMA2 / FMUL2) -------------------------------------------------
 typedef unsigned long long f32x2;
 
@@ -86,7 +97,8 @@ struct VsShadeShape {
 template <int F16, int DEG, bool COUNT>
 __global__ void __launch_bounds__(256, 3)
 k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams, const int4* __restrict__ vtx,
-        const uint32_t* __restrict__ tile_off, const uint32_t* __restrict__ ids, float* __restrict__ out_rgba,
+        const uint32_t* __restrict__ tile_off, const uint32_t* __restrict__ ids, unsigned long long* __restrict__ keys,
+        uint32_t* __restrict__ out_ids, float* __restrict__ out_rgba,
         uint32_t* __restrict__ texel_bits, unsigned long long* __restrict__ counters)
 {
     typedef VsShadeShape<F16, DEG> S;
@@ -108,7 +120,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     const bool inimg = px < W && py < H;
     const size_t pix = ((size_t)view * H + py) * W + px;
 
-    if (tile_off[view * tiles + tile] == tile_off[view * tiles + tile + 1]) {  // nothing binned here: background
+    if (tile_off && tile_off[view * tiles + tile] == tile_off[view * tiles + tile + 1]) {  // nothing binned here: background
         if (inimg) reinterpret_cast<float4*>(out_rgba)[pix] = make_float4(fr.bg[0], fr.bg[1], fr.bg[2], 0.0f);
         return;
     }
@@ -116,12 +128,26 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
 
     // ---------------- phase A: fragment records of all layers ----------------
     const size_t plane = (size_t)W * H;
-    const uint32_t* idp = ids + (size_t)view * sc.k * plane + (size_t)py * W + px;
+    const size_t pix0 = (size_t)view * sc.k * plane + (size_t)py * W + px;
+    const uint32_t* idp = ids + pix0;
     bool any_hit = false;
     for (uint32_t l0 = 0; l0 < sc.k; l0 += 3) {
         uint32_t id[3];
+        if (keys) {
+            // direct path: the key image of k_raster_direct; what is read is cleared for the next pass over this buffer
+            unsigned long long key[3];
 #pragma unroll
-        for (int u = 0; u < 3; ++u) id[u] = (inimg && l0 + u < sc.k) ? __ldg(idp + (size_t)(l0 + u) * plane) : VS_MISS;
+            for (int u = 0; u < 3; ++u) key[u] = (inimg && l0 + u < sc.k) ? keys[pix0 + (size_t)(l0 + u) * plane] : 0ull;
+#pragma unroll
+            for (int u = 0; u < 3; ++u) {
+                id[u] = key[u] ? 0xFFFFFFFFu - (uint32_t)key[u] : VS_MISS;
+                if (key[u]) keys[pix0 + (size_t)(l0 + u) * plane] = 0ull;
+                if (out_ids && inimg && l0 + u < sc.k) out_ids[pix0 + (size_t)(l0 + u) * plane] = id[u];
+            }
+        } else {
+#pragma unroll
+            for (int u = 0; u < 3; ++u) id[u] = (inimg && l0 + u < sc.k) ? __ldg(idp + (size_t)(l0 + u) * plane) : VS_MISS;
+        }
 #pragma unroll
         for (int u = 0; u < 3; ++u) {
             if (l0 + u < sc.k) {
@@ -140,6 +166,21 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
         }
     }
     // each thread reads back only its own records: no barrier needed
+    // pull the footprint of this pixel in layer `ln` into L2 (issued VS_SHADE_PF_DIST layers ahead of its use)
+    auto prefetch_layer = [&](uint32_t ln) {
+        const float2 abn = rec_ab[ln * VS_TILE_PIX + tid];
+        if (abn.x >= 0.0f) {
+            const uint32_t xy = rec_xy[ln * VS_TILE_PIX + tid];
+            const uint32_t cx0 = xy & 0x7FFFu, cy0 = (xy >> 16) & 0x7FFFu, Wt = sc.tex_w[ln];
+            const uint4* p0 = sc.tex[ln] + (size_t)(cy0 * Wt + cx0) * S::NVEC;
+            const uint4* p1 = p0 + ((xy >> 31) ? (size_t)Wt * S::NVEC : (size_t)0);
+            const uint32_t dx = ((xy >> 15) & 1u) * S::NVEC;
+            vs_prefetch_l2(p0); vs_prefetch_l2(p1);
+            if (VS_SHADE_PREFETCH > 1) { vs_prefetch_l2(p0 + dx); vs_prefetch_l2(p1 + dx); }
+        }
+    };
+    if (VS_SHADE_PREFETCH)
+        for (uint32_t ln = 0; ln < VS_SHADE_PF_DIST && ln < sc.k; ++ln) prefetch_layer(ln);
 
     if (!__any_sync(0xFFFFFFFFu, any_hit)) {
         if (inimg) reinterpret_cast<float4*>(out_rgba)[pix] = make_float4(fr.bg[0], fr.bg[1], fr.bg[2], 0.0f);
@@ -219,6 +260,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             }
         };
         issue(0, 0);
+        if (VS_SHADE_PREFETCH && l + VS_SHADE_PF_DIST < sc.k && alive) prefetch_layer(l + VS_SHADE_PF_DIST);
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
             if (j + 1 < 8) issue(j + 1, (j + 1) & 1);
@@ -274,7 +316,12 @@ static cudaError_t launch_sh2(const VsSceneDev& sc, const VsFrame& fr, const VsC
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     dim3 grid(fr.tiles_x * fr.tiles_y, ch.views);
-    kern<<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_off, ch.ids, ch.out_rgba, ch.texel_bits, ch.counters);
+    if (ch.keys)
+        kern<<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, nullptr, nullptr, ch.keys, ch.ids_is_output ? ch.ids : nullptr,
+                                      ch.out_rgba, ch.texel_bits, ch.counters);
+    else
+        kern<<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_off, ch.ids, nullptr, nullptr, ch.out_rgba, ch.texel_bits,
+                                      ch.counters);
     return cudaGetLastError();
 }
 

@@ -12,21 +12,24 @@ pytestmark = pytest.mark.gpu
 TOL = 1e-4
 
 
-@pytest.fixture(scope="module")
-def env():
+@pytest.fixture(scope="module", params=["direct", "tiled"])
+def env(request):
+    """Every test runs on both raster paths: the default triangle-parallel one (64-bit max keys in HBM/L2)
+    and the per-tile one behind VS_FLAG_TILED_PATH (binning + shared-memory keys)."""
     import torch
     assert torch.cuda.is_available(), "these tests need the B200"
     import oracle
     from paper_2409_02482_b200 import binding, synth
     binding.load_library()
-    return types.SimpleNamespace(torch=torch, oracle=oracle, binding=binding, synth=synth)
+    return types.SimpleNamespace(torch=torch, oracle=oracle, binding=binding, synth=synth,
+                                 path_flags=binding.VS_FLAG_TILED_PATH if request.param == "tiled" else 0)
 
 
 def gpu_render(env, sc, views, flags=0, t_min=None, background=None, views_per_chunk=0, want_ids=True):
     b = env.binding
     r = b.Renderer(sc)
     p = b.make_params(sc.width, sc.height, sc.near_plane, sc.t_min if t_min is None else t_min,
-                      sc.background if background is None else background, flags, views_per_chunk)
+                      sc.background if background is None else background, flags | env.path_flags, views_per_chunk)
     rgba, ids = r.render(sc.cameras[list(views)], p, want_ids=want_ids)
     env.torch.cuda.synchronize()
     stats = r.stats()
