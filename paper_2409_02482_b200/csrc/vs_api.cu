@@ -134,10 +134,11 @@ static vs_status scene_create_impl(const vs_scene_desc* desc, cudaStream_t st, v
         if (L.tex_w > 32768 || L.tex_h > 32768 || (uint64_t)L.tex_w * L.tex_h * d.texel_vecs >= (1ull << 32))
             return fail(VS_ERR_UNSUPPORTED, "layer %u: texture %ux%u too large", l, L.tex_w, L.tex_h);
         d.tri_off[l] = (uint32_t)tt;
+        d.vtx_off[l] = (uint32_t)vt;
         vt += L.num_vertices; tt += L.num_triangles;
         if (vt >= (1ull << 31) || tt >= (1ull << 31)) return fail(VS_ERR_UNSUPPORTED, "scene too large");
     }
-    for (uint32_t l = k; l <= VS_MAX_LAYERS; ++l) d.tri_off[l] = (uint32_t)tt;
+    for (uint32_t l = k; l <= VS_MAX_LAYERS; ++l) { d.tri_off[l] = (uint32_t)tt; d.vtx_off[l] = (uint32_t)vt; }
     uint64_t bits = 0;
     for (uint32_t l = 0; l <= VS_MAX_LAYERS; ++l) {
         d.tex_bit_off[l] = (uint32_t)bits;
@@ -303,6 +304,7 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
         const size_t had = s->keys.cap;
         CU(s->keys.reserve(id_words * 8 + 16));
         if (s->keys.cap != had) s->keys_dirty = true;
+        CU(s->tile_count.reserve((size_t)views * VS_MAX_LAYERS * 16));   // per-(view, layer) vertex bounding boxes
         CU(s->big_list.reserve((size_t)65536 * 8));
         CU(s->big_count.reserve(16));
     }
@@ -338,6 +340,10 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
     const bool timing = (p->flags & VS_FLAG_KERNEL_TIMING) != 0;
     vs_status r;
     CU(cudaMemcpyAsync(s->cams.p, cams, sizeof(VsCamDev) * views, cudaMemcpyHostToDevice, st));
+    if (!reference && !tiled) {
+        ch.rects = (int*)s->tile_count.p;
+        CU(cudaMemsetAsync(ch.rects, 0x80, (size_t)views * s->dev.k * 16, st));  // every int = -2139062144
+    }
     if ((r = span_begin(s, timing, 0, st)) != VS_OK) return r;
     CU(vs_launch_transform(s->dev, fr, ch, st));
     if ((r = span_end(s, timing, st)) != VS_OK) return r;
@@ -381,7 +387,7 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
                                   ch.counters + VS_CNT_TEXELS, st));
             s->launches += 1;
         }
-        const size_t scratch = s->cams.cap + s->vtx.cap + s->keys.cap + s->big_list.cap + s->big_count.cap;
+        const size_t scratch = s->cams.cap + s->vtx.cap + s->keys.cap + s->big_list.cap + s->big_count.cap + s->tile_count.cap;
         if (scratch > s->scratch_peak) s->scratch_peak = scratch;
         return VS_OK;
     }

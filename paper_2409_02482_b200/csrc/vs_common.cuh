@@ -23,6 +23,7 @@ struct VsSceneDev {
     uint32_t texel_vecs;                  // 16-byte vectors per texel in the internal layout (= 4 * np_pad * elem / 16)
     uint32_t np_pad;                      // coefficients per channel row of the internal layout [texel][ch][np_pad]
     uint32_t tri_off[VS_MAX_LAYERS + 1];  // global triangle id of each layer's triangle 0
+    uint32_t vtx_off[VS_MAX_LAYERS + 1];  // global vertex index of each layer's vertex 0
     const uint4* tex[VS_MAX_LAYERS];      // [tex_h][tex_w][texel_vecs] 16-byte vectors
     uint32_t tex_w[VS_MAX_LAYERS], tex_h[VS_MAX_LAYERS];
     uint32_t tex_bit_off[VS_MAX_LAYERS + 1];  // VS_FLAG_COUNT_TEXELS: first bitmap bit of each layer (multiple of 32)
@@ -241,6 +242,7 @@ struct VsChunk {                 // one pass over `views` cameras
     uint2* big_list;             // DEVICE [big_capacity] {view, global triangle} with very large boxes
     uint32_t* big_count;         // DEVICE entries appended this chunk (may exceed big_capacity: the rest was done in place)
     uint32_t big_capacity;
+    int* rects;                  // DEVICE [views][k][4] = max of {-X, -Y, X, Y} over the layer's valid snapped vertices (bytes 0x80 on entry)
 };
 
 cudaError_t vs_launch_transform(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);

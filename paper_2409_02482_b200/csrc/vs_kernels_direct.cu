@@ -63,7 +63,10 @@ __device__ __forceinline__ void vs_direct_large(int X0, int Y0, int X1, int Y1, 
     }
 }
 
-__global__ void __launch_bounds__(256)
+#ifndef VS_RD_MIN_CTAS
+#define VS_RD_MIN_CTAS 4
+#endif
+__global__ void __launch_bounds__(256, VS_RD_MIN_CTAS)
 k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, unsigned long long* __restrict__ keys,
                 uint2* __restrict__ big_list, uint32_t* __restrict__ big_count, uint32_t big_capacity,
                 unsigned long long* __restrict__ counters)

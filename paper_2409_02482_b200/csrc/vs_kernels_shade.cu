@@ -16,6 +16,7 @@
 //   (fma.rn.f32x2 -> FFMA2); the one or two lanes of a channel are summed with one shuffle and the
 //   four channel logits go back to the owner through shared memory.  Owners apply the sigmoid and
 //   composite front to back in registers.
+#include <climits>
 #include "vs_common.cuh"
 
 struct __align__(16) VsFragRec {
@@ -120,7 +121,24 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     const bool inimg = px < W && py < H;
     const size_t pix = ((size_t)view * H + py) * W + px;
 
-    if (tile_off && tile_off[view * tiles + tile] == tile_off[view * tiles + tile + 1]) {  // nothing binned here: background
+    // tiled path: tile_off = reference list offsets; direct path: tile_off = per-(view, layer) bounding boxes of the
+    // snapped vertices (k_transform), turned into the mask of layers that can have fragments in this tile
+    uint32_t lmask = 0xFFFFFFFFu;
+    if (keys) {
+        const int tx0 = (int)(tile % fr.tiles_x) * VS_TILE_W, ty0 = (int)(tile / fr.tiles_x) * VS_TILE_H;
+        const int* rc = reinterpret_cast<const int*>(tile_off) + (size_t)view * sc.k * 4;
+        lmask = 0u;
+        for (uint32_t l = 0; l < sc.k; ++l) {
+            const int4 e = *reinterpret_cast<const int4*>(rc + 4 * l);  // max of {-X, -Y, X, Y}
+            if (e.z < -(1 << 24)) continue;                              // still the fill value: no valid vertex
+            // pixel columns / rows whose samples lie inside the box (same rounding as the triangle boxes)
+            const int i0 = (-e.x + 127) >> 8, i1 = (e.z - 128) >> 8, j0 = (-e.y + 127) >> 8, j1 = (e.w - 128) >> 8;
+            if (i0 <= tx0 + VS_TILE_W - 1 && i1 >= tx0 && j0 <= ty0 + VS_TILE_H - 1 && j1 >= ty0) lmask |= 1u << l;
+        }
+    }
+    if (keys ? lmask == 0u : tile_off[view * tiles + tile] == tile_off[view * tiles + tile + 1]) {  // nothing drawn here: background
+        if (out_ids && inimg)
+            for (uint32_t l = 0; l < sc.k; ++l) out_ids[((size_t)view * sc.k + l) * ((size_t)W * H) + (size_t)py * W + px] = VS_MISS;
         if (inimg) reinterpret_cast<float4*>(out_rgba)[pix] = make_float4(fr.bg[0], fr.bg[1], fr.bg[2], 0.0f);
         return;
     }
@@ -137,7 +155,8 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             // direct path: the key image of k_raster_direct; what is read is cleared for the next pass over this buffer
             unsigned long long key[3];
 #pragma unroll
-            for (int u = 0; u < 3; ++u) key[u] = (inimg && l0 + u < sc.k) ? keys[pix0 + (size_t)(l0 + u) * plane] : 0ull;
+            for (int u = 0; u < 3; ++u)
+                key[u] = (inimg && l0 + u < sc.k && ((lmask >> (l0 + u)) & 1u)) ? keys[pix0 + (size_t)(l0 + u) * plane] : 0ull;
 #pragma unroll
             for (int u = 0; u < 3; ++u) {
                 id[u] = key[u] ? 0xFFFFFFFFu - (uint32_t)key[u] : VS_MISS;
@@ -317,7 +336,7 @@ static cudaError_t launch_sh2(const VsSceneDev& sc, const VsFrame& fr, const VsC
     if (e != cudaSuccess) return e;
     dim3 grid(fr.tiles_x * fr.tiles_y, ch.views);
     if (ch.keys)
-        kern<<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, nullptr, nullptr, ch.keys, ch.ids_is_output ? ch.ids : nullptr,
+        kern<<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_count, nullptr, ch.keys, ch.ids_is_output ? ch.ids : nullptr,
                                       ch.out_rgba, ch.texel_bits, ch.counters);
     else
         kern<<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_off, ch.ids, nullptr, nullptr, ch.out_rgba, ch.texel_bits,
