@@ -304,7 +304,7 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
         const size_t had = s->keys.cap;
         CU(s->keys.reserve(id_words * 8 + 16));
         if (s->keys.cap != had) s->keys_dirty = true;
-        CU(s->tile_count.reserve((size_t)views * VS_MAX_LAYERS * 16));   // per-(view, layer) vertex bounding boxes
+        CU(s->tile_count.reserve(ntile * 4));   // per-tile layer masks
         CU(s->big_list.reserve((size_t)65536 * 8));
         CU(s->big_count.reserve(16));
     }
@@ -340,10 +340,6 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
     const bool timing = (p->flags & VS_FLAG_KERNEL_TIMING) != 0;
     vs_status r;
     CU(cudaMemcpyAsync(s->cams.p, cams, sizeof(VsCamDev) * views, cudaMemcpyHostToDevice, st));
-    if (!reference && !tiled) {
-        ch.rects = (int*)s->tile_count.p;
-        CU(cudaMemsetAsync(ch.rects, 0x80, (size_t)views * s->dev.k * 16, st));  // every int = -2139062144
-    }
     if ((r = span_begin(s, timing, 0, st)) != VS_OK) return r;
     CU(vs_launch_transform(s->dev, fr, ch, st));
     if ((r = span_end(s, timing, st)) != VS_OK) return r;
@@ -372,6 +368,8 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
         if (s->keys_dirty) CU(cudaMemsetAsync(s->keys.p, 0, s->keys.cap, st));
         s->keys_dirty = true;
         CU(cudaMemsetAsync(ch.big_count, 0, 4, st));
+        ch.tile_mask = ch.tile_count;
+        CU(cudaMemsetAsync(ch.tile_mask, 0, ntile * 4, st));
         if ((r = span_begin(s, timing, 2, st)) != VS_OK) return r;
         CU(vs_launch_raster_direct(s->dev, fr, ch, st));
         if ((r = span_end(s, timing, st)) != VS_OK) return r;

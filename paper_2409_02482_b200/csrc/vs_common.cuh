@@ -242,7 +242,7 @@ struct VsChunk {                 // one pass over `views` cameras
     uint2* big_list;             // DEVICE [big_capacity] {view, global triangle} with very large boxes
     uint32_t* big_count;         // DEVICE entries appended this chunk (may exceed big_capacity: the rest was done in place)
     uint32_t big_capacity;
-    int* rects;                  // DEVICE [views][k][4] = max of {-X, -Y, X, Y} over the layer's valid snapped vertices (bytes 0x80 on entry)
+    uint32_t* tile_mask;         // DEVICE [views][tiles] layers whose triangles' boxes touch the 16x16 tile (zero on entry)
 };
 
 cudaError_t vs_launch_transform(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);

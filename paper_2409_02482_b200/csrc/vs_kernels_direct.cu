@@ -16,6 +16,7 @@
 //     box; triangles whose box exceeds VS_BIG_SAMPLES samples are appended to a list that k_raster_big
 //     spreads over the whole grid.
 // The key image must be zero on entry; k_shade reads it (id = ~low word) and clears what it read.
+// tile_mask[view][tile] (zero on entry) receives the layers whose triangles' boxes touch the tile.
 #include "vs_common.cuh"
 
 #define VS_RD_FIELDS 12
@@ -68,7 +69,7 @@ __device__ __forceinline__ void vs_direct_large(int X0, int Y0, int X1, int Y1, 
 #endif
 __global__ void __launch_bounds__(256, VS_RD_MIN_CTAS)
 k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, unsigned long long* __restrict__ keys,
-                uint2* __restrict__ big_list, uint32_t* __restrict__ big_count, uint32_t big_capacity,
+                uint32_t* __restrict__ tile_mask, uint2* __restrict__ big_list, uint32_t* __restrict__ big_count, uint32_t big_capacity,
                 unsigned long long* __restrict__ counters)
 {
     __shared__ int slab[8 * VS_RD_WARP_WORDS];
@@ -101,6 +102,25 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
             valid = i0 <= i1 && j0 <= j1;
             large = valid && !(narrow && i1 - i0 < 8 && j1 - j0 < 8);
         }
+    }
+    {
+        // layer bit of every 16x16 tile the box touches: k_shade skips the tiles and layers nothing was drawn into.
+        // A warp's 32 consecutive triangles share a handful of tiles: the lanes that report the same (tile, layer)
+        // elect one of them (match.any), so the L2 sees a few atomics per warp instead of one per triangle.
+        uint32_t* __restrict__ tm = tile_mask + (size_t)view * fr.tiles_x * fr.tiles_y;
+        const int tx0 = i0 / VS_TILE_W, tx1 = i1 / VS_TILE_W, ty0 = j0 / VS_TILE_H, ty1 = j1 / VS_TILE_H;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {  // the four corner tiles; a box of at most 8x8 samples touches no other
+            const int tx = (c & 1) ? tx1 : tx0, ty = (c & 2) ? ty1 : ty0;
+            const bool fresh = valid && !((c & 1) && tx1 == tx0) && !((c & 2) && ty1 == ty0);
+            const uint32_t tile = (uint32_t)ty * fr.tiles_x + (uint32_t)tx;
+            const uint32_t key = fresh ? tile * 16u + layer : 0xFFFFFFFFu;
+            const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key);
+            if (fresh && (uint32_t)(__ffs(peers) - 1) == lane) atomicOr(&tm[tile], 1u << layer);
+        }
+        if (large && (tx1 - tx0 > 1 || ty1 - ty0 > 1))  // the tiles between the corners
+            for (int ty = ty0; ty <= ty1; ++ty)
+                for (int tx = tx0; tx <= tx1; ++tx) atomicOr(&tm[(size_t)ty * fr.tiles_x + tx], 1u << layer);
     }
     {
         const unsigned dropped = __popc(__ballot_sync(0xFFFFFFFFu, status == 1));
@@ -273,7 +293,7 @@ cudaError_t vs_launch_raster_direct(const VsSceneDev& sc, const VsFrame& fr, con
     // key offsets inside one view are carried as uint32
     if ((unsigned long long)sc.k * fr.width * fr.height >= (1ull << 32)) return cudaErrorInvalidValue;
     dim3 grid((sc.t_total + 255) / 256, ch.views);
-    k_raster_direct<<<grid, 256, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.big_list, ch.big_count, ch.big_capacity, ch.counters);
+    k_raster_direct<<<grid, 256, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.tile_mask, ch.big_list, ch.big_count, ch.big_capacity, ch.counters);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     k_raster_big<<<148 * 4, 256, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.big_list, ch.big_count, ch.big_capacity);

@@ -1,6 +1,5 @@
 // vs_kernels_geom.cu -- S0 scene packing, S1 vertex transform, S2 triangle setup + S3 tile binning
 // (count / warp-scan prefix sum / scatter).  DESIGN.md §1, §3.1-3.2, §7.
-#include <climits>
 #include "vs_common.cuh"
 
 // ------------------------------------------------------------------------------------------------
@@ -67,72 +66,36 @@ cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, 
 // ------------------------------------------------------------------------------------------------
 // S1: vertex transform (fp32-exact).  One thread per (view, vertex).
 // ------------------------------------------------------------------------------------------------
-// With `rects` it also accumulates, per (view, layer), the bounding box of the snapped valid vertices: every
-// triangle lies inside the box of its layer, so k_shade can skip the tiles and layers outside it.
 __global__ void __launch_bounds__(256) k_transform(VsSceneDev sc, VsFrame fr, const VsCamDev* __restrict__ cams,
-                                                   int4* __restrict__ vtx, int* __restrict__ rects)
+                                                   int4* __restrict__ vtx)
 {
     const uint32_t v = blockIdx.x * blockDim.x + threadIdx.x;
+    if (v >= sc.v_total) return;
     const uint32_t view = blockIdx.y;
-    int e[4] = {INT_MIN, INT_MIN, INT_MIN, INT_MIN};  // max of {-X, -Y, X, Y}
-    if (v < sc.v_total) {
-        const VsCamDev c = cams[view];
-        float px = sc.positions[3 * (size_t)v], py = sc.positions[3 * (size_t)v + 1], pz = sc.positions[3 * (size_t)v + 2];
-        float xc = __fmaf_rn(c.R[0], px, __fmaf_rn(c.R[1], py, __fmaf_rn(c.R[2], pz, c.t[0])));
-        float yc = __fmaf_rn(c.R[3], px, __fmaf_rn(c.R[4], py, __fmaf_rn(c.R[5], pz, c.t[1])));
-        float w = __fmaf_rn(c.R[6], px, __fmaf_rn(c.R[7], py, __fmaf_rn(c.R[8], pz, c.t[2])));
-        int bad = 0;
-        if (!(w >= fr.near_plane)) bad = 1;
-        float q = __fdiv_rn(1.0f, w);
-        float xs = __fmaf_rn(c.fx, __fmul_rn(xc, q), c.cx);
-        float ys = __fmaf_rn(c.fy, __fmul_rn(yc, q), c.cy);
-        if (!bad && !(fabsf(xs) < 16384.0f && fabsf(ys) < 16384.0f)) bad = 2;
-        int X = 0, Y = 0;
-        if (!bad) {
-            X = __float2int_rn(__fmul_rn(xs, 256.0f));  // round-half-even
-            Y = __float2int_rn(__fmul_rn(ys, 256.0f));
-            e[0] = -X; e[1] = -Y; e[2] = X; e[3] = Y;
-        }
-        vtx[(size_t)view * sc.v_total + v] = make_int4(X, Y, __float_as_int(q), bad);
+    const VsCamDev c = cams[view];
+    float px = sc.positions[3 * (size_t)v], py = sc.positions[3 * (size_t)v + 1], pz = sc.positions[3 * (size_t)v + 2];
+    float xc = __fmaf_rn(c.R[0], px, __fmaf_rn(c.R[1], py, __fmaf_rn(c.R[2], pz, c.t[0])));
+    float yc = __fmaf_rn(c.R[3], px, __fmaf_rn(c.R[4], py, __fmaf_rn(c.R[5], pz, c.t[1])));
+    float w = __fmaf_rn(c.R[6], px, __fmaf_rn(c.R[7], py, __fmaf_rn(c.R[8], pz, c.t[2])));
+    int bad = 0;
+    if (!(w >= fr.near_plane)) bad = 1;
+    float q = __fdiv_rn(1.0f, w);
+    float xs = __fmaf_rn(c.fx, __fmul_rn(xc, q), c.cx);
+    float ys = __fmaf_rn(c.fy, __fmul_rn(yc, q), c.cy);
+    if (!bad && !(fabsf(xs) < 16384.0f && fabsf(ys) < 16384.0f)) bad = 2;
+    int X = 0, Y = 0;
+    if (!bad) {
+        X = __float2int_rn(__fmul_rn(xs, 256.0f));  // round-half-even
+        Y = __float2int_rn(__fmul_rn(ys, 256.0f));
     }
-    if (!rects) return;
-    // every thread of the CTA is still here.  A CTA whose vertices all belong to one layer (all but k-1 of them)
-    // reduces its box in shared memory and touches the four global values once.
-    __shared__ int sbox[4];
-    const uint32_t vfirst = blockIdx.x * blockDim.x, vlast = min(vfirst + blockDim.x, sc.v_total) - 1u;
-    uint32_t lfirst = 0, llast = 0, layer = 0;
-    const uint32_t vc = min(v, sc.v_total - 1u);
-    for (uint32_t l = 1; l < sc.k; ++l) {
-        lfirst += vfirst >= sc.vtx_off[l] ? 1u : 0u;
-        llast += vlast >= sc.vtx_off[l] ? 1u : 0u;
-        layer += vc >= sc.vtx_off[l] ? 1u : 0u;
-    }
-    if (lfirst == llast) {
-        if (threadIdx.x < 4) sbox[threadIdx.x] = INT_MIN;
-        __syncthreads();
-#pragma unroll
-        for (int i = 0; i < 4; ++i) e[i] = __reduce_max_sync(0xFFFFFFFFu, e[i]);
-        if ((threadIdx.x & 31) == 0)
-#pragma unroll
-            for (int i = 0; i < 4; ++i) atomicMax(&sbox[i], e[i]);
-        __syncthreads();
-        if (threadIdx.x < 4) {
-            int* r = rects + ((size_t)view * sc.k + lfirst) * 4 + threadIdx.x;
-            if (sbox[threadIdx.x] > __ldcg(r)) atomicMax(r, sbox[threadIdx.x]);
-        }
-    } else {
-        int* r = rects + ((size_t)view * sc.k + layer) * 4;
-#pragma unroll
-        for (int i = 0; i < 4; ++i)
-            if (e[i] > __ldcg(&r[i])) atomicMax(&r[i], e[i]);
-    }
+    vtx[(size_t)view * sc.v_total + v] = make_int4(X, Y, __float_as_int(q), bad);
 }
 
 cudaError_t vs_launch_transform(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
 {
     if (sc.v_total == 0) return cudaSuccess;
     dim3 grid((sc.v_total + 255) / 256, ch.views);
-    k_transform<<<grid, 256, 0, st>>>(sc, fr, ch.cams, ch.vtx, ch.rects);
+    k_transform<<<grid, 256, 0, st>>>(sc, fr, ch.cams, ch.vtx);
     return cudaGetLastError();
 }
 

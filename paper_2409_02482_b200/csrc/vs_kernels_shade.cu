@@ -16,7 +16,6 @@
 //   (fma.rn.f32x2 -> FFMA2); the one or two lanes of a channel are summed with one shuffle and the
 //   four channel logits go back to the owner through shared memory.  Owners apply the sigmoid and
 //   composite front to back in registers.
-#include <climits>
 #include "vs_common.cuh"
 
 struct __align__(16) VsFragRec {
@@ -96,7 +95,10 @@ struct VsShadeShape {
 };
 
 template <int F16, int DEG, bool COUNT>
-__global__ void __launch_bounds__(256, 3)
+#ifndef VS_SHADE_MIN_CTAS
+#define VS_SHADE_MIN_CTAS 3
+#endif
+__global__ void __launch_bounds__(256, VS_SHADE_MIN_CTAS)
 k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams, const int4* __restrict__ vtx,
         const uint32_t* __restrict__ tile_off, const uint32_t* __restrict__ ids, unsigned long long* __restrict__ keys,
         uint32_t* __restrict__ out_ids, float* __restrict__ out_rgba,
@@ -121,21 +123,8 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     const bool inimg = px < W && py < H;
     const size_t pix = ((size_t)view * H + py) * W + px;
 
-    // tiled path: tile_off = reference list offsets; direct path: tile_off = per-(view, layer) bounding boxes of the
-    // snapped vertices (k_transform), turned into the mask of layers that can have fragments in this tile
-    uint32_t lmask = 0xFFFFFFFFu;
-    if (keys) {
-        const int tx0 = (int)(tile % fr.tiles_x) * VS_TILE_W, ty0 = (int)(tile / fr.tiles_x) * VS_TILE_H;
-        const int* rc = reinterpret_cast<const int*>(tile_off) + (size_t)view * sc.k * 4;
-        lmask = 0u;
-        for (uint32_t l = 0; l < sc.k; ++l) {
-            const int4 e = *reinterpret_cast<const int4*>(rc + 4 * l);  // max of {-X, -Y, X, Y}
-            if (e.z < -(1 << 24)) continue;                              // still the fill value: no valid vertex
-            // pixel columns / rows whose samples lie inside the box (same rounding as the triangle boxes)
-            const int i0 = (-e.x + 127) >> 8, i1 = (e.z - 128) >> 8, j0 = (-e.y + 127) >> 8, j1 = (e.w - 128) >> 8;
-            if (i0 <= tx0 + VS_TILE_W - 1 && i1 >= tx0 && j0 <= ty0 + VS_TILE_H - 1 && j1 >= ty0) lmask |= 1u << l;
-        }
-    }
+    // tiled path: tile_off = reference list offsets; direct path: tile_off = per-tile masks of the layers drawn into
+    const uint32_t lmask = keys ? tile_off[view * tiles + tile] : 0xFFFFFFFFu;
     if (keys ? lmask == 0u : tile_off[view * tiles + tile] == tile_off[view * tiles + tile + 1]) {  // nothing drawn here: background
         if (out_ids && inimg)
             for (uint32_t l = 0; l < sc.k; ++l) out_ids[((size_t)view * sc.k + l) * ((size_t)W * H) + (size_t)py * W + px] = VS_MISS;
@@ -334,9 +323,13 @@ static cudaError_t launch_sh2(const VsSceneDev& sc, const VsFrame& fr, const VsC
     auto kern = k_shade<F16, DEG, COUNT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
+#ifdef VS_SHADE_CARVEOUT
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, VS_SHADE_CARVEOUT);
+    if (e != cudaSuccess) return e;
+#endif
     dim3 grid(fr.tiles_x * fr.tiles_y, ch.views);
     if (ch.keys)
-        kern<<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_count, nullptr, ch.keys, ch.ids_is_output ? ch.ids : nullptr,
+        kern<<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_mask, nullptr, ch.keys, ch.ids_is_output ? ch.ids : nullptr,
                                       ch.out_rgba, ch.texel_bits, ch.counters);
     else
         kern<<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_off, ch.ids, nullptr, nullptr, ch.out_rgba, ch.texel_bits,
