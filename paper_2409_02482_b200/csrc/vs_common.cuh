@@ -201,10 +201,10 @@ __device__ __forceinline__ void vs_texel_coord(float u0, float du, float fW, int
     c1 = (uint32_t)min(max(i0 + 1, 0), Wt - 1);
 }
 
-__device__ __forceinline__ void vs_fragment_setup(const VsSceneDev& sc, const int4* __restrict__ vv, uint32_t l,
-                                                  uint32_t local_tri, int px, int py, VsFrag& f)
+// `tri` = index record of the winning triangle of layer l
+__device__ __forceinline__ void vs_fragment_setup_tri(const VsSceneDev& sc, const int4* __restrict__ vv, uint32_t l,
+                                                      const uint4 tri, int px, int py, VsFrag& f)
 {
-    const uint4 tri = __ldg(&sc.tris[sc.tri_off[l] + local_tri]);
     const int4 a = __ldg(&vv[tri.x]), b = __ldg(&vv[tri.y]), c = __ldg(&vv[tri.z]);
     const float2 uva = __ldg(&sc.uvs[tri.x]), uvb = __ldg(&sc.uvs[tri.y]), uvc = __ldg(&sc.uvs[tri.z]);
     VsTri T;
@@ -219,6 +219,12 @@ __device__ __forceinline__ void vs_fragment_setup(const VsSceneDev& sc, const in
     const int Wt = (int)sc.tex_w[l], Ht = (int)sc.tex_h[l];
     vs_texel_coord(uv0.x, b1 * (uv1.x - uv0.x) + b2 * (uv2.x - uv0.x), (float)Wt, Wt, f.cx0, f.cx1, f.a);
     vs_texel_coord(uv0.y, b1 * (uv1.y - uv0.y) + b2 * (uv2.y - uv0.y), (float)Ht, Ht, f.cy0, f.cy1, f.b);
+}
+
+__device__ __forceinline__ void vs_fragment_setup(const VsSceneDev& sc, const int4* __restrict__ vv, uint32_t l,
+                                                  uint32_t local_tri, int px, int py, VsFrag& f)
+{
+    vs_fragment_setup_tri(sc, vv, l, __ldg(&sc.tris[sc.tri_off[l] + local_tri]), px, py, f);
 }
 
 // ---- host-side launchers (vs_kernels_*.cu) ------------------------------------------------------

@@ -138,38 +138,45 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     const size_t pix0 = (size_t)view * sc.k * plane + (size_t)py * W + px;
     const uint32_t* idp = ids + pix0;
     bool any_hit = false;
-    for (uint32_t l0 = 0; l0 < sc.k; l0 += 3) {
-        uint32_t id[3];
+    {
+        // The gather chain key/id -> index record -> 3 vertices + 3 uvs is walked level by level: all layers' keys
+        // first, then all index records, then the vertices three layers at a time (5 dependent round trips per
+        // tile instead of 3 per group of three layers).
+        uint32_t id[VS_MAX_LAYERS];
         if (keys) {
             // direct path: the key image of k_raster_direct; what is read is cleared for the next pass over this buffer
-            unsigned long long key[3];
+            unsigned long long key[VS_MAX_LAYERS];
 #pragma unroll
-            for (int u = 0; u < 3; ++u)
-                key[u] = (inimg && l0 + u < sc.k && ((lmask >> (l0 + u)) & 1u)) ? keys[pix0 + (size_t)(l0 + u) * plane] : 0ull;
+            for (int u = 0; u < VS_MAX_LAYERS; ++u)
+                key[u] = (inimg && u < (int)sc.k && ((lmask >> u) & 1u)) ? keys[pix0 + (size_t)u * plane] : 0ull;
 #pragma unroll
-            for (int u = 0; u < 3; ++u) {
+            for (int u = 0; u < VS_MAX_LAYERS; ++u) {
                 id[u] = key[u] ? 0xFFFFFFFFu - (uint32_t)key[u] : VS_MISS;
-                if (key[u]) keys[pix0 + (size_t)(l0 + u) * plane] = 0ull;
-                if (out_ids && inimg && l0 + u < sc.k) out_ids[pix0 + (size_t)(l0 + u) * plane] = id[u];
+                if (key[u]) keys[pix0 + (size_t)u * plane] = 0ull;
+                if (out_ids && inimg && u < (int)sc.k) out_ids[pix0 + (size_t)u * plane] = id[u];
             }
         } else {
 #pragma unroll
-            for (int u = 0; u < 3; ++u) id[u] = (inimg && l0 + u < sc.k) ? __ldg(idp + (size_t)(l0 + u) * plane) : VS_MISS;
+            for (int u = 0; u < VS_MAX_LAYERS; ++u) id[u] = (inimg && u < (int)sc.k) ? __ldg(idp + (size_t)u * plane) : VS_MISS;
         }
+        uint4 tri[VS_MAX_LAYERS];
 #pragma unroll
-        for (int u = 0; u < 3; ++u) {
-            if (l0 + u < sc.k) {
+        for (int u = 0; u < VS_MAX_LAYERS; ++u)
+            tri[u] = id[u] != VS_MISS ? __ldg(&sc.tris[sc.tri_off[u] + id[u]]) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+        for (int u = 0; u < VS_MAX_LAYERS; ++u) {
+            if (u < (int)sc.k) {
                 uint32_t xy = 0;
                 float2 ab = make_float2(-1.0f, 0.0f);
                 if (id[u] != VS_MISS) {
                     VsFrag f;
-                    vs_fragment_setup(sc, vv, l0 + u, id[u], px, py, f);
+                    vs_fragment_setup_tri(sc, vv, u, tri[u], px, py, f);
                     xy = vs_pack_frag(f);
                     ab = make_float2(f.a, f.b);
                     any_hit = true;
                 }
-                rec_xy[(l0 + u) * VS_TILE_PIX + tid] = xy;
-                rec_ab[(l0 + u) * VS_TILE_PIX + tid] = ab;
+                rec_xy[u * VS_TILE_PIX + tid] = xy;
+                rec_ab[u * VS_TILE_PIX + tid] = ab;
             }
         }
     }
