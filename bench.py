@@ -31,9 +31,10 @@ from paper_2409_02482_b200 import synth  # noqa: E402
 
 METRIC = "megapixels_per_sec_rendering_k_layers"
 UNIT = "MP/s"
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel from the committed
-# `ncu --set full` capture (profiles/), keyed by config; None until a capture exists.
-NCU_TRAFFIC_BYTES_PER_LAUNCH = {}
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel (k_shade, direct path) from the committed
+# `ncu --set full` capture (profiles/), divided by the views of the captured launch, keyed by config; reported
+# per launch of the timed run.  None until a capture exists.
+NCU_TRAFFIC_BYTES_PER_VIEW = {}
 
 
 def load_peaks():
@@ -155,13 +156,14 @@ def run_ours(args):
     sc = build_scene(args.config, rank, world, args)
     B, W, H = len(sc.cameras), sc.width, sc.height
     renderer = binding.Renderer(sc, dev)
-    flags = binding.VS_FLAG_KERNEL_TIMING
+    path_flag = binding.VS_FLAG_TILED_PATH if args.tiled else 0
+    flags = binding.VS_FLAG_KERNEL_TIMING | path_flag
     params = binding.make_params(W, H, sc.near_plane, sc.t_min, sc.background, flags, args.chunk)
     out = torch.empty((B, H, W, 4), dtype=torch.float32, device=dev)
     stream = torch.cuda.current_stream()
 
     # untimed: count the algorithmic texture bytes (unique texels per view) of this batch
-    cparams = binding.make_params(W, H, sc.near_plane, sc.t_min, sc.background, binding.VS_FLAG_COUNT_TEXELS, args.chunk)
+    cparams = binding.make_params(W, H, sc.near_plane, sc.t_min, sc.background, binding.VS_FLAG_COUNT_TEXELS | path_flag, args.chunk)
     binding.vs_render(renderer.handle, sc.cameras, cparams, out)
     cstats = renderer.stats()
     texel_bytes = 16 * ((sc.n_coef * 4 * sc.layers[0].texture.dtype.itemsize + 15) // 16)
@@ -199,7 +201,7 @@ def run_ours(args):
     # end to end through the C-ABI with HOST buffers: camera upload + image download every step
     e2e_steps = max(1, min(args.steps, 5))
     host_out = torch.empty((B, H, W, 4), dtype=torch.float32).pin_memory()
-    eparams = binding.make_params(W, H, sc.near_plane, sc.t_min, sc.background, 0, args.chunk)
+    eparams = binding.make_params(W, H, sc.near_plane, sc.t_min, sc.background, path_flag, args.chunk)
     binding.vs_render_host(renderer.handle, sc.cameras, eparams, host_out)
     vsdist.barrier()
     torch.cuda.synchronize()
@@ -223,7 +225,8 @@ def run_ours(args):
     achieved = bytes_per_launch / (per_launch_ms * 1e-3) / 1e9 if per_launch_ms > 0 else 0.0
     step_achieved = alg_bytes_step * world / (secs_max / args.steps) / 1e9
     roofline = {"bound": "hbm", "kernel": "k_shade", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": NCU_TRAFFIC_BYTES_PER_LAUNCH.get(args.config),
+                "frac": achieved / peak, "traffic": (NCU_TRAFFIC_BYTES_PER_VIEW[args.config] * B * args.steps / max(shade_launches, 1)
+                            if args.config in NCU_TRAFFIC_BYTES_PER_VIEW and not args.tiled else None),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_per_launch,
                 "launch_ms": per_launch_ms, "views_per_launch": B * args.steps / max(shade_launches, 1),
                 "kernel_share_of_step": shade_ms / (secs * 1e3),
@@ -249,6 +252,8 @@ def run_ours(args):
             "config": {"workload": sc.name, "k": sc.k, "triangles_per_layer": int(sc.layers[0].indices.shape[0]),
                        "width": W, "height": H, "views_per_step": B, "sh_degree": sc.sh_degree,
                        "texture": "%s %dx%d" % (sc.layers[0].texture.dtype, sc.layers[0].texture.shape[1], sc.layers[0].texture.shape[0]),
+                       "raster_path": "tiled (binning + per-tile shared-memory keys)" if args.tiled
+                       else "direct (triangle-parallel, 64-bit max keys in HBM/L2)",
                        "parallelism": "views sharded, scene replicated (dp%d)" % world,
                        "l2": "no flush: %.1f GiB of textures streamed per step >> 126 MB L2" % (
                            sum(ly.texture.nbytes for ly in sc.layers) / 2 ** 30),
@@ -274,6 +279,7 @@ def main():
     ap.add_argument("--chunk", type=int, default=0, help="views per internal pass (0 = automatic)")
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="oracle work of the cpu_baseline sample (whole views)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--tiled", action="store_true", help="time the per-tile raster path (VS_FLAG_TILED_PATH) instead of the default direct one")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -6,7 +6,7 @@ For each configuration the whole batch is rendered once; a sample of views (chos
 first, the last and -- for C5 -- a far and a close-up camera) is compared against the CPU oracle pixel
 by pixel: triangle ids BIT-EXACT, RGBA max abs error <= 1e-4.  Every view is additionally checked
 through properties that hold at any size (the AOV-less timed call and the AOV call give the same
-image bit for bit; alpha in [0,1]; pixels no layer hits are exactly the background; ids in range;
+image bit for bit; the default direct raster path and the per-tile path give the same ids and image; alpha in [0,1]; pixels no layer hits are exactly the background; ids in range;
 no dropped triangles)."""
 import types
 
@@ -34,6 +34,7 @@ def _check_config(env, cfg, sample_views, id_views):
     B, W, H, k = len(sc.cameras), sc.width, sc.height, sc.k
     r = b.Renderer(sc)
     p = b.make_params(W, H, sc.near_plane, sc.t_min, sc.background)
+    p_tiled = b.make_params(W, H, sc.near_plane, sc.t_min, sc.background, b.VS_FLAG_TILED_PATH)
     # (1) the timed launch configuration: whole batch, no AOV
     out = torch.empty((B, H, W, 4), dtype=torch.float32, device="cuda")
     b.vs_render(r.handle, sc.cameras, p, out)
@@ -52,6 +53,12 @@ def _check_config(env, cfg, sample_views, id_views):
         rgba = rgba.cpu().numpy()[0]
         ids = ids.cpu().numpy().view(np.uint32)[0]
         assert np.array_equal(rgba, rgba_all[v]), "AOV call and timed call differ in view %d" % v
+        # the per-tile raster path (binning + shared-memory keys) must give the same ids and image bit for bit
+        rgba_t, ids_t = r.render(sc.cameras[[v]], p_tiled, want_ids=True)
+        torch.cuda.synchronize()
+        assert np.array_equal(ids_t.cpu().numpy().view(np.uint32)[0], ids), "tiled and direct ids differ in view %d" % v
+        assert np.array_equal(rgba_t.cpu().numpy()[0], rgba), "tiled and direct images differ in view %d" % v
+        del rgba_t, ids_t
         ntri = np.array([ly.indices.shape[0] for ly in sc.layers], np.uint32)[:, None, None]
         hit = ids != b.MISS
         assert np.all(ids[hit] < np.broadcast_to(ntri, ids.shape)[hit])
