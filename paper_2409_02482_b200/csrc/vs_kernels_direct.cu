@@ -36,7 +36,9 @@ __device__ __forceinline__ float vs_depth_div(float f0, float f1, float f2, floa
 }
 
 // Whole warp, lane = pixel of an 8x4 chunk of the box [i0,i1] x [j0,j1]; chunks c = first, first+stride, ...
-template <typename I>
+// LINEAR: lane = sample 32 c + lane of the box in row-major order instead (boxes of a few hundred samples, where
+// 8x4 chunks would leave most lanes outside the box).
+template <typename I, bool LINEAR>
 __device__ __forceinline__ void vs_direct_large(int X0, int Y0, int X1, int Y1, int X2, int Y2, float q0, float q1, float q2,
                                                 float fA, int i0, int i1, int j0, int j1, int W,
                                                 unsigned long long* __restrict__ plane, uint32_t lid, uint32_t lane,
@@ -46,9 +48,20 @@ __device__ __forceinline__ void vs_direct_large(int X0, int Y0, int X1, int Y1, 
     const int m0 = ((dy0 < 0) || (dy0 == 0 && dx0 > 0)) ? 0 : 1;
     const int m1 = ((dy1 < 0) || (dy1 == 0 && dx1 > 0)) ? 0 : 1;
     const int m2 = ((dy2 < 0) || (dy2 == 0 && dx2 > 0)) ? 0 : 1;
-    const uint32_t ncx = (uint32_t)(i1 - i0 + 8) >> 3, ncy = (uint32_t)(j1 - j0 + 4) >> 2;
-    for (uint32_t c = first; c < ncx * ncy; c += stride) {
-        const int i = i0 + (int)(c % ncx) * 8 + (int)(lane & 7), j = j0 + (int)(c / ncx) * 4 + (int)(lane >> 3);
+    const uint32_t bw = (uint32_t)(i1 - i0 + 1), bh = (uint32_t)(j1 - j0 + 1);
+    const uint32_t ncx = (bw + 7) >> 3, ncy = (bh + 3) >> 2;
+    const uint32_t nchunks = LINEAR ? (bw * bh + 31) >> 5 : ncx * ncy;
+    const float inv_bw = 1.0f / (float)bw;
+    for (uint32_t c = first; c < nchunks; c += stride) {
+        int i, j;
+        if (LINEAR) {
+            // row = floor((s + 0.5) / bw): s + 0.5 is never within 0.5 / bw of a multiple of bw, so fp32 is exact here (s < 2^13)
+            const uint32_t sidx = 32u * c + lane;
+            const uint32_t row = (uint32_t)__float2int_rd(((float)sidx + 0.5f) * inv_bw);
+            i = i0 + (int)(sidx - row * bw); j = j0 + (int)row;
+        } else {
+            i = i0 + (int)(c % ncx) * 8 + (int)(lane & 7); j = j0 + (int)(c / ncx) * 4 + (int)(lane >> 3);
+        }
         if (i > i1 || j > j1) continue;
         const int Sx = 256 * i + 128, Sy = 256 * j + 128;
         const I e0 = (I)dx0 * (I)(Sy - Y1) - (I)dy0 * (I)(Sx - X1);
@@ -72,14 +85,14 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
                 uint32_t* __restrict__ tile_mask, uint2* __restrict__ big_list, uint32_t* __restrict__ big_count, uint32_t big_capacity,
                 unsigned long long* __restrict__ counters)
 {
-    __shared__ int slab[8 * VS_RD_WARP_WORDS];
+    __shared__ __align__(16) int slab[8 * VS_RD_WARP_WORDS];
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t view = blockIdx.y;
     const uint32_t gt = blockIdx.x * 256u + tid;
     const int W = (int)fr.width, H = (int)fr.height;
     const size_t plane_px = (size_t)W * H;
-    int* rec = slab + warp * VS_RD_WARP_WORDS;                                            // [field][lane]
-    unsigned short* queue = reinterpret_cast<unsigned short*>(rec + VS_RD_FIELDS * 32);   // [512]
+    int4* rec4 = reinterpret_cast<int4*>(slab + warp * VS_RD_WARP_WORDS);                 // [vector][lane]
+    unsigned short* queue = reinterpret_cast<unsigned short*>(slab + warp * VS_RD_WARP_WORDS + VS_RD_FIELDS * 32);   // [512]
     const int4* __restrict__ vv = vtx + (size_t)view * sc.v_total;
     unsigned long long* __restrict__ vkeys = keys + (size_t)view * sc.k * plane_px;
 
@@ -143,14 +156,10 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
         E2 = dx2 * (Sy - T.Y0) - dy2 * (Sx - T.X0);
         sx0 = -256 * dy0; sx1 = -256 * dy1; sx2 = -256 * dy2;  // one pixel in +x
         sy0 = 256 * dx0; sy1 = 256 * dx1; sy2 = 256 * dx2;     // one pixel in +y
-        rec[0 * 32 + lane] = E0; rec[1 * 32 + lane] = E1;
-        rec[2 * 32 + lane] = sx0; rec[3 * 32 + lane] = sx1;
-        rec[4 * 32 + lane] = sy0; rec[5 * 32 + lane] = sy1;
-        rec[6 * 32 + lane] = (int)T.A2;
-        rec[7 * 32 + lane] = __float_as_int(T.q0); rec[8 * 32 + lane] = __float_as_int(T.q1);
-        rec[9 * 32 + lane] = __float_as_int(T.q2);
-        rec[10 * 32 + lane] = (int)lid;
-        rec[11 * 32 + lane] = (int)((uint32_t)(layer * plane_px) + (uint32_t)(j0 * W + i0));  // < 2^32: checked by the launcher
+        // three 16-byte vectors per triangle: {E0, E1, sx0, sx1} {sy0, sy1, A2, key offset} {q0, q1, q2, id}
+        rec4[0 * 32 + lane] = make_int4(E0, E1, sx0, sx1);
+        rec4[1 * 32 + lane] = make_int4(sy0, sy1, (int)T.A2, (int)((uint32_t)(layer * plane_px) + (uint32_t)(j0 * W + i0)));  // < 2^32: checked by the launcher
+        rec4[2 * 32 + lane] = make_int4(__float_as_int(T.q0), __float_as_int(T.q1), __float_as_int(T.q2), (int)lid);
         // covered <=> E_e > 0 || (E_e == 0 && topleft_e) <=> F_e := E_e - (topleft_e ? 0 : 1) >= 0
         E0 -= ((dy0 < 0) || (dy0 == 0 && dx0 > 0)) ? 0 : 1;
         E1 -= ((dy1 < 0) || (dy1 == 0 && dx1 > 0)) ? 0 : 1;
@@ -218,14 +227,14 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
             const uint32_t code = queue[s];
             const uint32_t src = code >> 6;
             const int r = (int)((code >> 3) & 7u), c = (int)(code & 7u);
-            const int e0 = rec[0 * 32 + src] + r * rec[4 * 32 + src] + c * rec[2 * 32 + src];
-            const int e1 = rec[1 * 32 + src] + r * rec[5 * 32 + src] + c * rec[3 * 32 + src];
-            const int A2 = rec[6 * 32 + src];
+            const int4 ra = rec4[0 * 32 + src], rb = rec4[1 * 32 + src], rc = rec4[2 * 32 + src];
+            const int e0 = ra.x + r * rb.x + c * ra.z;
+            const int e1 = ra.y + r * rb.y + c * ra.w;
+            const int A2 = rb.z;
             const int e2 = A2 - e0 - e1;  // E0 + E1 + E2 == A2 at every point
             const float qp = vs_depth_div(__int2float_rn(e0), __int2float_rn(e1), __int2float_rn(e2),
-                                          __int_as_float(rec[7 * 32 + src]), __int_as_float(rec[8 * 32 + src]),
-                                          __int_as_float(rec[9 * 32 + src]), __int2float_rn(A2));
-            vs_key_red(&vkeys[(uint32_t)rec[11 * 32 + src] + (uint32_t)(r * W + c)], vs_make_key(qp, (uint32_t)rec[10 * 32 + src]));
+                                          __int_as_float(rc.x), __int_as_float(rc.y), __int_as_float(rc.z), __int2float_rn(A2));
+            vs_key_red(&vkeys[(uint32_t)rb.w + (uint32_t)(r * W + c)], vs_make_key(qp, (uint32_t)rc.w));
         }
         __syncwarp();
     }
@@ -253,8 +262,12 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
         const uint32_t blid = __shfl_sync(0xFFFFFFFFu, lid, src), blayer = __shfl_sync(0xFFFFFFFFu, layer, src);
         const bool bnarrow = __shfl_sync(0xFFFFFFFFu, (int)narrow, src) != 0;
         unsigned long long* plane = vkeys + blayer * plane_px;
-        if (bnarrow) vs_direct_large<int>(X0, Y0, X1, Y1, X2, Y2, q0, q1, q2, __ll2float_rn(A2), bi0, bi1, bj0, bj1, W, plane, blid, lane, 0u, 1u);
-        else vs_direct_large<long long>(X0, Y0, X1, Y1, X2, Y2, q0, q1, q2, __ll2float_rn(A2), bi0, bi1, bj0, bj1, W, plane, blid, lane, 0u, 1u);
+        const float fA = __ll2float_rn(A2);
+        // (only a box that did not fit the big list can be larger than VS_BIG_SAMPLES here)
+        const bool lin = (unsigned long long)(bi1 - bi0 + 1) * (unsigned long long)(bj1 - bj0 + 1) <= VS_BIG_SAMPLES;
+        if (bnarrow) vs_direct_large<int, true>(X0, Y0, X1, Y1, X2, Y2, q0, q1, q2, fA, bi0, bi1, bj0, bj1, W, plane, blid, lane, 0u, 1u);
+        else if (lin) vs_direct_large<long long, true>(X0, Y0, X1, Y1, X2, Y2, q0, q1, q2, fA, bi0, bi1, bj0, bj1, W, plane, blid, lane, 0u, 1u);
+        else vs_direct_large<long long, false>(X0, Y0, X1, Y1, X2, Y2, q0, q1, q2, fA, bi0, bi1, bj0, bj1, W, plane, blid, lane, 0u, 1u);
     }
 }
 
@@ -282,8 +295,8 @@ k_raster_big(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx
         const bool narrow = maxX - minX < 8192 && maxY - minY < 8192;
         unsigned long long* plane = keys + ((size_t)ent.x * sc.k + tri.w) * plane_px;
         const uint32_t lid = ent.y - sc.tri_off[tri.w];
-        if (narrow) vs_direct_large<int>(T.X0, T.Y0, T.X1, T.Y1, T.X2, T.Y2, T.q0, T.q1, T.q2, __ll2float_rn(T.A2), i0, i1, j0, j1, W, plane, lid, lane, gw, warps);
-        else vs_direct_large<long long>(T.X0, T.Y0, T.X1, T.Y1, T.X2, T.Y2, T.q0, T.q1, T.q2, __ll2float_rn(T.A2), i0, i1, j0, j1, W, plane, lid, lane, gw, warps);
+        if (narrow) vs_direct_large<int, false>(T.X0, T.Y0, T.X1, T.Y1, T.X2, T.Y2, T.q0, T.q1, T.q2, __ll2float_rn(T.A2), i0, i1, j0, j1, W, plane, lid, lane, gw, warps);
+        else vs_direct_large<long long, false>(T.X0, T.Y0, T.X1, T.Y1, T.X2, T.Y2, T.q0, T.q1, T.q2, __ll2float_rn(T.A2), i0, i1, j0, j1, W, plane, lid, lane, gw, warps);
     }
 }
 
