@@ -248,16 +248,19 @@ static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, u
     return VS_OK;
 }
 
-static uint32_t pick_chunk(const vs_scene* s, const vs_render_params* p, uint32_t n)
+// Views per internal pass.  Device outputs: as many as a ~3 GB scratch budget allows (fewer, larger launches:
+// C4 26.8 ms per 64 views at 16 against 27.7 ms at 4).  Host outputs: at most 4, so that the download of one
+// chunk overlaps the rendering of the next (C4 end to end: 3407 MP/s at 4 against 3025 MP/s at 16).
+static uint32_t pick_chunk(const vs_scene* s, const vs_render_params* p, uint32_t n, bool host_outputs)
 {
     if (p->views_per_chunk) return p->views_per_chunk < n ? p->views_per_chunk : n;
-    // keep the per-chunk scratch (transformed vertices, key image or packed tile ranges + id planes) near 1.5 GB
+    // keep the per-chunk scratch (transformed vertices, key image or packed tile ranges + id planes) under ~3 GB
     const bool tiled = (p->flags & VS_FLAG_TILED_PATH) != 0;
     const size_t per_view = (size_t)s->dev.v_total * 16 + (tiled ? (size_t)s->dev.t_total * 8 : 0) +
                             (size_t)p->width * p->height * (tiled ? 4 : 8) * s->dev.k;
-    size_t c = ((size_t)3 << 29) / (per_view ? per_view : 1);
+    size_t c = ((size_t)3 << 30) / (per_view ? per_view : 1);
     if (c < 1) c = 1;
-    if (c > 16) c = 16;
+    if (c > (host_outputs ? 4u : 16u)) c = host_outputs ? 4 : 16;
     return (uint32_t)(c < n ? c : n);
 }
 
@@ -453,7 +456,7 @@ extern "C" vs_status vs_render(vs_scene* scene, const vs_camera* cameras, uint32
     vs_status r = validate_render(scene, cameras, num_cameras, params, out_rgba);
     if (r != VS_OK) return r;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const uint32_t chunk = pick_chunk(scene, params, num_cameras);
+    const uint32_t chunk = pick_chunk(scene, params, num_cameras, false);
     const size_t px = (size_t)params->width * params->height;
     first_capacity_guess(scene, chunk);
     for (int attempt = 0; attempt < 4; ++attempt) {
@@ -480,7 +483,7 @@ extern "C" vs_status vs_render_host(vs_scene* scene, const vs_camera* cameras, u
     vs_status r = validate_render(scene, cameras, num_cameras, params, out_rgba);
     if (r != VS_OK) return r;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    const uint32_t chunk = pick_chunk(scene, params, num_cameras);
+    const uint32_t chunk = pick_chunk(scene, params, num_cameras, true);
     const size_t px = (size_t)params->width * params->height;
     const size_t rgba_bytes = px * 16, ids_bytes = px * 4 * scene->dev.k;
     first_capacity_guess(scene, chunk);
