@@ -33,8 +33,8 @@ METRIC = "megapixels_per_sec_rendering_k_layers"
 UNIT = "MP/s"
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel (k_shade, direct path) from the committed
 # `ncu --set full` capture (profiles/), divided by the views of the captured launch, keyed by config; reported
-# per launch of the timed run.  None until a capture exists.
-NCU_TRAFFIC_BYTES_PER_VIEW = {}
+# per launch of the timed run.  None for configs without a capture.
+NCU_TRAFFIC_BYTES_PER_VIEW = {4: (21.545490e9 + 1.304478e9) / 16}   # profiles/r1m_summary.md: one launch = 16 views
 
 
 def load_peaks():
