@@ -34,7 +34,10 @@ def lib():
         L.vso_render.argtypes = [C.POINTER(_Layer), C.c_uint32, C.c_uint32, C.c_int, C.c_void_p,
                                  C.c_uint32, C.c_uint32, C.c_float, C.c_double, C.c_void_p,
                                  C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
-                                 C.c_void_p, C.c_int]
+                                 C.c_void_p, C.c_int, C.c_int]
+        L.vso_alpha_attenuation.restype = C.c_double
+        L.vso_alpha_attenuation.argtypes = [C.c_void_p, C.c_void_p]
+        L.vso_face_normal.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.vso_half_to_double.restype = C.c_double
         L.vso_half_to_double.argtypes = [C.c_uint16]
         L.vso_sh_basis.argtypes = [C.c_int, C.c_void_p, C.c_void_p]
@@ -67,7 +70,8 @@ def max_threads() -> int:
 
 def render_view(layers, sh_degree: int, camera, width: int, height: int, *, near_plane: float = 0.05,
                 t_min: float = 2.0 ** -14, background=(0.0, 0.0, 0.0), num_threads: int = 0,
-                want_qp: bool = False, want_layer_rgba: bool = False, want_layer_uv: bool = False):
+                want_qp: bool = False, want_layer_rgba: bool = False, want_layer_uv: bool = False,
+                attenuation: bool = False):
     """Render one view.  `layers`: objects with positions/uvs/indices/texture numpy arrays
     (outermost first).  Returns dict(rgba [H,W,4] f64, ids [k,H,W] u32, stats [2] u64, ...)."""
     k = len(layers)
@@ -103,7 +107,7 @@ def render_view(layers, sh_degree: int, camera, width: int, height: int, *, near
     rc = lib().vso_render(arr, k, sh_degree, code, _ptr(cam), width, height, near_plane, t_min, _ptr(bg),
                           _ptr(rgba), _ptr(ids), _ptr(qp) if want_qp else None,
                           _ptr(lrgba) if want_layer_rgba else None, _ptr(luv) if want_layer_uv else None,
-                          _ptr(stats), num_threads)
+                          _ptr(stats), num_threads, 1 if attenuation else 0)
     if rc != 0:
         raise ValueError("vso_render rejected its arguments (rc=%d)" % rc)
     out = dict(rgba=rgba, ids=ids, stats=stats)
@@ -153,6 +157,19 @@ def decode_rgba(coef: np.ndarray, Y: np.ndarray) -> np.ndarray:
     out = np.empty(4, dtype=np.float64)
     lib().vso_decode_rgba(coef.shape[0], _ptr(coef), _ptr(Y), _ptr(out))
     return out
+
+
+def alpha_attenuation(v, n) -> float:
+    v = np.ascontiguousarray(v, dtype=np.float64)
+    n = np.ascontiguousarray(n, dtype=np.float64)
+    return float(lib().vso_alpha_attenuation(_ptr(v), _ptr(n)))
+
+
+def face_normal(p0, p1, p2) -> np.ndarray:
+    ps = [np.ascontiguousarray(p, dtype=np.float32) for p in (p0, p1, p2)]
+    n = np.empty(3, dtype=np.float64)
+    lib().vso_face_normal(_ptr(ps[0]), _ptr(ps[1]), _ptr(ps[2]), _ptr(n))
+    return n
 
 
 def blend(layer_rgba, hit=None, t_min: float = 0.0, background=(0.0, 0.0, 0.0)) -> np.ndarray:

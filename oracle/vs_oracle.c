@@ -238,6 +238,30 @@ void vso_blend(uint32_t k, const double* layer_rgba, const int32_t* hit, double 
     out[3] = 1.0 - T;
 }
 
+/* ---- Transparency attenuation (§4.2 "Transparency Attenuation":
+ *      "multiplying predicted transparencies with a weight alpha_w that depends on the angle between the
+ *      view direction and the surface normal", alpha_w = 2 Sigmoid(10 |v . n|) - 1  (= tanh(5 |v . n|));
+ *      SPEC.md:L462-470).  v, n: unit vectors; n = 0 (degenerate triangle) gives 0. ---- */
+double vso_alpha_attenuation(const double* v, const double* n)
+{
+    double d = fabs(v[0] * n[0] + v[1] * n[1] + v[2] * n[2]);
+    return 2.0 * (1.0 / (1.0 + exp(-10.0 * d))) - 1.0;
+}
+
+/* Surface normal of a fragment = unit geometric normal of its triangle in world space (the paper does not
+ * say where the baked renderer takes n from: reading Q13 in DESIGN.md).  Sign is irrelevant (|v . n|).
+ * Zero-area triangle -> n = 0. */
+void vso_face_normal(const float* p0, const float* p1, const float* p2, double* n)
+{
+    double a[3], b[3];
+    for (int c = 0; c < 3; ++c) { a[c] = (double)p1[c] - (double)p0[c]; b[c] = (double)p2[c] - (double)p0[c]; }
+    n[0] = a[1] * b[2] - a[2] * b[1];
+    n[1] = a[2] * b[0] - a[0] * b[2];
+    n[2] = a[0] * b[1] - a[1] * b[0];
+    double len = sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
+    for (int c = 0; c < 3; ++c) n[c] = len > 0.0 ? n[c] / len : 0.0;
+}
+
 /* view direction of pixel (i,j): camera -> scene, world frame, unit (reading Q4) */
 static void view_dir(const float* cam, int px, int py, double* v)
 {
@@ -259,12 +283,14 @@ static void view_dir(const float* cam, int px, int py, double* v)
  *   out_layer_rgba [k][H][W][4] double, decoded per-layer RGBA, 0 on miss            (optional)
  *   out_layer_uv   [k][H][W][2] double, interpolated UV, 0 on miss                   (optional)
  *   stats[0] += triangles dropped (near plane / guard band), stats[1] += zero-area triangles
+ *   attenuate != 0: every fragment's opacity is multiplied by alpha_w(v, face normal) before blending
+ *                   (PAPER.md:L279-286); the alpha of out_layer_rgba is the attenuated one
  * Returns 0, or -1 on bad arguments / allocation failure.
  */
 int vso_render(const vso_layer* layers, uint32_t k, uint32_t sh_degree, int tex_dtype, const float* cam,
                uint32_t width, uint32_t height, float near_plane, double t_min, const double* bg,
                double* out_rgba, uint32_t* out_ids, float* out_qp, double* out_layer_rgba,
-               double* out_layer_uv, uint64_t* stats, int num_threads)
+               double* out_layer_uv, uint64_t* stats, int num_threads, int attenuate)
 {
     if (!layers || k < 1 || k > VSO_MAX_LAYERS || sh_degree > 3 || !cam || !out_rgba || !out_ids || !(near_plane > 0.0f))
         return -1;
@@ -377,6 +403,13 @@ int vso_render(const vso_layer* layers, uint32_t k, uint32_t sh_degree, int tex_
                 }
                 vso_sample_bilinear(L->texture, tex_dtype, L->tex_w, L->tex_h, n, uu, vv, coef);
                 vso_decode_rgba(n, coef, Y, lrgba + 4 * l);
+                if (attenuate) {
+                    const uint32_t* ix = L->indices + 3 * (size_t)id;
+                    double nrm[3];
+                    vso_face_normal(L->positions + 3 * (size_t)ix[0], L->positions + 3 * (size_t)ix[1],
+                                    L->positions + 3 * (size_t)ix[2], nrm);
+                    lrgba[4 * l + 3] *= vso_alpha_attenuation(v, nrm);
+                }
                 if (out_layer_rgba) memcpy(out_layer_rgba + ((size_t)l * P + p) * 4, lrgba + 4 * l, 4 * sizeof(double));
                 if (out_layer_uv) { out_layer_uv[((size_t)l * P + p) * 2] = uu; out_layer_uv[((size_t)l * P + p) * 2 + 1] = vv; }
             }
