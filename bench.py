@@ -156,7 +156,7 @@ def run_ours(args):
     sc = build_scene(args.config, rank, world, args)
     B, W, H = len(sc.cameras), sc.width, sc.height
     renderer = binding.Renderer(sc, dev)
-    path_flag = binding.VS_FLAG_TILED_PATH if args.tiled else 0
+    path_flag = (binding.VS_FLAG_TILED_PATH if args.tiled else 0) | (binding.VS_FLAG_ATTENUATION if args.attenuation else 0)
     flags = binding.VS_FLAG_KERNEL_TIMING | path_flag
     params = binding.make_params(W, H, sc.near_plane, sc.t_min, sc.background, flags, args.chunk)
     out = torch.empty((B, H, W, 4), dtype=torch.float32, device=dev)
@@ -254,6 +254,7 @@ def run_ours(args):
                        "texture": "%s %dx%d" % (sc.layers[0].texture.dtype, sc.layers[0].texture.shape[1], sc.layers[0].texture.shape[0]),
                        "raster_path": "tiled (binning + per-tile shared-memory keys)" if args.tiled
                        else "direct (triangle-parallel, 64-bit max keys in HBM/L2)",
+                       "attenuation": bool(args.attenuation),
                        "parallelism": "views sharded, scene replicated (dp%d)" % world,
                        "l2": "no flush: %.1f GiB of textures streamed per step >> 126 MB L2" % (
                            sum(ly.texture.nbytes for ly in sc.layers) / 2 ** 30),
@@ -279,6 +280,7 @@ def main():
     ap.add_argument("--chunk", type=int, default=0, help="views per internal pass (0 = automatic)")
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="oracle work of the cpu_baseline sample (whole views)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--attenuation", action="store_true", help="render with VS_FLAG_ATTENUATION (PAPER.md:L279-286; not the headline workload)")
     ap.add_argument("--tiled", action="store_true", help="time the per-tile raster path (VS_FLAG_TILED_PATH) instead of the default direct one")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -90,9 +90,14 @@ enum {
                                          + one CTA per 16x16 tile with shared-memory keys) instead of the
                                          default triangle-parallel path (64-bit max keys in HBM/L2); same
                                          outputs bit for bit                                                */
-    VS_FLAG_COUNT_TEXELS   = 1u << 2  /* measurement aid: count shaded fragments and, per view, the UNIQUE
+    VS_FLAG_COUNT_TEXELS   = 1u << 2, /* measurement aid: count shaded fragments and, per view, the UNIQUE
                                          texels their 2x2 footprints reference (the algorithmic texture
                                          bytes of DESIGN.md §8); slower, not for timed runs                */
+    VS_FLAG_ATTENUATION    = 1u << 4  /* transparency attenuation (§4.2 "Transparency
+                                         Attenuation"): every fragment's opacity is multiplied by
+                                         alpha_w = 2 Sigmoid(10 |v . n|) - 1 before blending, v = the pixel's
+                                         unit view direction, n = the unit geometric normal of the fragment's
+                                         triangle in world space (reading Q13); off by default     */
 };
 
 typedef struct {

@@ -147,11 +147,12 @@ static vs_status scene_create_impl(const vs_scene_desc* desc, cudaStream_t st, v
     }
     d.v_total = (uint32_t)vt; d.t_total = (uint32_t)tt;
 
-    float* pos; float2* uvs; uint4* tris; uint32_t* flag;
+    float* pos; float2* uvs; uint4* tris; float4* nrm; uint32_t* flag;
     vs_status r;
     if ((r = dev_alloc(s, (void**)&pos, vt * 12)) != VS_OK) return r;
     if ((r = dev_alloc(s, (void**)&uvs, vt * 8)) != VS_OK) return r;
     if ((r = dev_alloc(s, (void**)&tris, tt * 16)) != VS_OK) return r;
+    if ((r = dev_alloc(s, (void**)&nrm, tt * 16)) != VS_OK) return r;
     if ((r = dev_alloc(s, (void**)&flag, 16)) != VS_OK) return r;
     CU(cudaMemsetAsync(flag, 0, 16, st));
     uint64_t voff = 0;
@@ -164,8 +165,8 @@ static vs_status scene_create_impl(const vs_scene_desc* desc, cudaStream_t st, v
         }
         const void* idx = nullptr;
         if ((r = stage_in(L.indices, (size_t)L.num_triangles * 12, desc->memory, st, temps, &idx)) != VS_OK) return r;
-        CU(vs_launch_pack_tris((const uint32_t*)idx, L.num_triangles, L.num_vertices, (uint32_t)voff, l,
-                               tris + d.tri_off[l], flag, st));
+        CU(vs_launch_pack_tris((const uint32_t*)idx, pos + 3 * voff, L.num_triangles, L.num_vertices, (uint32_t)voff, l,
+                               tris + d.tri_off[l], nrm + d.tri_off[l], flag, st));
         // texture -> internal layout (same element order, texel padded to a multiple of 16 bytes)
         const size_t texels = (size_t)L.tex_w * L.tex_h;
         const size_t src_bytes = texels * n * 4 * (f16 ? 2 : 4);
@@ -186,7 +187,7 @@ static vs_status scene_create_impl(const vs_scene_desc* desc, cudaStream_t st, v
     CU(cudaStreamSynchronize(st));
     if (hflag & 1u) return fail(VS_ERR_INVALID_ARG, "a triangle index is >= num_vertices of its layer");
     if (hflag & 2u) return fail(VS_ERR_INVALID_ARG, "a vertex position or uv is not finite");
-    d.positions = pos; d.uvs = uvs; d.tris = tris;
+    d.positions = pos; d.uvs = uvs; d.tris = tris; d.tri_nrm = nrm;
     CU(cudaHostAlloc((void**)&s->host_counters, VS_CNT_N * 8, cudaHostAllocDefault));
     CU(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
     for (int i = 0; i < 2; ++i) {
@@ -235,7 +236,7 @@ static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, u
     if (p->width > 16384 || p->height > 16384) return fail(VS_ERR_UNSUPPORTED, "image larger than 16384 px");
     if (!(p->near_plane > 0.0f) || !std::isfinite(p->near_plane)) return fail(VS_ERR_INVALID_ARG, "near_plane must be > 0");
     if (!(p->t_min >= 0.0f) || !std::isfinite(p->t_min)) return fail(VS_ERR_INVALID_ARG, "t_min must be >= 0");
-    if (p->flags & ~(uint32_t)(VS_FLAG_REFERENCE_PATH | VS_FLAG_KERNEL_TIMING | VS_FLAG_COUNT_TEXELS | VS_FLAG_TILED_PATH))
+    if (p->flags & ~(uint32_t)(VS_FLAG_REFERENCE_PATH | VS_FLAG_KERNEL_TIMING | VS_FLAG_COUNT_TEXELS | VS_FLAG_TILED_PATH | VS_FLAG_ATTENUATION))
         return fail(VS_ERR_INVALID_ARG, "reserved flag bits set");
     for (int i = 0; i < 3; ++i)
         if (!std::isfinite(p->background[i])) return fail(VS_ERR_INVALID_ARG, "background not finite");
@@ -295,6 +296,7 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
     fr.tiles_x = (p->width + VS_TILE_W - 1) / VS_TILE_W; fr.tiles_y = (p->height + VS_TILE_H - 1) / VS_TILE_H;
     fr.near_plane = p->near_plane; fr.t_min = p->t_min;
     for (int i = 0; i < 3; ++i) fr.bg[i] = p->background[i];
+    fr.attenuate = (p->flags & VS_FLAG_ATTENUATION) ? 1u : 0u;
     const size_t ntile = (size_t)views * fr.tiles_x * fr.tiles_y;
     if (ntile >= (1ull << 31)) return fail(VS_ERR_UNSUPPORTED, "too many tiles in one chunk");
     const bool reference = (p->flags & VS_FLAG_REFERENCE_PATH) != 0;

@@ -18,6 +18,8 @@ struct VsSceneDev {
     const float* positions;   // [v_total][3], all layers concatenated
     const float2* uvs;        // [v_total]
     const uint4* tris;        // [t_total] {i0, i1, i2 : global vertex index, w : layer}
+    const float4* tri_nrm;    // [t_total] unit geometric normal in world space (fp64 cross product rounded to fp32), w = 0;
+                              //           zero vector for zero-area triangles.  Read only under VS_FLAG_ATTENUATION
     uint32_t v_total, t_total;
     uint32_t k, sh_degree, n_coef;
     uint32_t texel_vecs;                  // 16-byte vectors per texel in the internal layout (= 4 * np_pad * elem / 16)
@@ -39,6 +41,7 @@ struct VsFrame {
     uint32_t width, height, tiles_x, tiles_y;
     float near_plane, t_min;
     float bg[3];
+    uint32_t attenuate;       // VS_FLAG_ATTENUATION: opacity *= alpha_w(view direction, face normal)
 };
 
 // counters[0] dropped, [1] degenerate, [2] tile refs, [3] shaded fragments, [4] unique texels,
@@ -179,6 +182,13 @@ __device__ __forceinline__ float vs_sigmoid(float s)
     return __fdividef(1.0f, 1.0f + __expf(-s));
 }
 
+// transparency attenuation alpha_w = 2 Sigmoid(10 |v . n|) - 1; v, n unit (n may be 0)
+__device__ __forceinline__ float vs_alpha_w(float vx, float vy, float vz, const float4 n)
+{
+    const float d = fabsf(fmaf(vx, n.x, fmaf(vy, n.y, vz * n.z)));
+    return fmaf(2.0f, vs_sigmoid(10.0f * d), -1.0f);
+}
+
 // ---- fragment setup (S5 addressing): winning triangle of a layer at pixel
 // (px, py) -> clamped texel columns / rows of the 2x2 footprint and the bilinear fractions.
 struct VsFrag {
@@ -262,8 +272,8 @@ cudaError_t vs_launch_popcount(const uint32_t* words, size_t n, unsigned long lo
 cudaError_t vs_launch_reference(const VsSceneDev& sc, int tex_f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 
 // scene construction helpers
-cudaError_t vs_launch_pack_tris(const uint32_t* indices, uint32_t num_tris, uint32_t num_vertices, uint32_t vtx_off,
-                                uint32_t layer, uint4* out, uint32_t* error_flag, cudaStream_t st);
+cudaError_t vs_launch_pack_tris(const uint32_t* indices, const float* layer_positions, uint32_t num_tris, uint32_t num_vertices,
+                                uint32_t vtx_off, uint32_t layer, uint4* out, float4* out_normals, uint32_t* error_flag, cudaStream_t st);
 cudaError_t vs_launch_check_finite(const float* v, size_t n, uint32_t* error_flag, cudaStream_t st);
 cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, uint32_t n_coef, uint32_t np_pad,
                                    uint4* dst, cudaStream_t st);

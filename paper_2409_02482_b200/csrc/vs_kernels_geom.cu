@@ -5,14 +5,23 @@
 // ------------------------------------------------------------------------------------------------
 // S0: scene packing (once per scene)
 // ------------------------------------------------------------------------------------------------
-__global__ void k_pack_tris(const uint32_t* __restrict__ idx, uint32_t nt, uint32_t nv, uint32_t voff, uint32_t layer,
-                            uint4* __restrict__ out, uint32_t* err)
+__global__ void k_pack_tris(const uint32_t* __restrict__ idx, const float* __restrict__ pos, uint32_t nt, uint32_t nv,
+                            uint32_t voff, uint32_t layer, uint4* __restrict__ out, float4* __restrict__ nrm, uint32_t* err)
 {
     uint32_t t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= nt) return;
     uint32_t a = idx[3 * (size_t)t], b = idx[3 * (size_t)t + 1], c = idx[3 * (size_t)t + 2];
     if (a >= nv || b >= nv || c >= nv) { atomicOr(err, 1u); a = b = c = 0; }
     out[t] = make_uint4(a + voff, b + voff, c + voff, layer);
+    // unit geometric normal (for the transparency attenuation): fp64 cross product of the fp32 positions, once per scene
+    const double ax = (double)pos[3 * (size_t)b] - (double)pos[3 * (size_t)a], ay = (double)pos[3 * (size_t)b + 1] - (double)pos[3 * (size_t)a + 1],
+                 az = (double)pos[3 * (size_t)b + 2] - (double)pos[3 * (size_t)a + 2];
+    const double bx = (double)pos[3 * (size_t)c] - (double)pos[3 * (size_t)a], by = (double)pos[3 * (size_t)c + 1] - (double)pos[3 * (size_t)a + 1],
+                 bz = (double)pos[3 * (size_t)c + 2] - (double)pos[3 * (size_t)a + 2];
+    const double nx = ay * bz - az * by, ny = az * bx - ax * bz, nz = ax * by - ay * bx;
+    const double len = sqrt(nx * nx + ny * ny + nz * nz);
+    const double inv = len > 0.0 ? 1.0 / len : 0.0;
+    nrm[t] = make_float4((float)(nx * inv), (float)(ny * inv), (float)(nz * inv), 0.0f);
 }
 
 __global__ void k_check_finite(const float* __restrict__ v, size_t n, uint32_t* err)
@@ -37,11 +46,12 @@ __global__ void k_pack_texture(const T* __restrict__ src, uint32_t n_texels, uin
     }
 }
 
-cudaError_t vs_launch_pack_tris(const uint32_t* indices, uint32_t num_tris, uint32_t num_vertices, uint32_t vtx_off,
-                                uint32_t layer, uint4* out, uint32_t* error_flag, cudaStream_t st)
+cudaError_t vs_launch_pack_tris(const uint32_t* indices, const float* layer_positions, uint32_t num_tris, uint32_t num_vertices,
+                                uint32_t vtx_off, uint32_t layer, uint4* out, float4* out_normals, uint32_t* error_flag, cudaStream_t st)
 {
     if (num_tris == 0) return cudaSuccess;
-    k_pack_tris<<<(num_tris + 255) / 256, 256, 0, st>>>(indices, num_tris, num_vertices, vtx_off, layer, out, error_flag);
+    k_pack_tris<<<(num_tris + 255) / 256, 256, 0, st>>>(indices, layer_positions, num_tris, num_vertices, vtx_off, layer, out,
+                                                        out_normals, error_flag);
     return cudaGetLastError();
 }
 

@@ -325,7 +325,8 @@ k_reference(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ 
                 }
                 s[ch] += Y[c] * v;
             }
-        const float A = vs_sigmoid(s[3]);
+        float A = vs_sigmoid(s[3]);
+        if (fr.attenuate) A *= vs_alpha_w(vx, vy, vz, sc.tri_nrm[sc.tri_off[l] + lid]);
         for (int ch = 0; ch < 3; ++ch) C[ch] += Tr * A * vs_sigmoid(s[ch]);
         Tr *= (1.0f - A);
         if (Tr < fr.t_min) alive = false;

@@ -112,6 +112,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     uint32_t* rec_xy = reinterpret_cast<uint32_t*>(smem);
     float2* rec_ab = reinterpret_cast<float2*>(smem + (size_t)sc.k * VS_TILE_PIX * 4);
     unsigned char* per_warp = smem + (size_t)sc.k * VS_TILE_PIX * 12;  // 8 x (2 KB basis + 1 KB records + 512 B logits)
+    float* rec_aw = reinterpret_cast<float*>(per_warp + 8 * 3584);      // [k][256] attenuation weights (only if fr.attenuate)
 
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t tile = blockIdx.x, view = blockIdx.y;
@@ -163,6 +164,14 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
 #pragma unroll
         for (int u = 0; u < VS_MAX_LAYERS; ++u)
             tri[u] = id[u] != VS_MISS ? __ldg(&sc.tris[sc.tri_off[u] + id[u]]) : make_uint4(0, 0, 0, 0);
+        if (fr.attenuate) {  // alpha_w of every layer's fragment: all of a pixel's fragments share its view direction
+            float vx, vy, vz;
+            vs_view_dir(cams[view], px, py, vx, vy, vz);
+#pragma unroll
+            for (int u = 0; u < VS_MAX_LAYERS; ++u)
+                if (u < (int)sc.k && id[u] != VS_MISS)
+                    rec_aw[u * VS_TILE_PIX + tid] = vs_alpha_w(vx, vy, vz, __ldg(&sc.tri_nrm[sc.tri_off[u] + id[u]]));
+        }
 #pragma unroll
         for (int u = 0; u < VS_MAX_LAYERS; ++u) {
             if (u < (int)sc.k) {
@@ -311,7 +320,8 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
         __syncwarp();
         if (shade) {
             const float4 s4 = part[own_slot];
-            const float A = vs_sigmoid(s4.w);
+            float A = vs_sigmoid(s4.w);
+            if (fr.attenuate) A *= rec_aw[l * VS_TILE_PIX + tid];
             const float TA = Tr * A;
             Cr += TA * vs_sigmoid(s4.x); Cg += TA * vs_sigmoid(s4.y); Cb += TA * vs_sigmoid(s4.z);
             Tr *= (1.0f - A);
@@ -326,7 +336,7 @@ template <int F16, int DEG, bool COUNT>
 static cudaError_t launch_sh2(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
 {
     if (sc.texel_vecs != (uint32_t)VsShadeShape<F16, DEG>::NVEC) return cudaErrorInvalidValue;
-    const size_t smem = (size_t)sc.k * VS_TILE_PIX * 12 + 8 * 3584;
+    const size_t smem = (size_t)sc.k * VS_TILE_PIX * (fr.attenuate ? 16 : 12) + 8 * 3584;
     auto kern = k_shade<F16, DEG, COUNT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

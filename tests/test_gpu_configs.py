@@ -89,6 +89,28 @@ def test_config4_full(env):
     _check_config(env, 4, [0, 29, 63], [0, 63])
 
 
+def test_config4_full_attenuation(env):
+    """SURVEY.md §8(f) NEXT-2 at the headline size: VS_FLAG_ATTENUATION on C4, whole batch in one
+    call as bench.py --attenuation times it; two views against the oracle."""
+    b, torch = env.binding, env.torch
+    sc = env.synth.make_config(4)
+    B, W, H = len(sc.cameras), sc.width, sc.height
+    r = b.Renderer(sc)
+    p = b.make_params(W, H, sc.near_plane, sc.t_min, sc.background, b.VS_FLAG_ATTENUATION)
+    out = torch.empty((B, H, W, 4), dtype=torch.float32, device="cuda")
+    b.vs_render(r.handle, sc.cameras, p, out)
+    torch.cuda.synchronize()
+    worst = 0.0
+    for v in (0, 63):
+        got = out[v].cpu().numpy()
+        ref = env.oracle.render_scene(sc, [v], attenuation=True)[0]
+        err = float(np.abs(got.astype(np.float64) - ref["rgba"]).max())
+        worst = max(worst, err)
+        assert err <= TOL, "C4 attenuated, view %d: max abs rgba error %.3e" % (v, err)
+    r.close()
+    print("C4 full size, attenuated: worst rgba err %.3e" % worst)
+
+
 def test_config5_full(env):
     # even views are far cameras (r = 3), odd views close-ups (r = 1.6) that fill the frame
     _check_config(env, 5, [0, 1, 15], [0, 1])

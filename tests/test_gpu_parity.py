@@ -38,9 +38,11 @@ def gpu_render(env, sc, views, flags=0, t_min=None, background=None, views_per_c
     return out
 
 
-def check_against_oracle(env, sc, views, **kw):
+def check_against_oracle(env, sc, views, attenuation=False, **kw):
+    if attenuation:
+        kw["flags"] = kw.get("flags", 0) | env.binding.VS_FLAG_ATTENUATION
     rgba, ids, stats = gpu_render(env, sc, views, **kw)
-    okw = {}
+    okw = {"attenuation": True} if attenuation else {}
     if "t_min" in kw and kw["t_min"] is not None:
         okw["t_min"] = kw["t_min"]
     if "background" in kw and kw["background"] is not None:
@@ -83,6 +85,44 @@ def test_reduced_configs(env, cfg, kw):
     sc = env.synth.make_config(cfg, **kw)
     worst, _, ids = check_against_oracle(env, sc, range(len(sc.cameras)), views_per_chunk=2)
     print("C%d reduced worst rgba err %.3e, coverage %.2f" % (cfg, worst, (ids != env.binding.MISS).mean()))
+
+
+# ---- transparency attenuation behind VS_FLAG_ATTENUATION ----
+def test_attenuation_config1(env):
+    sc = env.synth.make_config(1)
+    worst, rgba, ids = check_against_oracle(env, sc, range(4), attenuation=True)
+    plain = gpu_render(env, sc, range(4))
+    assert np.array_equal(plain[1], ids)                       # coverage does not depend on the flag
+    hit = (ids != env.binding.MISS).any(axis=1)
+    assert np.all(rgba[..., 3][hit] <= plain[0][..., 3][hit])  # alpha_w <= 1 can only lower the alpha
+    assert (rgba[..., 3][hit] < plain[0][..., 3][hit] - 1e-3).mean() > 0.05   # and does so near the silhouettes
+    # the brute-force kernel applies the same weight
+    check_against_oracle(env, sc, [1], attenuation=True, flags=env.binding.VS_FLAG_REFERENCE_PATH)
+    print("C1 attenuated worst rgba err %.3e" % worst)
+
+
+@pytest.mark.parametrize("cfg,kw", [
+    (3, dict(mesh_n=48, width=400, height=225, tex_size=256, num_cameras=3, k=7)),     # fp16 deg 3, low alpha
+    (5, dict(mesh_n=120, width=384, height=216, tex_size=512, num_cameras=4, k=9)),    # sub-pixel tris + close-ups
+])
+def test_attenuation_reduced_configs(env, cfg, kw):
+    sc = env.synth.make_config(cfg, **kw)
+    worst, _, _ = check_against_oracle(env, sc, range(len(sc.cameras)), attenuation=True, views_per_chunk=2)
+    check_against_oracle(env, sc, [0], attenuation=True, t_min=2.0 ** -6, background=(0.3, 0.1, 0.2))
+    print("C%d reduced, attenuated: worst rgba err %.3e" % (cfg, worst))
+
+
+def test_attenuation_degenerate_and_big_triangles(env):
+    s = env.synth
+    rng = np.random.default_rng(7)
+    # tilted big quad + a triangle whose world area is zero (its normal is 0 -> alpha_w = 0; it covers nothing anyway)
+    pos = np.array([[-2, -2, 3], [2, -2, 5], [2, 2, 5], [-2, 2, 3], [0, 0, 3.5]], np.float32)
+    uv = np.array([[0, 0], [1, 0], [1, 1], [0, 1], [0.5, 0.5]], np.float32)
+    idx = np.array([[0, 1, 2], [0, 2, 3], [0, 0, 1], [2, 1, 4]], np.uint32)
+    tex = rng.normal(0, 0.5, (32, 32, 4, 4)).astype(np.float32)
+    sc = s.Scene("att", [s.Layer(pos, uv, idx, tex)], 1,
+                 np.stack([s.look_at_camera((0.3, 0.2, -1.0), 150, 100, target=(0, 0, 4.0))]), 150, 100)
+    check_against_oracle(env, sc, [0], attenuation=True)
 
 
 def test_determinism_and_chunking(env):
