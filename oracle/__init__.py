@@ -23,6 +23,10 @@ class _Layer(C.Structure):
                 ("tex_w", C.c_uint32), ("tex_h", C.c_uint32)]
 
 
+class _Bands(C.Structure):
+    _fields_ = [("tex", C.c_void_p * 4), ("w", C.c_uint32 * 4), ("h", C.c_uint32 * 4)]
+
+
 _lib = None
 
 
@@ -35,6 +39,16 @@ def lib():
                                  C.c_uint32, C.c_uint32, C.c_float, C.c_double, C.c_void_p,
                                  C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                  C.c_void_p, C.c_int, C.c_int]
+        L.vso_render_banded.restype = C.c_int
+        L.vso_render_banded.argtypes = [C.POINTER(_Layer), C.POINTER(_Bands), C.c_double, C.c_double, C.c_uint32, C.c_uint32,
+                                        C.c_void_p, C.c_uint32, C.c_uint32, C.c_float, C.c_double, C.c_void_p,
+                                        C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
+                                        C.c_void_p, C.c_int, C.c_int]
+        L.vso_quantize.restype = C.c_double
+        L.vso_quantize.argtypes = [C.c_double]
+        L.vso_rescale.restype = C.c_double
+        L.vso_rescale.argtypes = [C.c_double, C.c_double, C.c_double]
+        L.vso_sample_banded.argtypes = [C.POINTER(_Bands), C.c_uint32, C.c_double, C.c_double, C.c_double, C.c_double, C.c_void_p]
         L.vso_alpha_attenuation.restype = C.c_double
         L.vso_alpha_attenuation.argtypes = [C.c_void_p, C.c_void_p]
         L.vso_face_normal.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -71,28 +85,43 @@ def max_threads() -> int:
 def render_view(layers, sh_degree: int, camera, width: int, height: int, *, near_plane: float = 0.05,
                 t_min: float = 2.0 ** -14, background=(0.0, 0.0, 0.0), num_threads: int = 0,
                 want_qp: bool = False, want_layer_rgba: bool = False, want_layer_uv: bool = False,
-                attenuation: bool = False):
+                attenuation: bool = False, v_range=None):
     """Render one view.  `layers`: objects with positions/uvs/indices/texture numpy arrays
-    (outermost first).  Returns dict(rgba [H,W,4] f64, ids [k,H,W] u32, stats [2] u64, ...)."""
+    (outermost first); layers with a `band_textures` list (uint8 [h_b, w_b, 2b+1, 4] per SH band) are
+    rendered in the paper's banded 8-bit format, re-scaled to `v_range` = (v_min, v_max).
+    Returns dict(rgba [H,W,4] f64, ids [k,H,W] u32, stats [2] u64, ...)."""
     k = len(layers)
     n = (sh_degree + 1) ** 2
     keep = []
     arr = (_Layer * k)()
+    banded = getattr(layers[0], "band_textures", None) is not None
+    bands = (_Bands * k)() if banded else None
     code = None
     for i, L in enumerate(layers):
         pos = np.ascontiguousarray(L.positions, dtype=np.float32)
         uv = np.ascontiguousarray(L.uvs, dtype=np.float32)
         idx = np.ascontiguousarray(L.indices, dtype=np.uint32)
+        assert pos.ndim == 2 and pos.shape[1] == 3 and uv.shape == (pos.shape[0], 2)
+        assert idx.ndim == 2 and idx.shape[1] == 3
+        assert idx.size == 0 or int(idx.max()) < pos.shape[0]
+        keep += [pos, uv, idx]
+        if banded:
+            assert len(L.band_textures) == sh_degree + 1 and v_range is not None
+            for b, t in enumerate(L.band_textures):
+                t = np.ascontiguousarray(t)
+                assert t.dtype == np.uint8 and t.ndim == 4 and t.shape[2] == 2 * b + 1 and t.shape[3] == 4, t.shape
+                keep.append(t)
+                bands[i].tex[b] = t.ctypes.data
+                bands[i].w[b], bands[i].h[b] = t.shape[1], t.shape[0]
+            arr[i] = _Layer(_ptr(pos), _ptr(uv), _ptr(idx), None, pos.shape[0], idx.shape[0], 0, 0)
+            continue
         tex = np.ascontiguousarray(L.texture)
         c = _dtype_code(tex)
         if code is None:
             code = c
         assert c == code, "all layers must share one texture dtype"
         assert tex.ndim == 4 and tex.shape[2] == n and tex.shape[3] == 4, tex.shape
-        assert pos.ndim == 2 and pos.shape[1] == 3 and uv.shape == (pos.shape[0], 2)
-        assert idx.ndim == 2 and idx.shape[1] == 3
-        assert idx.size == 0 or int(idx.max()) < pos.shape[0]
-        keep += [pos, uv, idx, tex]
+        keep.append(tex)
         arr[i] = _Layer(_ptr(pos), _ptr(uv), _ptr(idx), _ptr(tex), pos.shape[0], idx.shape[0],
                         tex.shape[1], tex.shape[0])
     cam = np.ascontiguousarray(camera, dtype=np.float32)
@@ -104,10 +133,14 @@ def render_view(layers, sh_degree: int, camera, width: int, height: int, *, near
     lrgba = np.empty((k, height, width, 4), dtype=np.float64) if want_layer_rgba else None
     luv = np.empty((k, height, width, 2), dtype=np.float64) if want_layer_uv else None
     stats = np.zeros(2, dtype=np.uint64)
-    rc = lib().vso_render(arr, k, sh_degree, code, _ptr(cam), width, height, near_plane, t_min, _ptr(bg),
-                          _ptr(rgba), _ptr(ids), _ptr(qp) if want_qp else None,
-                          _ptr(lrgba) if want_layer_rgba else None, _ptr(luv) if want_layer_uv else None,
-                          _ptr(stats), num_threads, 1 if attenuation else 0)
+    tail = (_ptr(rgba), _ptr(ids), _ptr(qp) if want_qp else None,
+            _ptr(lrgba) if want_layer_rgba else None, _ptr(luv) if want_layer_uv else None,
+            _ptr(stats), num_threads, 1 if attenuation else 0)
+    if banded:
+        rc = lib().vso_render_banded(arr, bands, float(v_range[0]), float(v_range[1]), k, sh_degree, _ptr(cam), width,
+                                     height, near_plane, t_min, _ptr(bg), *tail)
+    else:
+        rc = lib().vso_render(arr, k, sh_degree, code, _ptr(cam), width, height, near_plane, t_min, _ptr(bg), *tail)
     if rc != 0:
         raise ValueError("vso_render rejected its arguments (rc=%d)" % rc)
     out = dict(rgba=rgba, ids=ids, stats=stats)
@@ -126,6 +159,8 @@ def render_scene(scene, views=None, **kw):
     kw.setdefault("near_plane", scene.near_plane)
     kw.setdefault("t_min", scene.t_min)
     kw.setdefault("background", scene.background)
+    if getattr(scene, "v_range", None) is not None:
+        kw.setdefault("v_range", scene.v_range)
     return [render_view(scene.layers, scene.sh_degree, scene.cameras[v], scene.width, scene.height, **kw)
             for v in views]
 
@@ -156,6 +191,28 @@ def decode_rgba(coef: np.ndarray, Y: np.ndarray) -> np.ndarray:
     Y = np.ascontiguousarray(Y, dtype=np.float64)
     out = np.empty(4, dtype=np.float64)
     lib().vso_decode_rgba(coef.shape[0], _ptr(coef), _ptr(Y), _ptr(out))
+    return out
+
+
+def quantize(x: float) -> float:
+    return float(lib().vso_quantize(float(x)))
+
+
+def rescale(q: float, v_min: float, v_max: float) -> float:
+    return float(lib().vso_rescale(float(q), float(v_min), float(v_max)))
+
+
+def sample_banded(band_textures, v_min: float, v_max: float, u: float, v: float) -> np.ndarray:
+    deg = len(band_textures) - 1
+    B = _Bands()
+    keep = []
+    for b, t in enumerate(band_textures):
+        t = np.ascontiguousarray(t, dtype=np.uint8)
+        keep.append(t)
+        B.tex[b] = t.ctypes.data
+        B.w[b], B.h[b] = t.shape[1], t.shape[0]
+    out = np.empty(((deg + 1) ** 2, 4), dtype=np.float64)
+    lib().vso_sample_banded(C.byref(B), deg, float(v_min), float(v_max), float(u), float(v), _ptr(out))
     return out
 
 

@@ -189,6 +189,7 @@ void vso_sh_basis(int degree, const double* v, double* Y)
 static inline double tex_fetch(const void* tex, int dtype, uint32_t W, uint32_t n, int64_t ix, int64_t iy, uint32_t e)
 {
     size_t o = (((size_t)iy * W + (size_t)ix) * n) * 4 + e;
+    if (dtype == 2) return (double)((const uint8_t*)tex)[o]; /* stored byte t = 255 q, 0..255 (banded format below) */
     return dtype == 0 ? (double)((const float*)tex)[o] : vso_half_to_double(((const uint16_t*)tex)[o]);
 }
 
@@ -208,6 +209,39 @@ void vso_sample_bilinear(const void* tex, int dtype, uint32_t W, uint32_t H, uin
         double t00 = tex_fetch(tex, dtype, W, n, ix0, iy0, e), t01 = tex_fetch(tex, dtype, W, n, ix1, iy0, e);
         double t10 = tex_fetch(tex, dtype, W, n, ix0, iy1, e), t11 = tex_fetch(tex, dtype, W, n, ix1, iy1, e);
         out[e] = (1.0 - b) * ((1.0 - a) * t00 + a * t01) + b * ((1.0 - a) * t10 + a * t11);
+    }
+}
+
+/* ---- The paper's baked texture format (§4.5 "Mixed resolutions", "Squeezing and quantization";
+ *      SURVEY.md §8(f) NEXT-1): one 8-bit image set per SH band b = 0..deg, band b holding its 2b+1 coefficients x 4
+ *      channels at its OWN resolution ("scaling texture resolution proportionally to the SH coefficient degree: the
+ *      base color at the highest resolution (2048^2), the highest SH degree at the lowest (256^2)").  A stored byte t
+ *      is 255 q(sh^) with q(x) = round(255 x)/255; "before rendering, we re-scale value to a hyper-parameters
+ *      controlled range": sh = v_min + (v_max - v_min) q.  Each band is sampled bilinearly at its own texel centres
+ *      (the stored values are what the texture unit interpolates; the affine re-scale follows), and the bands are
+ *      "concatenated over the coefficient dimension" (L438) into coef[c][ch], c = b^2 .. b^2 + 2b. ---- */
+typedef struct {
+    const uint8_t* tex[4]; /* band b: [h[b]][w[b]][2b+1][4] */
+    uint32_t w[4], h[4];
+} vso_bands;
+
+double vso_quantize(double x) /* q(x) = round(255 x) / 255, x in [0,1]; halves round away from zero (C round()) */
+{
+    return round(255.0 * x) / 255.0;
+}
+
+double vso_rescale(double q, double v_min, double v_max) /* sh = v_min + (v_max - v_min) q */
+{
+    return v_min + (v_max - v_min) * q;
+}
+
+void vso_sample_banded(const vso_bands* B, uint32_t degree, double v_min, double v_max, double u, double v, double* coef)
+{
+    double t[4 * 7];
+    for (uint32_t b = 0; b <= degree; ++b) {
+        uint32_t nb = 2 * b + 1;
+        vso_sample_bilinear(B->tex[b], 2, B->w[b], B->h[b], nb, u, v, t);
+        for (uint32_t e = 0; e < 4 * nb; ++e) coef[4 * (b * b) + e] = vso_rescale(t[e] / 255.0, v_min, v_max);
     }
 }
 
@@ -287,10 +321,11 @@ static void view_dir(const float* cam, int px, int py, double* v)
  *                   (PAPER.md:L279-286); the alpha of out_layer_rgba is the attenuated one
  * Returns 0, or -1 on bad arguments / allocation failure.
  */
-int vso_render(const vso_layer* layers, uint32_t k, uint32_t sh_degree, int tex_dtype, const float* cam,
-               uint32_t width, uint32_t height, float near_plane, double t_min, const double* bg,
-               double* out_rgba, uint32_t* out_ids, float* out_qp, double* out_layer_rgba,
-               double* out_layer_uv, uint64_t* stats, int num_threads, int attenuate)
+static int render_impl(const vso_layer* layers, const vso_bands* btex, double v_min, double v_max, uint32_t k,
+                       uint32_t sh_degree, int tex_dtype, const float* cam,
+                       uint32_t width, uint32_t height, float near_plane, double t_min, const double* bg,
+                       double* out_rgba, uint32_t* out_ids, float* out_qp, double* out_layer_rgba,
+                       double* out_layer_uv, uint64_t* stats, int num_threads, int attenuate)
 {
     if (!layers || k < 1 || k > VSO_MAX_LAYERS || sh_degree > 3 || !cam || !out_rgba || !out_ids || !(near_plane > 0.0f))
         return -1;
@@ -401,7 +436,8 @@ int vso_render(const vso_layer* layers, uint32_t k, uint32_t sh_degree, int tex_
                     uu += b * (double)L->uvs[2 * (size_t)tri.vi[c] + 0];
                     vv += b * (double)L->uvs[2 * (size_t)tri.vi[c] + 1];
                 }
-                vso_sample_bilinear(L->texture, tex_dtype, L->tex_w, L->tex_h, n, uu, vv, coef);
+                if (btex) vso_sample_banded(&btex[l], sh_degree, v_min, v_max, uu, vv, coef);
+                else vso_sample_bilinear(L->texture, tex_dtype, L->tex_w, L->tex_h, n, uu, vv, coef);
                 vso_decode_rgba(n, coef, Y, lrgba + 4 * l);
                 if (attenuate) {
                     const uint32_t* ix = L->indices + 3 * (size_t)id;
@@ -422,6 +458,29 @@ int vso_render(const vso_layer* layers, uint32_t k, uint32_t sh_degree, int tex_
     free(vtx);
     free(keys);
     return 0;
+}
+
+int vso_render(const vso_layer* layers, uint32_t k, uint32_t sh_degree, int tex_dtype, const float* cam,
+               uint32_t width, uint32_t height, float near_plane, double t_min, const double* bg,
+               double* out_rgba, uint32_t* out_ids, float* out_qp, double* out_layer_rgba,
+               double* out_layer_uv, uint64_t* stats, int num_threads, int attenuate)
+{
+    return render_impl(layers, NULL, 0.0, 0.0, k, sh_degree, tex_dtype, cam, width, height, near_plane, t_min, bg, out_rgba,
+                       out_ids, out_qp, out_layer_rgba, out_layer_uv, stats, num_threads, attenuate);
+}
+
+/* The same render with the paper's banded 8-bit textures (layers[l].texture is ignored; bands[l] is used). */
+int vso_render_banded(const vso_layer* layers, const vso_bands* bands, double v_min, double v_max, uint32_t k,
+                      uint32_t sh_degree, const float* cam, uint32_t width, uint32_t height, float near_plane,
+                      double t_min, const double* bg, double* out_rgba, uint32_t* out_ids, float* out_qp,
+                      double* out_layer_rgba, double* out_layer_uv, uint64_t* stats, int num_threads, int attenuate)
+{
+    if (!bands) return -1;
+    for (uint32_t l = 0; l < k && l < VSO_MAX_LAYERS; ++l)
+        for (uint32_t b = 0; b <= sh_degree && b < 4; ++b)
+            if (!bands[l].tex[b] || bands[l].w[b] == 0 || bands[l].h[b] == 0) return -1;
+    return render_impl(layers, bands, v_min, v_max, k, sh_degree, 2, cam, width, height, near_plane, t_min, bg, out_rgba,
+                       out_ids, out_qp, out_layer_rgba, out_layer_uv, stats, num_threads, attenuate);
 }
 
 int vso_max_threads(void)

@@ -27,7 +27,8 @@ class Layer:
     positions: np.ndarray  # [V,3] float32, world space
     uvs: np.ndarray        # [V,2] float32 in [0,1]
     indices: np.ndarray    # [T,3] uint32
-    texture: np.ndarray    # [H,W,n,4] float32 or float16 ; ch 0-2 RGB, ch 3 opacity logit
+    texture: np.ndarray    # [H,W,n,4] float32 or float16 ; ch 0-2 RGB, ch 3 opacity logit (None for banded scenes)
+    band_textures: list | None = None   # banded 8-bit format: band b = uint8 [H_b, W_b, 2b+1, 4]
 
 
 @dataclasses.dataclass
@@ -41,6 +42,7 @@ class Scene:
     near_plane: float = 0.05
     t_min: float = 2.0 ** -14
     background: tuple = (0.0, 0.0, 0.0)
+    v_range: tuple | None = None   # banded scenes: (v_min, v_max) the stored bytes are re-scaled to
 
     @property
     def k(self) -> int:
@@ -52,7 +54,7 @@ class Scene:
 
     @property
     def tex_dtype(self):
-        return self.layers[0].texture.dtype
+        return np.dtype(np.uint8) if self.layers[0].band_textures is not None else self.layers[0].texture.dtype
 
 
 # ------------------------------------------------------------------------------------------------
@@ -224,6 +226,24 @@ def normal_texture(seed_key, tex_h: int, tex_w: int, n_coef: int, sigma: float, 
     return tex
 
 
+def banded_textures(seed_key, base_size: int, degree: int, sigma_lsb: float = 2.55):
+    """The paper's baked texture format: one 8-bit image set per SH band, band b at
+    (base_size >> b)^2 ("base color at the highest resolution, the highest SH degree at the lowest": 2048^2 .. 256^2
+    for degree 3).  Bytes ~ round(N(127.5, sigma_lsb)) clipped to 0..255: with the paper's range [-15, 15]
+    (30/255 per step) sigma_lsb = 2.55 is the N(0, 0.3) coefficient spread of the float configurations."""
+    rng = np.random.default_rng(seed_key)
+    out = []
+    for b in range(degree + 1):
+        size = max(1, base_size >> b)
+        t = rng.standard_normal((size, size, 2 * b + 1, 4), dtype=np.float32)
+        t *= np.float32(sigma_lsb)
+        t += np.float32(127.5)
+        np.rint(t, out=t)
+        np.clip(t, 0, 255, out=t)
+        out.append(t.astype(np.uint8))
+    return out
+
+
 def _parallel(fns):
     with ThreadPoolExecutor(max_workers=min(len(fns), 16)) as ex:
         return list(ex.map(lambda f: f(), fns))
@@ -244,9 +264,11 @@ CONFIG_NAMES = {
 
 def make_config(cfg: int, *, seed: int = 0, mesh_n: int | None = None, width: int | None = None,
                 height: int | None = None, tex_size: int | None = None, num_cameras: int | None = None,
-                k: int | None = None, camera_rotate: float = 0.0) -> Scene:
+                k: int | None = None, camera_rotate: float = 0.0, banded: bool = False) -> Scene:
     """Build configuration `cfg` (1..5).  The keyword overrides give *reduced* variants of the same
-    recipe (used by the CPU tests, where the full sizes would take too long)."""
+    recipe (used by the CPU tests, where the full sizes would take too long).  `banded=True` gives the
+    same geometry and cameras with the paper's 8-bit mixed-resolution textures (`banded_textures`, v_range (-15, 15))
+    instead of the float ones."""
     if cfg == 1:
         k = k or 3
         ts = tex_size or 256
@@ -256,12 +278,17 @@ def make_config(cfg: int, *, seed: int = 0, mesh_n: int | None = None, width: in
         layers = []
         for l in range(k):
             pos, uv, idx = icosphere_charted(3 if mesh_n is None else mesh_n, radii[l], ts)
+            if banded:
+                layers.append(Layer(pos, uv, idx, None, banded_textures([seed, 101, l], ts, 1, 8.0)))
+                continue
             rng = np.random.default_rng([seed, 1, l])
             tex = np.empty((ts, ts, 4, 4), dtype=np.float32)
             tex[..., :3] = rng.uniform(-0.5, 0.5, size=(ts, ts, 4, 3))
             tex[..., 3] = rng.standard_normal((ts, ts, 4))
             layers.append(Layer(pos, uv, idx, tex))
         cams = circle_cameras(B, 3.0, W, H)
+        if banded:
+            return Scene(CONFIG_NAMES[1] + " [banded u8]", layers, 1, cams, W, H, v_range=(-15.0, 15.0))
         return Scene(CONFIG_NAMES[1], layers, 1, cams, W, H)
 
     spec = {
@@ -278,13 +305,20 @@ def make_config(cfg: int, *, seed: int = 0, mesh_n: int | None = None, width: in
     deg = spec["deg"]
     ncoef = (deg + 1) ** 2
     shells = noise_shells(k, n, ts, seed)
-    texs = _parallel([
-        (lambda l=l: normal_texture([seed, cfg, l], ts, ts, ncoef, 0.3, np.float16, spec["op"]))
-        for l in range(k)])
-    layers = [Layer(p, uv, idx, texs[l]) for l, (p, uv, idx) in enumerate(shells)]
+    if banded:
+        texs = _parallel([(lambda l=l: banded_textures([seed, 100 + cfg, l], ts, deg)) for l in range(k)])
+        layers = [Layer(p, uv, idx, None, texs[l]) for l, (p, uv, idx) in enumerate(shells)]
+    else:
+        texs = _parallel([
+            (lambda l=l: normal_texture([seed, cfg, l], ts, ts, ncoef, 0.3, np.float16, spec["op"]))
+            for l in range(k)])
+        layers = [Layer(p, uv, idx, texs[l]) for l, (p, uv, idx) in enumerate(shells)]
     if cfg == 5:
         radius = np.where(np.arange(B) % 2 == 0, 3.0, 1.6)  # far / close-up alternate
     else:
         radius = 3.0
     cams = fibonacci_cameras(B, radius, W, H, rotate=camera_rotate)
+    if banded:
+        return Scene(CONFIG_NAMES[cfg] + " [banded u8 %d^2..%d^2]" % (ts, max(1, ts >> deg)), layers, deg, cams, W, H,
+                     v_range=(-15.0, 15.0))
     return Scene(CONFIG_NAMES[cfg], layers, deg, cams, W, H)
