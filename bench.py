@@ -101,6 +101,8 @@ def build_scene(cfg, rank, world, args):
     kw = {}
     if args.views:
         kw["num_cameras"] = args.views
+    if getattr(args, "banded", False):
+        kw["banded"] = True
     return synth.make_config(cfg, camera_rotate=vsdist.rank_camera_rotation(rank, world), **kw)
 
 
@@ -109,7 +111,7 @@ def time_oracle(sc, views, threads=0):
     t0 = time.perf_counter()
     for v in views:
         oracle.render_view(sc.layers, sc.sh_degree, sc.cameras[v], sc.width, sc.height, near_plane=sc.near_plane,
-                           t_min=sc.t_min, background=sc.background, num_threads=threads)
+                           t_min=sc.t_min, background=sc.background, num_threads=threads, v_range=sc.v_range)
     return time.perf_counter() - t0
 
 
@@ -166,8 +168,9 @@ def run_ours(args):
     cparams = binding.make_params(W, H, sc.near_plane, sc.t_min, sc.background, binding.VS_FLAG_COUNT_TEXELS | path_flag, args.chunk)
     binding.vs_render(renderer.handle, sc.cameras, cparams, out)
     cstats = renderer.stats()
-    texel_bytes = 16 * ((sc.n_coef * 4 * sc.layers[0].texture.dtype.itemsize + 15) // 16)
-    b_tex = cstats["unique_texels"] * texel_bytes
+    banded = sc.layers[0].band_textures is not None
+    texel_bytes = 0 if banded else 16 * ((sc.n_coef * 4 * sc.layers[0].texture.dtype.itemsize + 15) // 16)
+    b_tex = cstats["unique_texels"] * texel_bytes      # banded scenes: not counted (ALU-bound path, see below)
     b_geom = geometry_bytes_per_view(sc) * B
     b_fb = W * H * 16 * B
     alg_bytes_step = b_tex + b_geom + b_fb
@@ -236,6 +239,23 @@ def run_ours(args):
                 "stage_ms_per_step": {"transform": xf_ms / args.steps, "binning": bin_ms / args.steps,
                                       "raster": raster_ms / args.steps, "shade": shade_ms / args.steps}}
 
+    if banded:
+        # The banded 8-bit path is bound by the plain FP32/ALU pipes: algorithmic lane-ops per shaded
+        # fragment at degree d = 4 texels x 4(d+1)^2 byte->float conversions + as many bilinear FMAs + 4(d+1)^2 SH FMAs
+        # (576 at degree 3); peak = 148 SMs x 128 FP32 lanes x the maximum SM clock.
+        n4 = 4 * sc.n_coef
+        ops_per_frag = 4 * n4 + 4 * n4 + n4
+        frags_per_launch = cstats["shaded_fragments"] * args.steps / max(shade_launches, 1)
+        alu_achieved = frags_per_launch * ops_per_frag / (per_launch_ms * 1e-3) / 1e12 if per_launch_ms > 0 else 0.0
+        alu_peak = 148 * 128 * ((clocks or {}).get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+        roofline = {"bound": "alu", "kernel": "k_shade_banded", "achieved": alu_achieved, "peak": alu_peak, "unit": "Tlane-op/s",
+                    "frac": alu_achieved / alu_peak, "traffic": None,
+                    "peak_source": "derived: 148 SMs x 128 FP32 lanes x max SM clock (B200_PROFILING.md unit counts)",
+                    "lane_ops_per_fragment": ops_per_frag, "launch_ms": per_launch_ms,
+                    "views_per_launch": B * args.steps / max(shade_launches, 1),
+                    "kernel_share_of_step": shade_ms / (secs * 1e3),
+                    "stage_ms_per_step": roofline["stage_ms_per_step"]}
+
     cpu_baseline = None
     if world == 1 and not args.no_cpu:
         import oracle
@@ -251,13 +271,15 @@ def run_ours(args):
             "dtype": "f32", "data": "synthetic", "fps": fps,
             "config": {"workload": sc.name, "k": sc.k, "triangles_per_layer": int(sc.layers[0].indices.shape[0]),
                        "width": W, "height": H, "views_per_step": B, "sh_degree": sc.sh_degree,
-                       "texture": "%s %dx%d" % (sc.layers[0].texture.dtype, sc.layers[0].texture.shape[1], sc.layers[0].texture.shape[0]),
+                       "texture": ("uint8 banded " + " ".join("%dx%d" % (t.shape[1], t.shape[0]) for t in sc.layers[0].band_textures)
+                                   + " range [%g, %g]" % sc.v_range) if banded else
+                                  "%s %dx%d" % (sc.layers[0].texture.dtype, sc.layers[0].texture.shape[1], sc.layers[0].texture.shape[0]),
                        "raster_path": "tiled (binning + per-tile shared-memory keys)" if args.tiled
                        else "direct (triangle-parallel, 64-bit max keys in HBM/L2)",
                        "attenuation": bool(args.attenuation),
                        "parallelism": "views sharded, scene replicated (dp%d)" % world,
-                       "l2": "no flush: %.1f GiB of textures streamed per step >> 126 MB L2" % (
-                           sum(ly.texture.nbytes for ly in sc.layers) / 2 ** 30),
+                       "l2": "no flush: %.2f GiB of textures streamed per step >> 126 MB L2" % (
+                           sum(sum(t.nbytes for t in ly.band_textures) if banded else ly.texture.nbytes for ly in sc.layers) / 2 ** 30),
                        "shaded_fragments_per_view": cstats["shaded_fragments"] / B,
                        "tile_refs_per_view": cstats["tile_refs"] / B},
             "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu_baseline,
@@ -280,6 +302,7 @@ def main():
     ap.add_argument("--chunk", type=int, default=0, help="views per internal pass (0 = automatic)")
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="oracle work of the cpu_baseline sample (whole views)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--banded", action="store_true", help="the paper's 8-bit mixed-resolution textures on the same geometry (PAPER.md:L445-459; not the headline workload)")
     ap.add_argument("--attenuation", action="store_true", help="render with VS_FLAG_ATTENUATION (PAPER.md:L279-286; not the headline workload)")
     ap.add_argument("--tiled", action="store_true", help="time the per-tile raster path (VS_FLAG_TILED_PATH) instead of the default direct one")
     args = ap.parse_args()

@@ -128,6 +128,41 @@ typedef struct {
     double   ms_shade;             /*   texel fetch + SH + composite kernel                                */
 } vs_render_stats;
 
+/* The paper's own baked texture format (§4.5 "Mixed resolutions" and "Squeezing and
+ * quantization"): 8-bit images, one set per SH band, band b at its OWN resolution
+ * ("the base color is modeled at the highest resolution (2048^2), while the highest SH degree coefficients are
+ * modeled at the lowest resolution (256^2)").  A stored byte t stands for q = t/255 (q(x) = round(255 x)/255 of the
+ * squeezed coefficient); "before rendering, we re-scale value to a hyper-parameters controlled range":
+ * sh = v_min + (v_max - v_min) q, [-15, 15] in the paper.  Each band is sampled bilinearly at its own texel
+ * centres (same addressing rule as the float textures), re-scaled, and the bands are concatenated over the
+ * coefficient dimension, c = b*b .. b*b + 2b. */
+typedef struct {
+    const float*    positions;       /* as vs_layer_desc                                                  */
+    const float*    uvs;
+    uint32_t        num_vertices;
+    const uint32_t* indices;
+    uint32_t        num_triangles;
+    const uint8_t*  band_texture[4]; /* band b <= sh_degree: [band_h[b]][band_w[b]][2b+1][4] bytes; channel
+                                        0-2 = RGB, 3 = opacity; coefficient order m = -b..b; others ignored */
+    uint32_t        band_w[4], band_h[4]; /* >= 1, <= 8192                                                 */
+} vs_layer_desc_banded;
+
+typedef struct {
+    uint32_t  num_layers;            /* 1..9; layers[0] is the OUTERMOST shell                            */
+    uint32_t  sh_degree;             /* 0..3                                                               */
+    vs_memory memory;                /* where the arrays of ALL layers live                                */
+    float     v_min, v_max;          /* finite; range the bytes are re-scaled to                           */
+    const vs_layer_desc_banded* layers; /* HOST array of num_layers descriptors                            */
+} vs_scene_desc_banded;
+
+/*
+ * vs_scene_create_banded -- vs_scene_create for the banded 8-bit format.  The resulting scene is rendered
+ * with the same vs_render / vs_render_host calls (S1-S4 are identical; S5-S6 run in a kernel specialised for
+ * byte texels, k_shade_banded).  VS_FLAG_REFERENCE_PATH and the unique-texel count of VS_FLAG_COUNT_TEXELS are
+ * not available on such scenes (VS_ERR_UNSUPPORTED / shaded fragments only).
+ */
+vs_status vs_scene_create_banded(const vs_scene_desc_banded* desc, void* cuda_stream, vs_scene** out_scene);
+
 /*
  * vs_scene_create -- S0: upload / re-lay-out the baked asset once.
  *   Copies every array (the caller may free or overwrite its inputs as soon as the call returns: the

@@ -21,7 +21,7 @@ VS_FLAG_REFERENCE_PATH, VS_FLAG_KERNEL_TIMING, VS_FLAG_COUNT_TEXELS, VS_FLAG_TIL
 VS_FLAG_ATTENUATION = 16
 MISS = 0xFFFFFFFF
 
-EXPORTS = ["vs_scene_create", "vs_render", "vs_render_host", "vs_query_last_render", "vs_scene_destroy",
+EXPORTS = ["vs_scene_create", "vs_scene_create_banded", "vs_render", "vs_render_host", "vs_query_last_render", "vs_scene_destroy",
            "vs_last_error", "vs_version"]
 
 
@@ -40,6 +40,17 @@ class vs_layer_desc(C.Structure):
 class vs_scene_desc(C.Structure):
     _fields_ = [("num_layers", C.c_uint32), ("sh_degree", C.c_uint32), ("tex_dtype", C.c_int),
                 ("memory", C.c_int), ("layers", C.POINTER(vs_layer_desc))]
+
+
+class vs_layer_desc_banded(C.Structure):
+    _fields_ = [("positions", C.c_void_p), ("uvs", C.c_void_p), ("num_vertices", C.c_uint32),
+                ("indices", C.c_void_p), ("num_triangles", C.c_uint32), ("band_texture", C.c_void_p * 4),
+                ("band_w", C.c_uint32 * 4), ("band_h", C.c_uint32 * 4)]
+
+
+class vs_scene_desc_banded(C.Structure):
+    _fields_ = [("num_layers", C.c_uint32), ("sh_degree", C.c_uint32), ("memory", C.c_int),
+                ("v_min", C.c_float), ("v_max", C.c_float), ("layers", C.POINTER(vs_layer_desc_banded))]
 
 
 class vs_camera(C.Structure):
@@ -81,6 +92,8 @@ def load_library(build_if_missing: bool = True):
     L = C.CDLL(LIB_PATH)
     L.vs_scene_create.restype = C.c_int
     L.vs_scene_create.argtypes = [C.POINTER(vs_scene_desc), C.c_void_p, C.POINTER(C.c_void_p)]
+    L.vs_scene_create_banded.restype = C.c_int
+    L.vs_scene_create_banded.argtypes = [C.POINTER(vs_scene_desc_banded), C.c_void_p, C.POINTER(C.c_void_p)]
     for name in ("vs_render", "vs_render_host"):
         f = getattr(L, name)
         f.restype = C.c_int
@@ -161,6 +174,42 @@ def vs_scene_create(layers, sh_degree: int, stream=None) -> int:
     return handle.value
 
 
+def vs_scene_create_banded(layers, sh_degree: int, v_min: float, v_max: float, stream=None) -> int:
+    """The paper's banded 8-bit format: `layers` as for vs_scene_create but with .band_textures = list of
+    sh_degree + 1 uint8 arrays [H_b, W_b, 2b+1, 4] instead of .texture (all torch CUDA tensors or all numpy arrays)."""
+    L = load_library()
+    k = len(layers)
+    arr = (vs_layer_desc_banded * max(k, 1))()
+    keep = []
+    on_host = k > 0 and isinstance(layers[0].positions, np.ndarray)
+    for i, ly in enumerate(layers):
+        assert len(ly.band_textures) == sh_degree + 1
+        if on_host:
+            pos = np.ascontiguousarray(ly.positions, dtype=np.float32)
+            uv = np.ascontiguousarray(ly.uvs, dtype=np.float32)
+            idx = np.ascontiguousarray(ly.indices, dtype=np.uint32)
+            bands = [np.ascontiguousarray(t, dtype=np.uint8) for t in ly.band_textures]
+            ptr = lambda a: a.ctypes.data
+        else:
+            pos, uv, idx = ly.positions.contiguous(), ly.uvs.contiguous(), ly.indices.contiguous()
+            bands = [t.contiguous() for t in ly.band_textures]
+            assert pos.is_cuda and uv.is_cuda and idx.is_cuda and all(t.is_cuda and t.element_size() == 1 for t in bands)
+            ptr = lambda a: a.data_ptr()
+        keep += [pos, uv, idx] + bands
+        d = vs_layer_desc_banded()
+        d.positions, d.uvs, d.num_vertices = ptr(pos), ptr(uv), pos.shape[0]
+        d.indices, d.num_triangles = ptr(idx), idx.shape[0]
+        for b, t in enumerate(bands):
+            assert t.ndim == 4 and t.shape[2] == 2 * b + 1 and t.shape[3] == 4, tuple(t.shape)
+            d.band_texture[b] = ptr(t)
+            d.band_w[b], d.band_h[b] = t.shape[1], t.shape[0]
+        arr[i] = d
+    desc = vs_scene_desc_banded(k, sh_degree, VS_MEM_HOST if on_host else VS_MEM_DEVICE, float(v_min), float(v_max), arr)
+    handle = C.c_void_p()
+    _check(L.vs_scene_create_banded(C.byref(desc), _stream_ptr(stream), C.byref(handle)))
+    return handle.value
+
+
 def _cams(cameras):
     cams = np.ascontiguousarray(cameras, dtype=np.float32)
     assert cams.ndim == 2 and cams.shape[1] == 16
@@ -223,13 +272,25 @@ class Renderer:
         with torch.cuda.device(self.device):
             self.handle = None
             layers = []
+            banded = getattr(scene.layers[0], "band_textures", None) is not None
             for ly in scene.layers:
+                if banded:
+                    layers.append(types.SimpleNamespace(
+                        positions=torch.from_numpy(np.ascontiguousarray(ly.positions, dtype=np.float32)).to(self.device),
+                        uvs=torch.from_numpy(np.ascontiguousarray(ly.uvs, dtype=np.float32)).to(self.device),
+                        indices=torch.from_numpy(np.ascontiguousarray(ly.indices, dtype=np.uint32).view(np.int32)).to(self.device),
+                        band_textures=[torch.from_numpy(np.ascontiguousarray(t, dtype=np.uint8)).to(self.device)
+                                       for t in ly.band_textures]))
+                    continue
                 layers.append(types.SimpleNamespace(
                     positions=torch.from_numpy(np.ascontiguousarray(ly.positions, dtype=np.float32)).to(self.device),
                     uvs=torch.from_numpy(np.ascontiguousarray(ly.uvs, dtype=np.float32)).to(self.device),
                     indices=torch.from_numpy(np.ascontiguousarray(ly.indices, dtype=np.uint32).view(np.int32)).to(self.device),
                     texture=torch.from_numpy(np.ascontiguousarray(ly.texture)).to(self.device)))
-            self.handle = vs_scene_create(layers, scene.sh_degree)
+            if banded:
+                self.handle = vs_scene_create_banded(layers, scene.sh_degree, scene.v_range[0], scene.v_range[1])
+            else:
+                self.handle = vs_scene_create(layers, scene.sh_degree)
             del layers
             torch.cuda.empty_cache()
 

@@ -114,7 +114,9 @@ static vs_status stage_in(const void* src, size_t bytes, vs_memory mem, cudaStre
     return VS_OK;
 }
 
-static vs_status scene_create_impl(const vs_scene_desc* desc, cudaStream_t st, vs_scene* s, std::vector<void*>& temps)
+// `bd` != nullptr: banded 8-bit scene; `desc` then carries the geometry only (its texture fields are placeholders)
+static vs_status scene_create_impl(const vs_scene_desc* desc, const vs_scene_desc_banded* bd, cudaStream_t st, vs_scene* s,
+                                   std::vector<void*>& temps)
 {
     const uint32_t k = desc->num_layers;
     const uint32_t n = (desc->sh_degree + 1) * (desc->sh_degree + 1);
@@ -167,6 +169,22 @@ static vs_status scene_create_impl(const vs_scene_desc* desc, cudaStream_t st, v
         if ((r = stage_in(L.indices, (size_t)L.num_triangles * 12, desc->memory, st, temps, &idx)) != VS_OK) return r;
         CU(vs_launch_pack_tris((const uint32_t*)idx, pos + 3 * voff, L.num_triangles, L.num_vertices, (uint32_t)voff, l,
                                tris + d.tri_off[l], nrm + d.tri_off[l], flag, st));
+        if (bd) {
+            // banded 8-bit textures: one padded texel array per band
+            const vs_layer_desc_banded& BL = bd->layers[l];
+            for (uint32_t b = 0; b <= desc->sh_degree; ++b) {
+                const size_t texels = (size_t)BL.band_w[b] * BL.band_h[b];
+                unsigned char* bt;
+                if ((r = dev_alloc(s, (void**)&bt, texels * VS_BAND_STRIDE(b))) != VS_OK) return r;
+                const void* bsrc = nullptr;
+                if ((r = stage_in(BL.band_texture[b], texels * (2 * b + 1) * 4, desc->memory, st, temps, &bsrc)) != VS_OK) return r;
+                CU(vs_launch_pack_band((const unsigned char*)bsrc, (uint32_t)texels, b, bt, st));
+                d.btex[l][b] = bt; d.bw[l][b] = BL.band_w[b]; d.bh[l][b] = BL.band_h[b];
+            }
+            d.tex[l] = nullptr; d.tex_w[l] = BL.band_w[0]; d.tex_h[l] = BL.band_h[0];
+            voff += L.num_vertices;
+            continue;
+        }
         // texture -> internal layout (same element order, texel padded to a multiple of 16 bytes)
         const size_t texels = (size_t)L.tex_w * L.tex_h;
         const size_t src_bytes = texels * n * 4 * (f16 ? 2 : 4);
@@ -188,6 +206,8 @@ static vs_status scene_create_impl(const vs_scene_desc* desc, cudaStream_t st, v
     if (hflag & 1u) return fail(VS_ERR_INVALID_ARG, "a triangle index is >= num_vertices of its layer");
     if (hflag & 2u) return fail(VS_ERR_INVALID_ARG, "a vertex position or uv is not finite");
     d.positions = pos; d.uvs = uvs; d.tris = tris; d.tri_nrm = nrm;
+    d.banded = bd ? 1u : 0u;
+    if (bd) { d.v_min = bd->v_min; d.v_scale = (bd->v_max - bd->v_min) / 255.0f; }
     CU(cudaHostAlloc((void**)&s->host_counters, VS_CNT_N * 8, cudaHostAllocDefault));
     CU(cudaStreamCreateWithFlags(&s->copy_stream, cudaStreamNonBlocking));
     for (int i = 0; i < 2; ++i) {
@@ -216,7 +236,54 @@ extern "C" vs_status vs_scene_create(const vs_scene_desc* desc, void* cuda_strea
     if (!s) return fail(VS_ERR_OUT_OF_MEMORY, "host allocation failed");
     cudaGetDevice(&s->device);
     std::vector<void*> temps;
-    vs_status r = scene_create_impl(desc, (cudaStream_t)cuda_stream, s, temps);
+    vs_status r = scene_create_impl(desc, nullptr, (cudaStream_t)cuda_stream, s, temps);
+    cudaStreamSynchronize((cudaStream_t)cuda_stream);
+    for (void* p : temps) cudaFree(p);
+    if (r != VS_OK) {
+        delete s;
+        cudaGetLastError();
+        return r;
+    }
+    *out_scene = s;
+    return VS_OK;
+}
+
+extern "C" vs_status vs_scene_create_banded(const vs_scene_desc_banded* bd, void* cuda_stream, vs_scene** out_scene)
+{
+    g_err[0] = 0;
+    if (out_scene) *out_scene = nullptr;
+    if (!bd || !out_scene) return fail(VS_ERR_INVALID_ARG, "NULL argument");
+    if (bd->num_layers < 1 || bd->num_layers > VS_MAX_LAYERS) return fail(VS_ERR_INVALID_ARG, "num_layers must be 1..9");
+    if (bd->sh_degree > 3) return fail(VS_ERR_INVALID_ARG, "sh_degree must be 0..3");
+    if (bd->memory != VS_MEM_DEVICE && bd->memory != VS_MEM_HOST) return fail(VS_ERR_INVALID_ARG, "bad memory kind");
+    if (!bd->layers) return fail(VS_ERR_INVALID_ARG, "NULL layers");
+    if (!std::isfinite(bd->v_min) || !std::isfinite(bd->v_max)) return fail(VS_ERR_INVALID_ARG, "v_min / v_max not finite");
+    // geometry through the common path: a float descriptor whose texture fields are placeholders
+    std::vector<vs_layer_desc> geo(bd->num_layers);
+    for (uint32_t l = 0; l < bd->num_layers; ++l) {
+        const vs_layer_desc_banded& B = bd->layers[l];
+        for (uint32_t b = 0; b <= bd->sh_degree; ++b) {
+            if (!B.band_texture[b]) return fail(VS_ERR_INVALID_ARG, "layer %u: band %u texture is NULL", l, b);
+            if (B.band_w[b] == 0 || B.band_h[b] == 0) return fail(VS_ERR_INVALID_ARG, "layer %u: band %u is empty", l, b);
+            if (B.band_w[b] > 8192 || B.band_h[b] > 8192) return fail(VS_ERR_UNSUPPORTED, "layer %u: band %u larger than 8192", l, b);
+        }
+        geo[l].positions = B.positions; geo[l].uvs = B.uvs; geo[l].num_vertices = B.num_vertices;
+        geo[l].indices = B.indices; geo[l].num_triangles = B.num_triangles;
+        geo[l].texture = B.band_texture[0]; geo[l].tex_w = 1; geo[l].tex_h = 1;
+    }
+    vs_scene_desc desc;
+    desc.num_layers = bd->num_layers; desc.sh_degree = bd->sh_degree; desc.tex_dtype = VS_F32; desc.memory = bd->memory;
+    desc.layers = geo.data();
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        cudaGetLastError();
+        return fail(VS_ERR_CUDA, "no CUDA device available (this library has no CPU fallback)");
+    }
+    vs_scene* s = new (std::nothrow) vs_scene();
+    if (!s) return fail(VS_ERR_OUT_OF_MEMORY, "host allocation failed");
+    cudaGetDevice(&s->device);
+    std::vector<void*> temps;
+    vs_status r = scene_create_impl(&desc, bd, (cudaStream_t)cuda_stream, s, temps);
     cudaStreamSynchronize((cudaStream_t)cuda_stream);
     for (void* p : temps) cudaFree(p);
     if (r != VS_OK) {
@@ -238,6 +305,8 @@ static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, u
     if (!(p->t_min >= 0.0f) || !std::isfinite(p->t_min)) return fail(VS_ERR_INVALID_ARG, "t_min must be >= 0");
     if (p->flags & ~(uint32_t)(VS_FLAG_REFERENCE_PATH | VS_FLAG_KERNEL_TIMING | VS_FLAG_COUNT_TEXELS | VS_FLAG_TILED_PATH | VS_FLAG_ATTENUATION))
         return fail(VS_ERR_INVALID_ARG, "reserved flag bits set");
+    if (scene->dev.banded && (p->flags & VS_FLAG_REFERENCE_PATH))
+        return fail(VS_ERR_UNSUPPORTED, "VS_FLAG_REFERENCE_PATH is not available on banded scenes");
     for (int i = 0; i < 3; ++i)
         if (!std::isfinite(p->background[i])) return fail(VS_ERR_INVALID_ARG, "background not finite");
     for (uint32_t c = 0; c < n; ++c) {
@@ -358,7 +427,9 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
         CU(cudaMemsetAsync(ch.tile_count, 0, ntile * 4, st));
         CU(cudaMemsetAsync(ch.tile_cursor, 0, ntile * 4, st));
     }
-    if (p->flags & VS_FLAG_COUNT_TEXELS) {
+    if ((p->flags & VS_FLAG_COUNT_TEXELS) && s->dev.banded) {
+        ch.count_fragments = 1;   // banded scenes: shaded fragments only (no unique-texel bitmap)
+    } else if (p->flags & VS_FLAG_COUNT_TEXELS) {
         const size_t words = (size_t)views * (s->dev.tex_bit_off[s->dev.k] >> 5);
         CU(s->texel_bits.reserve(words * 4 + 16));
         CU(cudaMemsetAsync(s->texel_bits.p, 0, words * 4, st));
@@ -379,7 +450,7 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
         CU(vs_launch_raster_direct(s->dev, fr, ch, st));
         if ((r = span_end(s, timing, st)) != VS_OK) return r;
         if ((r = span_begin(s, timing, 3, st)) != VS_OK) return r;
-        CU(vs_launch_shade(s->dev, s->tex_f16, fr, ch, st));
+        CU(s->dev.banded ? vs_launch_shade_banded(s->dev, fr, ch, st) : vs_launch_shade(s->dev, s->tex_f16, fr, ch, st));
         if ((r = span_end(s, timing, st)) != VS_OK) return r;
         s->keys_dirty = false;
         s->launches += (s->dev.t_total ? 2 : 0) + 1;
@@ -403,7 +474,7 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
     CU(vs_launch_raster(s->dev, fr, ch, st));
     if ((r = span_end(s, timing, st)) != VS_OK) return r;
     if ((r = span_begin(s, timing, 3, st)) != VS_OK) return r;
-    CU(vs_launch_shade(s->dev, s->tex_f16, fr, ch, st));
+    CU(s->dev.banded ? vs_launch_shade_banded(s->dev, fr, ch, st) : vs_launch_shade(s->dev, s->tex_f16, fr, ch, st));
     if ((r = span_end(s, timing, st)) != VS_OK) return r;
     s->launches += (s->dev.t_total ? 3 : 1) + 2;
     s->raster_launches += 1;

@@ -29,7 +29,14 @@ struct VsSceneDev {
     const uint4* tex[VS_MAX_LAYERS];      // [tex_h][tex_w][texel_vecs] 16-byte vectors
     uint32_t tex_w[VS_MAX_LAYERS], tex_h[VS_MAX_LAYERS];
     uint32_t tex_bit_off[VS_MAX_LAYERS + 1];  // VS_FLAG_COUNT_TEXELS: first bitmap bit of each layer (multiple of 32)
+    // banded 8-bit scenes (vs_scene_create_banded): band b of layer l is [bh][bw] texels of
+    // VS_BAND_STRIDE(b) = {4, 16, 32, 32} bytes holding its (2b+1) x 4 bytes in API order, zero padded
+    uint32_t banded;
+    float v_min, v_scale;                      // sh = v_min + v_scale * byte, v_scale = (v_max - v_min) / 255
+    const unsigned char* btex[VS_MAX_LAYERS][4];
+    uint32_t bw[VS_MAX_LAYERS][4], bh[VS_MAX_LAYERS][4];
 };
+#define VS_BAND_STRIDE(b) ((b) == 0 ? 4u : (b) == 1 ? 16u : 32u)
 
 struct VsCamDev {  // == vs_camera
     float fx, fy, cx, cy;
@@ -253,6 +260,7 @@ struct VsChunk {                 // one pass over `views` cameras
     int ids_is_output;           // ids is the caller's AOV: empty tiles must be filled with MISS too
     float* out_rgba;             // DEVICE [views][H][W][4]
     uint32_t* texel_bits;        // DEVICE [views][tex_bit_off[k] / 32] or nullptr (VS_FLAG_COUNT_TEXELS)
+    int count_fragments;         // banded scenes under VS_FLAG_COUNT_TEXELS: count shaded fragments only
     // direct (untiled) path: non-null keys selects it in vs_launch_shade
     unsigned long long* keys;    // DEVICE [views][k][H][W] max keys, zero between passes
     uint2* big_list;             // DEVICE [big_capacity] {view, global triangle} with very large boxes
@@ -274,6 +282,8 @@ cudaError_t vs_launch_reference(const VsSceneDev& sc, int tex_f16, const VsFrame
 // scene construction helpers
 cudaError_t vs_launch_pack_tris(const uint32_t* indices, const float* layer_positions, uint32_t num_tris, uint32_t num_vertices,
                                 uint32_t vtx_off, uint32_t layer, uint4* out, float4* out_normals, uint32_t* error_flag, cudaStream_t st);
+cudaError_t vs_launch_pack_band(const unsigned char* src, uint32_t n_texels, uint32_t band, unsigned char* dst, cudaStream_t st);
+cudaError_t vs_launch_shade_banded(const VsSceneDev& sc, const VsFrame& fr, const struct VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_check_finite(const float* v, size_t n, uint32_t* error_flag, cudaStream_t st);
 cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, uint32_t n_coef, uint32_t np_pad,
                                    uint4* dst, cudaStream_t st);

@@ -46,6 +46,24 @@ __global__ void k_pack_texture(const T* __restrict__ src, uint32_t n_texels, uin
     }
 }
 
+// banded 8-bit textures: API texel of (2b+1) x 4 bytes -> internal texel of VS_BAND_STRIDE(b) bytes, zero padded
+__global__ void k_pack_band(const unsigned char* __restrict__ src, uint32_t n_texels, uint32_t src_stride, uint32_t dst_stride,
+                            unsigned char* __restrict__ dst)
+{
+    const size_t total = (size_t)n_texels * dst_stride;
+    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (size_t)gridDim.x * blockDim.x) {
+        const size_t texel = i / dst_stride;
+        const uint32_t e = (uint32_t)(i - texel * dst_stride);
+        dst[i] = e < src_stride ? src[texel * src_stride + e] : (unsigned char)0;
+    }
+}
+
+cudaError_t vs_launch_pack_band(const unsigned char* src, uint32_t n_texels, uint32_t band, unsigned char* dst, cudaStream_t st)
+{
+    k_pack_band<<<148 * 8, 256, 0, st>>>(src, n_texels, (2 * band + 1) * 4, VS_BAND_STRIDE(band), dst);
+    return cudaGetLastError();
+}
+
 cudaError_t vs_launch_pack_tris(const uint32_t* indices, const float* layer_positions, uint32_t num_tris, uint32_t num_vertices,
                                 uint32_t vtx_off, uint32_t layer, uint4* out, float4* out_normals, uint32_t* error_flag, cudaStream_t st)
 {

@@ -1,0 +1,189 @@
+// vs_kernels_shade_banded.cu -- S5-S7 for the paper's banded 8-bit texture format (§4.5 "Mixed
+// resolutions" / "Squeezing and quantization").
+//
+// A fragment reads, per SH band b, the 2x2 footprint of THAT band's image (its own resolution): 4, 12, 20, 28 bytes per
+// texel (padded to 4, 16, 32, 32), 64 coefficient bytes per texel set instead of the 128 of the fp16 format, and the
+// higher bands touch 4-64x fewer distinct texels.  The byte textures of a whole C4 scene (315 MB) nearly fit the L2,
+// so this path is bound by the plain FP32/ALU pipes, not by HBM: ~580 lane-ops per fragment (256 byte->float
+// conversions, 256 bilinear FMAs, 64 SH FMAs).  There is no reason for the octet mapping of k_shade (which exists to
+// form 128-byte line requests): one lane = one pixel, all layers composited in registers, no shared memory.
+//
+//   s_ch = sum_b sum_m Y_{b,m} (v_min + v_scale * bilinear_b(t)[m][ch]) = v_min sum_c Y_c + v_scale sum_c Y_c blend_c[ch]
+//
+// bytes -> float: PRMT of the byte into the mantissa of 2^23 (0x4B000000), then one FADD of -2^23 (exact).
+#include "vs_common.cuh"
+
+template <int SEL>
+__device__ __forceinline__ float vs_byte_f32(uint32_t w)
+{
+    return __uint_as_float(__byte_perm(w, 0x4B000000u, 0x7540 + SEL)) - 8388608.0f;
+}
+
+// one 4-byte word = the 4 channels of one coefficient of one texel; Z = bilinear weight x SH basis value x v_scale
+__device__ __forceinline__ void vs_acc_word(uint32_t w, float Z, float& s0, float& s1, float& s2, float& s3)
+{
+    s0 = fmaf(Z, vs_byte_f32<0>(w), s0);
+    s1 = fmaf(Z, vs_byte_f32<1>(w), s1);
+    s2 = fmaf(Z, vs_byte_f32<2>(w), s2);
+    s3 = fmaf(Z, vs_byte_f32<3>(w), s3);
+}
+
+// perspective-correct UV of the winning triangle at the pixel, as base + offset
+__device__ __forceinline__ void vs_fragment_uv(const VsSceneDev& sc, const int4* __restrict__ vv, const uint4 tri, int px, int py,
+                                               float& u0, float& du, float& v0, float& dv)
+{
+    const int4 a = __ldg(&vv[tri.x]), b = __ldg(&vv[tri.y]), c = __ldg(&vv[tri.z]);
+    const float2 uva = __ldg(&sc.uvs[tri.x]), uvb = __ldg(&sc.uvs[tri.y]), uvc = __ldg(&sc.uvs[tri.z]);
+    VsTri T;
+    vs_setup_tri(a, b, c, T);
+    const float2 uv1 = T.swapped ? uvc : uvb, uv2 = T.swapped ? uvb : uvc;
+    VsEdges e;
+    vs_edges_at(T, px, py, e);
+    const float g0 = __ll2float_rn(e.E0) * T.q0, g1 = __ll2float_rn(e.E1) * T.q1, g2 = __ll2float_rn(e.E2) * T.q2;
+    const float inv = __fdividef(1.0f, g0 + g1 + g2);
+    const float b1 = g1 * inv, b2 = g2 * inv;
+    u0 = uva.x; du = b1 * (uv1.x - uva.x) + b2 * (uv2.x - uva.x);
+    v0 = uva.y; dv = b1 * (uv1.y - uva.y) + b2 * (uv2.y - uva.y);
+}
+
+// band B of one fragment: 2x2 footprint at the band's own resolution, accumulated into the four channel sums
+template <int B>
+__device__ __forceinline__ void vs_band(const VsSceneDev& sc, uint32_t l, float u0, float du, float v0, float dv, const float* Y,
+                                        float& s0, float& s1, float& s2, float& s3)
+{
+    constexpr int NB = 2 * B + 1;                 // coefficients = 4-byte words of this band
+    constexpr uint32_t STRIDE = VS_BAND_STRIDE(B);
+    const int Wb = (int)sc.bw[l][B], Hb = (int)sc.bh[l][B];
+    uint32_t cx0, cx1, cy0, cy1;
+    float fa, fb;
+    vs_texel_coord(u0, du, (float)Wb, Wb, cx0, cx1, fa);
+    vs_texel_coord(v0, dv, (float)Hb, Hb, cy0, cy1, fb);
+    const unsigned char* base = sc.btex[l][B];
+    const uint32_t o[4] = {(cy0 * (uint32_t)Wb + cx0) * STRIDE, (cy0 * (uint32_t)Wb + cx1) * STRIDE,
+                           (cy1 * (uint32_t)Wb + cx0) * STRIDE, (cy1 * (uint32_t)Wb + cx1) * STRIDE};
+    const float wq[4] = {(1.0f - fa) * (1.0f - fb) * sc.v_scale, fa * (1.0f - fb) * sc.v_scale,
+                         (1.0f - fa) * fb * sc.v_scale, fa * fb * sc.v_scale};
+    uint32_t w[4][NB <= 1 ? 1 : (NB <= 4 ? 4 : 8)];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) {
+        if (B == 0) {
+            w[q][0] = __ldg(reinterpret_cast<const uint32_t*>(base + o[q]));
+        } else {
+            const uint4 t0 = __ldg(reinterpret_cast<const uint4*>(base + o[q]));
+            w[q][0] = t0.x; w[q][1] = t0.y; w[q][2] = t0.z; w[q][3] = t0.w;
+            if (B >= 2) {
+                const uint4 t1 = __ldg(reinterpret_cast<const uint4*>(base + o[q]) + 1);
+                w[q][4] = t1.x; w[q][5] = t1.y; w[q][6] = t1.z; w[q][7] = t1.w;
+            }
+        }
+    }
+#pragma unroll
+    for (int m = 0; m < NB; ++m) {
+        const float y = Y[B * B + m];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) vs_acc_word(w[q][m], wq[q] * y, s0, s1, s2, s3);
+    }
+}
+
+template <int DEG, bool COUNT>
+__global__ void __launch_bounds__(256, 2)
+k_shade_banded(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams, const int4* __restrict__ vtx,
+               const uint32_t* __restrict__ tile_off, const uint32_t* __restrict__ ids, unsigned long long* __restrict__ keys,
+               uint32_t* __restrict__ out_ids, float* __restrict__ out_rgba, unsigned long long* __restrict__ counters)
+{
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t tile = blockIdx.x, view = blockIdx.y;
+    const uint32_t tiles = fr.tiles_x * fr.tiles_y;
+    const int W = (int)fr.width, H = (int)fr.height;
+    const int lx = (int)(warp & 1) * 8 + (int)(lane & 7), ly = (int)(warp >> 1) * 4 + (int)(lane >> 3);
+    const int px = (int)(tile % fr.tiles_x) * VS_TILE_W + lx, py = (int)(tile / fr.tiles_x) * VS_TILE_H + ly;
+    const bool inimg = px < W && py < H;
+    const size_t pix = ((size_t)view * H + py) * W + px;
+    const size_t plane = (size_t)W * H;
+    const size_t pix0 = (size_t)view * sc.k * plane + (size_t)py * W + px;
+
+    // tiled path: tile_off = reference list offsets; direct path: tile_off = per-tile masks of the layers drawn into
+    const uint32_t lmask = keys ? tile_off[view * tiles + tile] : 0xFFFFFFFFu;
+    if (keys ? lmask == 0u : tile_off[view * tiles + tile] == tile_off[view * tiles + tile + 1]) {
+        if (out_ids && inimg)
+            for (uint32_t l = 0; l < sc.k; ++l) out_ids[pix0 + (size_t)l * plane] = VS_MISS;
+        if (inimg) reinterpret_cast<float4*>(out_rgba)[pix] = make_float4(fr.bg[0], fr.bg[1], fr.bg[2], 0.0f);
+        return;
+    }
+    const int4* __restrict__ vv = vtx + (size_t)view * sc.v_total;
+
+    float Y[16];
+#pragma unroll
+    for (int c = 0; c < 16; ++c) Y[c] = 0.0f;
+    float vx, vy, vz;
+    vs_view_dir(cams[view], px, py, vx, vy, vz);
+    vs_sh_basis<DEG>(vx, vy, vz, Y);
+    float ysum = 0.0f;
+#pragma unroll
+    for (int c = 0; c < (DEG + 1) * (DEG + 1); ++c) ysum += Y[c];
+    const float sbase = sc.v_min * ysum;          // v_min sum_c Y_c: the constant part of every channel's logit
+
+    float Tr = 1.0f, Cr = 0.0f, Cg = 0.0f, Cb = 0.0f;
+    bool alive = true;
+    unsigned nfrag = 0;
+    for (uint32_t l = 0; l < sc.k; ++l) {
+        uint32_t id = VS_MISS;
+        if (keys) {
+            // direct path: the key image of k_raster_direct; what is read is cleared for the next pass over this buffer
+            if (inimg && ((lmask >> l) & 1u)) {
+                const unsigned long long key = keys[pix0 + (size_t)l * plane];
+                if (key) { id = 0xFFFFFFFFu - (uint32_t)key; keys[pix0 + (size_t)l * plane] = 0ull; }
+            }
+            if (out_ids && inimg) out_ids[pix0 + (size_t)l * plane] = id;
+        } else if (inimg) {
+            id = __ldg(ids + pix0 + (size_t)l * plane);
+        }
+        if (id == VS_MISS || !alive) continue;
+        const uint4 tri = __ldg(&sc.tris[sc.tri_off[l] + id]);
+        float u0, du, v0, dv;
+        vs_fragment_uv(sc, vv, tri, px, py, u0, du, v0, dv);
+        float s0 = sbase, s1 = sbase, s2 = sbase, s3 = sbase;
+        vs_band<0>(sc, l, u0, du, v0, dv, Y, s0, s1, s2, s3);
+        if (DEG >= 1) vs_band<1>(sc, l, u0, du, v0, dv, Y, s0, s1, s2, s3);
+        if (DEG >= 2) vs_band<2>(sc, l, u0, du, v0, dv, Y, s0, s1, s2, s3);
+        if (DEG >= 3) vs_band<3>(sc, l, u0, du, v0, dv, Y, s0, s1, s2, s3);
+        if (COUNT) ++nfrag;
+        float A = vs_sigmoid(s3);
+        if (fr.attenuate) A *= vs_alpha_w(vx, vy, vz, __ldg(&sc.tri_nrm[sc.tri_off[l] + id]));
+        const float TA = Tr * A;
+        Cr += TA * vs_sigmoid(s0); Cg += TA * vs_sigmoid(s1); Cb += TA * vs_sigmoid(s2);
+        Tr *= (1.0f - A);
+        if (Tr < fr.t_min) alive = false;
+    }
+    if (COUNT) {
+        for (int o = 16; o > 0; o >>= 1) nfrag += __shfl_xor_sync(0xFFFFFFFFu, nfrag, o);
+        if (lane == 0 && nfrag) atomicAdd(&counters[VS_CNT_FRAGS], (unsigned long long)nfrag);
+    }
+    if (inimg)
+        reinterpret_cast<float4*>(out_rgba)[pix] = make_float4(Cr + Tr * fr.bg[0], Cg + Tr * fr.bg[1], Cb + Tr * fr.bg[2], 1.0f - Tr);
+}
+
+template <int DEG, bool COUNT>
+static cudaError_t launch_b(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
+{
+    dim3 grid(fr.tiles_x * fr.tiles_y, ch.views);
+    auto kern = k_shade_banded<DEG, COUNT>;
+    if (ch.keys)
+        kern<<<grid, 256, 0, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_mask, nullptr, ch.keys, ch.ids_is_output ? ch.ids : nullptr,
+                                   ch.out_rgba, ch.counters);
+    else
+        kern<<<grid, 256, 0, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_off, ch.ids, nullptr, nullptr, ch.out_rgba, ch.counters);
+    return cudaGetLastError();
+}
+
+cudaError_t vs_launch_shade_banded(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
+{
+    const bool cnt = ch.count_fragments != 0;
+    switch (sc.sh_degree) {
+        case 0: return cnt ? launch_b<0, true>(sc, fr, ch, st) : launch_b<0, false>(sc, fr, ch, st);
+        case 1: return cnt ? launch_b<1, true>(sc, fr, ch, st) : launch_b<1, false>(sc, fr, ch, st);
+        case 2: return cnt ? launch_b<2, true>(sc, fr, ch, st) : launch_b<2, false>(sc, fr, ch, st);
+        case 3: return cnt ? launch_b<3, true>(sc, fr, ch, st) : launch_b<3, false>(sc, fr, ch, st);
+    }
+    return cudaErrorInvalidValue;
+}

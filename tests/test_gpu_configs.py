@@ -111,6 +111,33 @@ def test_config4_full_attenuation(env):
     print("C4 full size, attenuated: worst rgba err %.3e" % worst)
 
 
+def test_config4_full_banded(env):
+    """SURVEY.md §8(f) NEXT-1 at the headline size: C4 geometry and cameras with the paper's banded 8-bit textures
+    (2048^2 .. 256^2 per band), whole batch in one call as bench.py --banded times it; two views
+    against the oracle, ids bit-exact."""
+    b, torch = env.binding, env.torch
+    sc = env.synth.make_config(4, banded=True)
+    B, W, H = len(sc.cameras), sc.width, sc.height
+    r = b.Renderer(sc)
+    p = b.make_params(W, H, sc.near_plane, sc.t_min, sc.background)
+    out = torch.empty((B, H, W, 4), dtype=torch.float32, device="cuda")
+    b.vs_render(r.handle, sc.cameras, p, out)
+    torch.cuda.synchronize()
+    assert r.stats()["dropped_triangles"] == 0
+    worst = 0.0
+    for v in (0, 63):
+        rgba, ids = r.render(sc.cameras[[v]], p, want_ids=True)
+        torch.cuda.synchronize()
+        assert np.array_equal(rgba.cpu().numpy()[0], out[v].cpu().numpy())
+        ref = env.oracle.render_scene(sc, [v])[0]
+        assert np.array_equal(ids.cpu().numpy().view(np.uint32)[0], ref["ids"])
+        err = float(np.abs(rgba.cpu().numpy()[0].astype(np.float64) - ref["rgba"]).max())
+        worst = max(worst, err)
+        assert err <= TOL, "C4 banded, view %d: max abs rgba error %.3e" % (v, err)
+    r.close()
+    print("C4 full size, banded: worst rgba err %.3e" % worst)
+
+
 def test_config5_full(env):
     # even views are far cameras (r = 3), odd views close-ups (r = 1.6) that fill the frame
     _check_config(env, 5, [0, 1, 15], [0, 1])

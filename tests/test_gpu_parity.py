@@ -125,6 +125,63 @@ def test_attenuation_degenerate_and_big_triangles(env):
     check_against_oracle(env, sc, [0], attenuation=True)
 
 
+# ---- the paper's banded 8-bit mixed-resolution textures ----
+def test_banded_config1(env):
+    sc = env.synth.make_config(1, banded=True)
+    worst, rgba, ids = check_against_oracle(env, sc, range(4))
+    assert (ids != env.binding.MISS).mean() > 0.5
+    # same geometry as the float C1: identical coverage
+    plain = gpu_render(env, env.synth.make_config(1), range(4))
+    assert np.array_equal(plain[1], ids)
+    print("C1 banded worst rgba err %.3e" % worst)
+
+
+@pytest.mark.parametrize("cfg,kw", [
+    (2, dict(mesh_n=40, width=333, height=250, tex_size=256, num_cameras=4)),          # deg 2, ragged tiles
+    (4, dict(mesh_n=64, width=480, height=270, tex_size=512, num_cameras=5, k=9)),     # deg 3, k = 9, bands 512..64
+    (5, dict(mesh_n=120, width=384, height=216, tex_size=512, num_cameras=4, k=9)),    # sub-pixel tris + close-ups
+])
+def test_banded_reduced_configs(env, cfg, kw):
+    sc = env.synth.make_config(cfg, banded=True, **kw)
+    worst, _, ids = check_against_oracle(env, sc, range(len(sc.cameras)), views_per_chunk=2)
+    check_against_oracle(env, sc, [1], attenuation=True, t_min=2.0 ** -6, background=(0.3, 0.1, 0.2))
+    print("C%d reduced, banded: worst rgba err %.3e, coverage %.2f" % (cfg, worst, (ids != env.binding.MISS).mean()))
+
+
+@pytest.mark.parametrize("deg", [0, 1, 2, 3])
+def test_banded_formats_and_odd_sizes(env, deg):
+    """Every degree; bands of unrelated, non-square sizes (incl. 1x1), full-range white-noise bytes, a range other than
+    the paper's [-15, 15]."""
+    rng = np.random.default_rng(11 + deg)
+    sc = env.synth.make_config(1, width=96, height=80, num_cameras=2, banded=True)
+    sizes = [(48, 64), (7, 5), (1, 1), (33, 2)]
+    for ly in sc.layers:
+        ly.band_textures = [rng.integers(0, 256, size=(sizes[b][0], sizes[b][1], 2 * b + 1, 4), dtype=np.uint8)
+                            for b in range(deg + 1)]
+    sc.sh_degree = deg
+    sc.v_range = (-3.0, 2.0)
+    check_against_oracle(env, sc, [0, 1])
+
+
+def test_banded_host_descriptors_and_errors(env):
+    b, torch = env.binding, env.torch
+    sc = env.synth.make_config(2, mesh_n=24, width=160, height=120, tex_size=64, num_cameras=3, banded=True)
+    dev_rgba, dev_ids, _ = gpu_render(env, sc, range(3))
+    h = b.vs_scene_create_banded(sc.layers, sc.sh_degree, *sc.v_range)        # numpy arrays: VS_MEM_HOST
+    out = torch.empty((3, 120, 160, 4), dtype=torch.float32).pin_memory()
+    ids = torch.empty((3, sc.k, 120, 160), dtype=torch.int32).pin_memory()
+    b.vs_render_host(h, sc.cameras, b.make_params(160, 120, flags=env.path_flags), out, ids)
+    assert np.array_equal(out.numpy(), dev_rgba) and np.array_equal(ids.numpy().view(np.uint32), dev_ids)
+    dout = torch.empty((3, 120, 160, 4), dtype=torch.float32, device="cuda")
+    with pytest.raises(b.VsError) as e:                                          # no brute-force kernel for this format
+        b.vs_render(h, sc.cameras, b.make_params(160, 120, flags=b.VS_FLAG_REFERENCE_PATH), dout)
+    assert e.value.status == b.VS_ERR_UNSUPPORTED
+    b.vs_scene_destroy(h)
+    with pytest.raises(b.VsError) as e:
+        b.vs_scene_create_banded(sc.layers, sc.sh_degree, float("nan"), 15.0)
+    assert e.value.status == b.VS_ERR_INVALID_ARG
+
+
 def test_determinism_and_chunking(env):
     sc = env.synth.make_config(2, mesh_n=30, width=200, height=150, tex_size=128, num_cameras=6)
     a = gpu_render(env, sc, range(6), views_per_chunk=1)
