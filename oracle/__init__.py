@@ -38,12 +38,12 @@ def lib():
         L.vso_render.argtypes = [C.POINTER(_Layer), C.c_uint32, C.c_uint32, C.c_int, C.c_void_p,
                                  C.c_uint32, C.c_uint32, C.c_float, C.c_double, C.c_void_p,
                                  C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
-                                 C.c_void_p, C.c_int, C.c_int]
+                                 C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.vso_render_banded.restype = C.c_int
         L.vso_render_banded.argtypes = [C.POINTER(_Layer), C.POINTER(_Bands), C.c_double, C.c_double, C.c_uint32, C.c_uint32,
                                         C.c_void_p, C.c_uint32, C.c_uint32, C.c_float, C.c_double, C.c_void_p,
                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
-                                        C.c_void_p, C.c_int, C.c_int]
+                                        C.c_void_p, C.c_int, C.c_int, C.c_void_p]
         L.vso_quantize.restype = C.c_double
         L.vso_quantize.argtypes = [C.c_double]
         L.vso_rescale.restype = C.c_double
@@ -85,7 +85,7 @@ def max_threads() -> int:
 def render_view(layers, sh_degree: int, camera, width: int, height: int, *, near_plane: float = 0.05,
                 t_min: float = 2.0 ** -14, background=(0.0, 0.0, 0.0), num_threads: int = 0,
                 want_qp: bool = False, want_layer_rgba: bool = False, want_layer_uv: bool = False,
-                attenuation: bool = False, v_range=None):
+                attenuation: bool = False, v_range=None, want_layer_normal: bool = False):
     """Render one view.  `layers`: objects with positions/uvs/indices/texture numpy arrays
     (outermost first); layers with a `band_textures` list (uint8 [h_b, w_b, 2b+1, 4] per SH band) are
     rendered in the paper's banded 8-bit format, re-scaled to `v_range` = (v_min, v_max).
@@ -132,10 +132,11 @@ def render_view(layers, sh_degree: int, camera, width: int, height: int, *, near
     qp = np.empty((k, height, width), dtype=np.float32) if want_qp else None
     lrgba = np.empty((k, height, width, 4), dtype=np.float64) if want_layer_rgba else None
     luv = np.empty((k, height, width, 2), dtype=np.float64) if want_layer_uv else None
+    lnrm = np.empty((k, height, width, 3), dtype=np.float64) if want_layer_normal else None
     stats = np.zeros(2, dtype=np.uint64)
     tail = (_ptr(rgba), _ptr(ids), _ptr(qp) if want_qp else None,
             _ptr(lrgba) if want_layer_rgba else None, _ptr(luv) if want_layer_uv else None,
-            _ptr(stats), num_threads, 1 if attenuation else 0)
+            _ptr(stats), num_threads, 1 if attenuation else 0, _ptr(lnrm) if want_layer_normal else None)
     if banded:
         rc = lib().vso_render_banded(arr, bands, float(v_range[0]), float(v_range[1]), k, sh_degree, _ptr(cam), width,
                                      height, near_plane, t_min, _ptr(bg), *tail)
@@ -150,6 +151,8 @@ def render_view(layers, sh_degree: int, camera, width: int, height: int, *, near
         out["layer_rgba"] = lrgba
     if want_layer_uv:
         out["layer_uv"] = luv
+    if want_layer_normal:
+        out["layer_normal"] = lnrm
     return out
 
 

@@ -317,6 +317,8 @@ static void view_dir(const float* cam, int px, int py, double* v)
  *   out_layer_rgba [k][H][W][4] double, decoded per-layer RGBA, 0 on miss            (optional)
  *   out_layer_uv   [k][H][W][2] double, interpolated UV, 0 on miss                   (optional)
  *   stats[0] += triangles dropped (near plane / guard band), stats[1] += zero-area triangles
+ *   out_layer_normal [k][H][W][3] double, unit face normal of the winning fragment's triangle (world space), signed so that
+ *                   it faces the viewer (v . n <= 0), 0 on miss or zero-area triangles                  (optional, last argument)
  *   attenuate != 0: every fragment's opacity is multiplied by alpha_w(v, face normal) before blending
  *                   (PAPER.md:L279-286); the alpha of out_layer_rgba is the attenuated one
  * Returns 0, or -1 on bad arguments / allocation failure.
@@ -325,7 +327,7 @@ static int render_impl(const vso_layer* layers, const vso_bands* btex, double v_
                        uint32_t sh_degree, int tex_dtype, const float* cam,
                        uint32_t width, uint32_t height, float near_plane, double t_min, const double* bg,
                        double* out_rgba, uint32_t* out_ids, float* out_qp, double* out_layer_rgba,
-                       double* out_layer_uv, uint64_t* stats, int num_threads, int attenuate)
+                       double* out_layer_uv, uint64_t* stats, int num_threads, int attenuate, double* out_layer_normal)
 {
     if (!layers || k < 1 || k > VSO_MAX_LAYERS || sh_degree > 3 || !cam || !out_rgba || !out_ids || !(near_plane > 0.0f))
         return -1;
@@ -406,6 +408,7 @@ static int render_impl(const vso_layer* layers, const vso_bands* btex, double v_
         }
     if (out_layer_rgba) memset(out_layer_rgba, 0, sizeof(double) * P * k * 4);
     if (out_layer_uv) memset(out_layer_uv, 0, sizeof(double) * P * k * 2);
+    if (out_layer_normal) memset(out_layer_normal, 0, sizeof(double) * P * k * 3);
 
     /* S5-S7: shade and composite, per pixel, in double */
 #pragma omp parallel for num_threads(num_threads) schedule(dynamic, 4)
@@ -439,12 +442,16 @@ static int render_impl(const vso_layer* layers, const vso_bands* btex, double v_
                 if (btex) vso_sample_banded(&btex[l], sh_degree, v_min, v_max, uu, vv, coef);
                 else vso_sample_bilinear(L->texture, tex_dtype, L->tex_w, L->tex_h, n, uu, vv, coef);
                 vso_decode_rgba(n, coef, Y, lrgba + 4 * l);
-                if (attenuate) {
+                if (attenuate || out_layer_normal) {
                     const uint32_t* ix = L->indices + 3 * (size_t)id;
                     double nrm[3];
                     vso_face_normal(L->positions + 3 * (size_t)ix[0], L->positions + 3 * (size_t)ix[1],
                                     L->positions + 3 * (size_t)ix[2], nrm);
-                    lrgba[4 * l + 3] *= vso_alpha_attenuation(v, nrm);
+                    if (attenuate) lrgba[4 * l + 3] *= vso_alpha_attenuation(v, nrm);
+                    if (out_layer_normal) { /* "Surface normals" buffer: oriented towards the viewer */
+                        double sgn = (v[0] * nrm[0] + v[1] * nrm[1] + v[2] * nrm[2]) > 0.0 ? -1.0 : 1.0;
+                        for (int c = 0; c < 3; ++c) out_layer_normal[((size_t)l * P + p) * 3 + c] = sgn * nrm[c];
+                    }
                 }
                 if (out_layer_rgba) memcpy(out_layer_rgba + ((size_t)l * P + p) * 4, lrgba + 4 * l, 4 * sizeof(double));
                 if (out_layer_uv) { out_layer_uv[((size_t)l * P + p) * 2] = uu; out_layer_uv[((size_t)l * P + p) * 2 + 1] = vv; }
@@ -463,24 +470,25 @@ static int render_impl(const vso_layer* layers, const vso_bands* btex, double v_
 int vso_render(const vso_layer* layers, uint32_t k, uint32_t sh_degree, int tex_dtype, const float* cam,
                uint32_t width, uint32_t height, float near_plane, double t_min, const double* bg,
                double* out_rgba, uint32_t* out_ids, float* out_qp, double* out_layer_rgba,
-               double* out_layer_uv, uint64_t* stats, int num_threads, int attenuate)
+               double* out_layer_uv, uint64_t* stats, int num_threads, int attenuate, double* out_layer_normal)
 {
     return render_impl(layers, NULL, 0.0, 0.0, k, sh_degree, tex_dtype, cam, width, height, near_plane, t_min, bg, out_rgba,
-                       out_ids, out_qp, out_layer_rgba, out_layer_uv, stats, num_threads, attenuate);
+                       out_ids, out_qp, out_layer_rgba, out_layer_uv, stats, num_threads, attenuate, out_layer_normal);
 }
 
 /* The same render with the paper's banded 8-bit textures (layers[l].texture is ignored; bands[l] is used). */
 int vso_render_banded(const vso_layer* layers, const vso_bands* bands, double v_min, double v_max, uint32_t k,
                       uint32_t sh_degree, const float* cam, uint32_t width, uint32_t height, float near_plane,
                       double t_min, const double* bg, double* out_rgba, uint32_t* out_ids, float* out_qp,
-                      double* out_layer_rgba, double* out_layer_uv, uint64_t* stats, int num_threads, int attenuate)
+                      double* out_layer_rgba, double* out_layer_uv, uint64_t* stats, int num_threads, int attenuate,
+                      double* out_layer_normal)
 {
     if (!bands) return -1;
     for (uint32_t l = 0; l < k && l < VSO_MAX_LAYERS; ++l)
         for (uint32_t b = 0; b <= sh_degree && b < 4; ++b)
             if (!bands[l].tex[b] || bands[l].w[b] == 0 || bands[l].h[b] == 0) return -1;
     return render_impl(layers, bands, v_min, v_max, k, sh_degree, 2, cam, width, height, near_plane, t_min, bg, out_rgba,
-                       out_ids, out_qp, out_layer_rgba, out_layer_uv, stats, num_threads, attenuate);
+                       out_ids, out_qp, out_layer_rgba, out_layer_uv, stats, num_threads, attenuate, out_layer_normal);
 }
 
 int vso_max_threads(void)
