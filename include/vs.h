@@ -158,8 +158,8 @@ typedef struct {
 /*
  * vs_scene_create_banded -- vs_scene_create for the banded 8-bit format.  The resulting scene is rendered
  * with the same vs_render / vs_render_host calls (S1-S4 are identical; S5-S6 run in a kernel specialised for
- * byte texels, k_shade_banded).  VS_FLAG_REFERENCE_PATH and the unique-texel count of VS_FLAG_COUNT_TEXELS are
- * not available on such scenes (VS_ERR_UNSUPPORTED / shaded fragments only).
+ * byte texels, k_shade_banded).  VS_FLAG_COUNT_TEXELS counts shaded fragments only on such scenes (no unique-texel
+ * count).
  */
 vs_status vs_scene_create_banded(const vs_scene_desc_banded* desc, void* cuda_stream, vs_scene** out_scene);
 
@@ -203,6 +203,29 @@ vs_status vs_render(vs_scene* scene, const vs_camera* cameras, uint32_t num_came
 vs_status vs_render_host(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
                          const vs_render_params* params, float* out_rgba, uint32_t* out_tri_ids,
                          void* cuda_stream);
+
+/* Per-layer render buffers (supplement Fig. "render buffers": a) surface normals, b) surface UVs,
+ * c) surface opacity, d) surface colors of every layer).  Every pointer is DEVICE memory or
+ * NULL (buffer not wanted); layer index l = 0 is the outermost shell; pixels a layer does not hit hold zeros (ids: MISS).
+ * The buffers describe the nearest fragment of EVERY layer, also of layers the compositor never reached because the
+ * transmittance fell below t_min. */
+typedef struct {
+    uint32_t* tri_ids;      /* [num_cameras][k][H][W]     as vs_render's out_tri_ids                                  */
+    float*    layer_rgba;   /* [num_cameras][k][H][W][4]  rgb = Sigmoid of the SH dot (NOT premultiplied, NOT composited),
+                                                           a = opacity as blended (after VS_FLAG_ATTENUATION's alpha_w)  */
+    float*    layer_uv;     /* [num_cameras][k][H][W][2]  perspective-correct UV of the fragment                       */
+    float*    layer_normal; /* [num_cameras][k][H][W][3]  unit geometric normal of the fragment's triangle, world space,
+                                                           signed to face the viewer (v . n <= 0)                        */
+} vs_aov_buffers;
+
+/*
+ * vs_render_aov -- vs_render plus the per-layer buffers of `aov` (which may be NULL: then it is vs_render without ids).
+ *   The image is produced by the same kernels as vs_render (bit-identical); the buffers are written by a separate plain
+ *   kernel (k_layer_aov) from the triangle-id planes, so the hot path carries no cost for them.  Asynchronous outputs on
+ *   `cuda_stream`, same synchronisation and scratch rules as vs_render.
+ */
+vs_status vs_render_aov(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
+                        const vs_render_params* params, float* out_rgba, const vs_aov_buffers* aov, void* cuda_stream);
 
 /* Counters of the last completed render on this scene. */
 vs_status vs_query_last_render(vs_scene* scene, vs_render_stats* out_stats);

@@ -21,7 +21,7 @@ VS_FLAG_REFERENCE_PATH, VS_FLAG_KERNEL_TIMING, VS_FLAG_COUNT_TEXELS, VS_FLAG_TIL
 VS_FLAG_ATTENUATION = 16
 MISS = 0xFFFFFFFF
 
-EXPORTS = ["vs_scene_create", "vs_scene_create_banded", "vs_render", "vs_render_host", "vs_query_last_render", "vs_scene_destroy",
+EXPORTS = ["vs_scene_create", "vs_scene_create_banded", "vs_render", "vs_render_aov", "vs_render_host", "vs_query_last_render", "vs_scene_destroy",
            "vs_last_error", "vs_version"]
 
 
@@ -51,6 +51,10 @@ class vs_layer_desc_banded(C.Structure):
 class vs_scene_desc_banded(C.Structure):
     _fields_ = [("num_layers", C.c_uint32), ("sh_degree", C.c_uint32), ("memory", C.c_int),
                 ("v_min", C.c_float), ("v_max", C.c_float), ("layers", C.POINTER(vs_layer_desc_banded))]
+
+
+class vs_aov_buffers(C.Structure):
+    _fields_ = [("tri_ids", C.c_void_p), ("layer_rgba", C.c_void_p), ("layer_uv", C.c_void_p), ("layer_normal", C.c_void_p)]
 
 
 class vs_camera(C.Structure):
@@ -99,6 +103,9 @@ def load_library(build_if_missing: bool = True):
         f.restype = C.c_int
         f.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(vs_render_params), C.c_void_p,
                       C.c_void_p, C.c_void_p]
+    L.vs_render_aov.restype = C.c_int
+    L.vs_render_aov.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(vs_render_params), C.c_void_p,
+                                C.POINTER(vs_aov_buffers), C.c_void_p]
     L.vs_query_last_render.restype = C.c_int
     L.vs_query_last_render.argtypes = [C.c_void_p, C.POINTER(vs_render_stats)]
     L.vs_scene_destroy.restype = None
@@ -227,6 +234,21 @@ def vs_render(scene: int, cameras, params: vs_render_params, out_rgba, out_tri_i
         ids_ptr = out_tri_ids.data_ptr()
     _check(load_library().vs_render(scene, cams.ctypes.data, cams.shape[0], C.byref(params),
                                     out_rgba.data_ptr(), ids_ptr, _stream_ptr(stream)))
+
+
+def vs_render_aov(scene: int, cameras, params: vs_render_params, out_rgba, tri_ids=None, layer_rgba=None, layer_uv=None,
+                  layer_normal=None, stream=None):
+    """vs_render plus the per-layer buffers (CUDA tensors or None): tri_ids [B,k,H,W] int32, layer_rgba [B,k,H,W,4],
+    layer_uv [B,k,H,W,2], layer_normal [B,k,H,W,3] float32."""
+    cams = _cams(cameras)
+    assert out_rgba.is_cuda and out_rgba.is_contiguous()
+    a = vs_aov_buffers()
+    for name, t in (("tri_ids", tri_ids), ("layer_rgba", layer_rgba), ("layer_uv", layer_uv), ("layer_normal", layer_normal)):
+        if t is not None:
+            assert t.is_cuda and t.is_contiguous() and t.element_size() == 4
+            setattr(a, name, t.data_ptr())
+    _check(load_library().vs_render_aov(scene, cams.ctypes.data, cams.shape[0], C.byref(params), out_rgba.data_ptr(),
+                                        C.byref(a), _stream_ptr(stream)))
 
 
 def vs_render_host(scene: int, cameras, params: vs_render_params, out_rgba, out_tri_ids=None, stream=None):

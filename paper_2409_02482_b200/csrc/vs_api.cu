@@ -54,6 +54,7 @@ struct vs_scene {
     // scratch, reused between calls
     DevBuf cams, vtx, tri_tiles, tile_count, tile_off, tile_cursor, tile_tris, ids, counters, texel_bits, stage_rgba[2], stage_ids[2];
     DevBuf keys, big_list, big_count;  // direct path
+    DevBuf aov_ids;                    // vs_render_aov without a caller-supplied id buffer
     bool keys_dirty = true;            // the key image holds something other than zeros (fresh allocation or an aborted pass)
     // per-call bookkeeping
     uint64_t launches = 0, raster_launches = 0, shade_launches = 0;
@@ -71,7 +72,7 @@ struct vs_scene {
     {
         for (void* p : owned) cudaFree(p);
         DevBuf* bufs[] = {&cams, &vtx, &tri_tiles, &tile_count, &tile_off, &tile_cursor, &tile_tris, &ids, &counters, &texel_bits,
-                          &stage_rgba[0], &stage_rgba[1], &stage_ids[0], &stage_ids[1], &keys, &big_list, &big_count};
+                          &stage_rgba[0], &stage_rgba[1], &stage_ids[0], &stage_ids[1], &keys, &big_list, &big_count, &aov_ids};
         for (cudaEvent_t e : event_pool) cudaEventDestroy(e);
         for (DevBuf* b : bufs) b->release();
         if (host_counters) cudaFreeHost(host_counters);
@@ -305,8 +306,6 @@ static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, u
     if (!(p->t_min >= 0.0f) || !std::isfinite(p->t_min)) return fail(VS_ERR_INVALID_ARG, "t_min must be >= 0");
     if (p->flags & ~(uint32_t)(VS_FLAG_REFERENCE_PATH | VS_FLAG_KERNEL_TIMING | VS_FLAG_COUNT_TEXELS | VS_FLAG_TILED_PATH | VS_FLAG_ATTENUATION))
         return fail(VS_ERR_INVALID_ARG, "reserved flag bits set");
-    if (scene->dev.banded && (p->flags & VS_FLAG_REFERENCE_PATH))
-        return fail(VS_ERR_UNSUPPORTED, "VS_FLAG_REFERENCE_PATH is not available on banded scenes");
     for (int i = 0; i < 3; ++i)
         if (!std::isfinite(p->background[i])) return fail(VS_ERR_INVALID_ARG, "background not finite");
     for (uint32_t c = 0; c < n; ++c) {
@@ -540,6 +539,51 @@ extern "C" vs_status vs_render(vs_scene* scene, const vs_camera* cameras, uint32
             r = render_chunk(scene, cameras + v0, nv, params, out_rgba + (size_t)v0 * px * 4,
                              out_tri_ids ? out_tri_ids + (size_t)v0 * scene->dev.k * px : nullptr, st);
             if (r != VS_OK) return r;
+        }
+        bool retry = false;
+        if ((r = finish_render(scene, st, &retry)) != VS_OK) return r;
+        if (!retry) return VS_OK;
+    }
+    return fail(VS_ERR_CUDA, "triangle reference list kept overflowing");
+}
+
+extern "C" vs_status vs_render_aov(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
+                                   const vs_render_params* params, float* out_rgba, const vs_aov_buffers* aov,
+                                   void* cuda_stream)
+{
+    if (!aov || (!aov->layer_rgba && !aov->layer_uv && !aov->layer_normal))
+        return vs_render(scene, cameras, num_cameras, params, out_rgba, aov ? aov->tri_ids : nullptr, cuda_stream);
+    g_err[0] = 0;
+    vs_status r = validate_render(scene, cameras, num_cameras, params, out_rgba);
+    if (r != VS_OK) return r;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const uint32_t chunk = pick_chunk(scene, params, num_cameras, false);
+    const size_t px = (size_t)params->width * params->height, kpx = px * scene->dev.k;
+    VsFrame fr;
+    fr.width = params->width; fr.height = params->height;
+    fr.tiles_x = (params->width + VS_TILE_W - 1) / VS_TILE_W; fr.tiles_y = (params->height + VS_TILE_H - 1) / VS_TILE_H;
+    fr.near_plane = params->near_plane; fr.t_min = params->t_min;
+    for (int i = 0; i < 3; ++i) fr.bg[i] = params->background[i];
+    fr.attenuate = (params->flags & VS_FLAG_ATTENUATION) ? 1u : 0u;
+    first_capacity_guess(scene, chunk);
+    for (int attempt = 0; attempt < 4; ++attempt) {
+        if ((r = begin_render(scene, st)) != VS_OK) return r;
+        if (num_cameras == 0) return VS_OK;
+        for (uint32_t v0 = 0; v0 < num_cameras; v0 += chunk) {
+            const uint32_t nv = num_cameras - v0 < chunk ? num_cameras - v0 : chunk;
+            uint32_t* ids = aov->tri_ids ? aov->tri_ids + (size_t)v0 * kpx : nullptr;
+            if (!ids) {
+                CU(scene->aov_ids.reserve(kpx * 4 * chunk + 16));
+                ids = (uint32_t*)scene->aov_ids.p;
+            }
+            r = render_chunk(scene, cameras + v0, nv, params, out_rgba + (size_t)v0 * px * 4, ids, st);
+            if (r != VS_OK) return r;
+            // the chunk's cameras and transformed vertices are still in the scene's scratch
+            CU(vs_launch_layer_aov(scene->dev, scene->tex_f16, fr, nv, (const VsCamDev*)scene->cams.p, (const int4*)scene->vtx.p, ids,
+                                   aov->layer_rgba ? aov->layer_rgba + (size_t)v0 * kpx * 4 : nullptr,
+                                   aov->layer_uv ? aov->layer_uv + (size_t)v0 * kpx * 2 : nullptr,
+                                   aov->layer_normal ? aov->layer_normal + (size_t)v0 * kpx * 3 : nullptr, st));
+            scene->launches += 1;
         }
         bool retry = false;
         if ((r = finish_render(scene, st, &retry)) != VS_OK) return r;

@@ -244,6 +244,24 @@ __device__ __forceinline__ void vs_fragment_setup(const VsSceneDev& sc, const in
     vs_fragment_setup_tri(sc, vv, l, __ldg(&sc.tris[sc.tri_off[l] + local_tri]), px, py, f);
 }
 
+// perspective-correct UV of the winning triangle at the pixel, as base + offset
+__device__ __forceinline__ void vs_fragment_uv(const VsSceneDev& sc, const int4* __restrict__ vv, const uint4 tri, int px, int py,
+                                               float& u0, float& du, float& v0, float& dv)
+{
+    const int4 a = __ldg(&vv[tri.x]), b = __ldg(&vv[tri.y]), c = __ldg(&vv[tri.z]);
+    const float2 uva = __ldg(&sc.uvs[tri.x]), uvb = __ldg(&sc.uvs[tri.y]), uvc = __ldg(&sc.uvs[tri.z]);
+    VsTri T;
+    vs_setup_tri(a, b, c, T);
+    const float2 uv1 = T.swapped ? uvc : uvb, uv2 = T.swapped ? uvb : uvc;
+    VsEdges e;
+    vs_edges_at(T, px, py, e);
+    const float g0 = __ll2float_rn(e.E0) * T.q0, g1 = __ll2float_rn(e.E1) * T.q1, g2 = __ll2float_rn(e.E2) * T.q2;
+    const float inv = __fdividef(1.0f, g0 + g1 + g2);
+    const float b1 = g1 * inv, b2 = g2 * inv;
+    u0 = uva.x; du = b1 * (uv1.x - uva.x) + b2 * (uv2.x - uva.x);
+    v0 = uva.y; dv = b1 * (uv1.y - uva.y) + b2 * (uv2.y - uva.y);
+}
+
 // ---- host-side launchers (vs_kernels_*.cu) ------------------------------------------------------
 struct VsChunk {                 // one pass over `views` cameras
     uint32_t views;
@@ -284,6 +302,8 @@ cudaError_t vs_launch_pack_tris(const uint32_t* indices, const float* layer_posi
                                 uint32_t vtx_off, uint32_t layer, uint4* out, float4* out_normals, uint32_t* error_flag, cudaStream_t st);
 cudaError_t vs_launch_pack_band(const unsigned char* src, uint32_t n_texels, uint32_t band, unsigned char* dst, cudaStream_t st);
 cudaError_t vs_launch_shade_banded(const VsSceneDev& sc, const VsFrame& fr, const struct VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_layer_aov(const VsSceneDev& sc, int f16, const VsFrame& fr, uint32_t views, const VsCamDev* cams, const int4* vtx,
+                                const uint32_t* ids, float* layer_rgba, float* layer_uv, float* layer_normal, cudaStream_t st);
 cudaError_t vs_launch_check_finite(const float* v, size_t n, uint32_t* error_flag, cudaStream_t st);
 cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, uint32_t n_coef, uint32_t np_pad,
                                    uint4* dst, cudaStream_t st);

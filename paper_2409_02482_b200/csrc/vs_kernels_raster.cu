@@ -16,6 +16,7 @@
 // for all k layers of the tile at once and is written out as the triangle-id planes the shading
 // kernel (and the parity tests) read.
 #include "vs_common.cuh"
+#include "vs_plain.cuh"
 
 #define VS_RS_FIELDS 12                      // words per small-triangle record
 #define VS_RS_QUEUE 512u                    // (lane, sample) codes per compaction round
@@ -308,23 +309,8 @@ k_reference(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ 
         const uint32_t lid = 0xFFFFFFFFu - (uint32_t)best;
         if (out_ids) out_ids[(((size_t)view * sc.k + l) * H + py) * W + px] = hit ? lid : VS_MISS;
         if (!hit || !alive) continue;
-        VsFrag f;
-        vs_fragment_setup(sc, vv, l, lid, px, py, f);
-        const uint32_t Wt = sc.tex_w[l], nv = sc.texel_vecs;
-        const uint32_t offs[4] = {(f.cy0 * Wt + f.cx0) * nv, (f.cy0 * Wt + f.cx1) * nv, (f.cy1 * Wt + f.cx0) * nv, (f.cy1 * Wt + f.cx1) * nv};
-        const float ws[4] = {(1.0f - f.a) * (1.0f - f.b), f.a * (1.0f - f.b), (1.0f - f.a) * f.b, f.a * f.b};
-        float s[4] = {0.0f, 0.0f, 0.0f, 0.0f};
-        for (uint32_t c = 0; c < sc.n_coef; ++c)
-            for (int ch = 0; ch < 4; ++ch) {
-                float v = 0.0f;
-                for (int q = 0; q < 4; ++q) {
-                    float tv;
-                    if (F16) tv = __half2float(reinterpret_cast<const __half*>(sc.tex[l] + offs[q])[ch * sc.np_pad + c]);
-                    else tv = reinterpret_cast<const float*>(sc.tex[l] + offs[q])[ch * sc.np_pad + c];
-                    v += ws[q] * tv;
-                }
-                s[ch] += Y[c] * v;
-            }
+        float s[4], uv[2];
+        vs_plain_logits<F16>(sc, vv, l, lid, px, py, Y, s, uv);
         float A = vs_sigmoid(s[3]);
         if (fr.attenuate) A *= vs_alpha_w(vx, vy, vz, sc.tri_nrm[sc.tri_off[l] + lid]);
         for (int ch = 0; ch < 3; ++ch) C[ch] += Tr * A * vs_sigmoid(s[ch]);

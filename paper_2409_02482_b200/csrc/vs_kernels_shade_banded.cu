@@ -72,24 +72,6 @@ __device__ __forceinline__ void vs_acc_coef(uint32_t w0, uint32_t w1, uint32_t w
     acc[3] = vs_fma2(Z23, vs_add2(vs_bytes_magic<3>(w2, w3), NM), acc[3]);
 }
 
-// perspective-correct UV of the winning triangle at the pixel, as base + offset
-__device__ __forceinline__ void vs_fragment_uv(const VsSceneDev& sc, const int4* __restrict__ vv, const uint4 tri, int px, int py,
-                                               float& u0, float& du, float& v0, float& dv)
-{
-    const int4 a = __ldg(&vv[tri.x]), b = __ldg(&vv[tri.y]), c = __ldg(&vv[tri.z]);
-    const float2 uva = __ldg(&sc.uvs[tri.x]), uvb = __ldg(&sc.uvs[tri.y]), uvc = __ldg(&sc.uvs[tri.z]);
-    VsTri T;
-    vs_setup_tri(a, b, c, T);
-    const float2 uv1 = T.swapped ? uvc : uvb, uv2 = T.swapped ? uvb : uvc;
-    VsEdges e;
-    vs_edges_at(T, px, py, e);
-    const float g0 = __ll2float_rn(e.E0) * T.q0, g1 = __ll2float_rn(e.E1) * T.q1, g2 = __ll2float_rn(e.E2) * T.q2;
-    const float inv = __fdividef(1.0f, g0 + g1 + g2);
-    const float b1 = g1 * inv, b2 = g2 * inv;
-    u0 = uva.x; du = b1 * (uv1.x - uva.x) + b2 * (uv2.x - uva.x);
-    v0 = uva.y; dv = b1 * (uv1.y - uva.y) + b2 * (uv2.y - uva.y);
-}
-
 // band B of one fragment: 2x2 footprint at the band's own resolution, accumulated into the four channel sums
 template <int B>
 __device__ __forceinline__ void vs_band(const VsSceneDev& sc, uint32_t l, float u0, float du, float v0, float dv, const float* Y,

@@ -172,14 +172,64 @@ def test_banded_host_descriptors_and_errors(env):
     ids = torch.empty((3, sc.k, 120, 160), dtype=torch.int32).pin_memory()
     b.vs_render_host(h, sc.cameras, b.make_params(160, 120, flags=env.path_flags), out, ids)
     assert np.array_equal(out.numpy(), dev_rgba) and np.array_equal(ids.numpy().view(np.uint32), dev_ids)
-    dout = torch.empty((3, 120, 160, 4), dtype=torch.float32, device="cuda")
-    with pytest.raises(b.VsError) as e:                                          # no brute-force kernel for this format
-        b.vs_render(h, sc.cameras, b.make_params(160, 120, flags=b.VS_FLAG_REFERENCE_PATH), dout)
-    assert e.value.status == b.VS_ERR_UNSUPPORTED
     b.vs_scene_destroy(h)
+    # the brute-force kernel reads the banded format too and agrees with the fast path
+    ref = gpu_render(env, sc, [0, 2], flags=b.VS_FLAG_REFERENCE_PATH)
+    assert np.array_equal(ref[1], dev_ids[[0, 2]]) and np.abs(ref[0] - dev_rgba[[0, 2]]).max() <= 2e-6
     with pytest.raises(b.VsError) as e:
         b.vs_scene_create_banded(sc.layers, sc.sh_degree, float("nan"), 15.0)
     assert e.value.status == b.VS_ERR_INVALID_ARG
+
+
+# ---- per-layer render buffers through vs_render_aov ----
+def check_aov(env, sc, views, attenuation=False, t_min=None, views_per_chunk=0, give_ids=True):
+    b, torch = env.binding, env.torch
+    flags = env.path_flags | (b.VS_FLAG_ATTENUATION if attenuation else 0)
+    p = b.make_params(sc.width, sc.height, sc.near_plane, sc.t_min if t_min is None else t_min, sc.background, flags, views_per_chunk)
+    r = b.Renderer(sc)
+    B, k, H, W = len(views), sc.k, sc.height, sc.width
+    dev = lambda *shape, dt=torch.float32: torch.full(shape, 7, dtype=dt, device="cuda")
+    out, ids = dev(B, H, W, 4), dev(B, k, H, W, dt=torch.int32) if give_ids else None
+    lrgba, luv, lnrm = dev(B, k, H, W, 4), dev(B, k, H, W, 2), dev(B, k, H, W, 3)
+    b.vs_render_aov(r.handle, sc.cameras[list(views)], p, out, ids, lrgba, luv, lnrm)
+    torch.cuda.synchronize()
+    plain, _ = r.render(sc.cameras[list(views)], p)
+    torch.cuda.synchronize()
+    assert torch.equal(plain, out), "vs_render_aov and vs_render images differ"
+    r.close()
+    okw = dict(want_layer_rgba=True, want_layer_uv=True, want_layer_normal=True, attenuation=attenuation)
+    if t_min is not None:
+        okw["t_min"] = t_min
+    for n, v in enumerate(views):
+        ref = env.oracle.render_scene(sc, [v], **okw)[0]
+        if give_ids:
+            assert np.array_equal(ids[n].cpu().numpy().view(np.uint32), ref["ids"])
+        assert np.abs(out[n].cpu().numpy() - ref["rgba"]).max() <= TOL
+        assert np.abs(lrgba[n].cpu().numpy() - ref["layer_rgba"]).max() <= TOL
+        assert np.abs(luv[n].cpu().numpy() - ref["layer_uv"]).max() <= 1e-5
+        assert np.abs(lnrm[n].cpu().numpy() - ref["layer_normal"]).max() <= 1e-6
+    return lrgba, luv, lnrm
+
+
+def test_aov_config1(env):
+    sc = env.synth.make_config(1)
+    lrgba, luv, lnrm = check_aov(env, sc, range(4), views_per_chunk=3)
+    assert float(luv.min()) >= 0.0 and float(luv.max()) <= 1.0            # SPEC.md:L503 "UV buffer values in [0,1]^2"
+    check_aov(env, sc, [1], attenuation=True, give_ids=False)
+
+
+def test_aov_early_exit_layers_still_filled(env):
+    sc = env.synth.make_config(1, width=100, height=60, num_cameras=1, tex_size=64)
+    for ly in sc.layers:
+        ly.texture[:, :, 0, 3] += 12.0                                       # near-opaque: compositing stops after layer 0
+    lrgba, _, _ = check_aov(env, sc, [0], t_min=2.0 ** -6)
+    assert float(lrgba[0, 2, ..., 3].max()) > 0.99                           # ... the innermost layer's buffer is filled anyway
+
+
+@pytest.mark.parametrize("banded", [False, True])
+def test_aov_reduced_config4(env, banded):
+    sc = env.synth.make_config(4, mesh_n=64, width=480, height=270, tex_size=512, num_cameras=3, k=9, banded=banded)
+    check_aov(env, sc, range(3), attenuation=True, views_per_chunk=2)
 
 
 def test_determinism_and_chunking(env):
