@@ -44,6 +44,10 @@ def lib():
                                         C.c_void_p, C.c_uint32, C.c_uint32, C.c_float, C.c_double, C.c_void_p,
                                         C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p,
                                         C.c_void_p, C.c_int, C.c_int, C.c_void_p]
+        L.vso_render_backward.restype = C.c_int
+        L.vso_render_backward.argtypes = [C.POINTER(_Layer), C.c_uint32, C.c_uint32, C.c_int, C.c_void_p, C.c_uint32, C.c_uint32,
+                                          C.c_float, C.c_double, C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p),
+                                          C.c_int, C.c_int]
         L.vso_quantize.restype = C.c_double
         L.vso_quantize.argtypes = [C.c_double]
         L.vso_rescale.restype = C.c_double
@@ -154,6 +158,40 @@ def render_view(layers, sh_degree: int, camera, width: int, height: int, *, near
     if want_layer_normal:
         out["layer_normal"] = lnrm
     return out
+
+
+def render_backward(layers, sh_degree: int, camera, width: int, height: int, ids, grad_out, grad_tex=None, *,
+                    near_plane: float = 0.05, t_min: float = 2.0 ** -14, background=(0.0, 0.0, 0.0),
+                    attenuation: bool = False, num_threads: int = 0):
+    """Accumulate dL/d(texture) of every layer for one view, given the forward ids of that view and the upstream
+    gradient grad_out [H,W,4].  grad_tex: list of float64 arrays shaped like the textures (created as zeros if None);
+    returned."""
+    k = len(layers)
+    arr = (_Layer * k)()
+    keep, code = [], None
+    for i, L in enumerate(layers):
+        pos = np.ascontiguousarray(L.positions, dtype=np.float32)
+        uv = np.ascontiguousarray(L.uvs, dtype=np.float32)
+        idx = np.ascontiguousarray(L.indices, dtype=np.uint32)
+        tex = np.ascontiguousarray(L.texture)
+        code = _dtype_code(tex)
+        keep += [pos, uv, idx, tex]
+        arr[i] = _Layer(_ptr(pos), _ptr(uv), _ptr(idx), _ptr(tex), pos.shape[0], idx.shape[0], tex.shape[1], tex.shape[0])
+    if grad_tex is None:
+        grad_tex = [np.zeros(L.texture.shape, dtype=np.float64) for L in layers]
+    for gt, L in zip(grad_tex, layers):
+        assert gt.dtype == np.float64 and gt.flags.c_contiguous and gt.shape == L.texture.shape
+    gptr = (C.c_void_p * k)(*[g.ctypes.data for g in grad_tex])
+    cam = np.ascontiguousarray(camera, dtype=np.float32)
+    bg = np.asarray(background, dtype=np.float64)
+    ids = np.ascontiguousarray(ids, dtype=np.uint32)
+    go = np.ascontiguousarray(grad_out, dtype=np.float64)
+    assert ids.shape == (k, height, width) and go.shape == (height, width, 4)
+    rc = lib().vso_render_backward(arr, k, sh_degree, code, _ptr(cam), width, height, near_plane, t_min, _ptr(bg),
+                                   _ptr(ids), _ptr(go), gptr, 1 if attenuation else 0, num_threads)
+    if rc != 0:
+        raise ValueError("vso_render_backward rejected its arguments (rc=%d)" % rc)
+    return grad_tex
 
 
 def render_scene(scene, views=None, **kw):

@@ -491,6 +491,131 @@ int vso_render_banded(const vso_layer* layers, const vso_bands* bands, double v_
                        out_ids, out_qp, out_layer_rgba, out_layer_uv, stats, num_threads, attenuate, out_layer_normal);
 }
 
+/*
+ * Backward pass to the texels (§4.5: the baked textures are optimised through
+ * the same bilinear lookup "such that when displayed in our real-time renderer, images match ... those synthesized by our
+ * differentiable renderer").  Given the triangle ids of a forward render of the SAME view and settings
+ * (`ids` [k][H][W], as written by vso_render) and an upstream gradient g = dL/d(out_rgba) [H][W][4], ACCUMULATES
+ * dL/d(texture of layer l) into grad_tex[l] ([tex_h][tex_w][n][4] double, same layout as the texture), by the chain rule
+ * through A.8 blend -> A.7 sigmoid / SH dot -> A.6 bilinear weights (and alpha_w, a constant factor, if `attenuate`):
+ *   out_rgb = sum_l T_l A_l rgb_l + T_end bg,  out_a = 1 - T_end,  T_{l+1} = T_l (1 - A_l)
+ *   R_end = bg . g_rgb - g_a ;  R_{l-1} = A_l (rgb_l . g_rgb) + (1 - A_l) R_l       (what lies behind layer l, per unit T)
+ *   dL/dA_l = T_l (rgb_l . g_rgb - R_l) ;  dL/drgb_l = T_l A_l g_rgb
+ *   dL/ds_ch = dL/drgb_ch rgb_ch (1 - rgb_ch) ;  dL/ds_3 = dL/dA alpha_w sigma(s_3) (1 - sigma(s_3))
+ *   dL/dtex[q][c][ch] += w_q Y_c dL/ds_ch           for the four texels q of the footprint
+ * The early exit is a constant of the differentiation (layers behind it get no gradient); coverage and UVs do not depend
+ * on the textures.  Float textures only (dtype 0 / 1).  Returns 0, or -1 on bad arguments.
+ */
+int vso_render_backward(const vso_layer* layers, uint32_t k, uint32_t sh_degree, int tex_dtype, const float* cam,
+                        uint32_t width, uint32_t height, float near_plane, double t_min, const double* bg,
+                        const uint32_t* ids, const double* grad_out, double* const* grad_tex, int attenuate, int num_threads)
+{
+    if (!layers || k < 1 || k > VSO_MAX_LAYERS || sh_degree > 3 || !cam || !ids || !grad_out || !grad_tex || tex_dtype > 1)
+        return -1;
+    const uint32_t n = (sh_degree + 1) * (sh_degree + 1);
+    const size_t P = (size_t)width * height;
+#ifdef _OPENMP
+    if (num_threads < 1) num_threads = omp_get_max_threads();
+#else
+    num_threads = 1;
+#endif
+    vso_vtx** vtx = (vso_vtx**)calloc(k, sizeof(vso_vtx*));
+    if (!vtx) return -1;
+    for (uint32_t l = 0; l < k; ++l) {
+        vtx[l] = (vso_vtx*)malloc(sizeof(vso_vtx) * (layers[l].num_vertices ? layers[l].num_vertices : 1));
+        if (!vtx[l]) return -1;
+        for (int64_t i = 0; i < (int64_t)layers[l].num_vertices; ++i) {
+            int32_t bad;
+            vso_transform_vertex(cam, near_plane, layers[l].positions + 3 * i, &vtx[l][i].X, &vtx[l][i].Y, &vtx[l][i].q, &bad);
+            vtx[l][i].bad = bad;
+        }
+    }
+#pragma omp parallel for num_threads(num_threads) schedule(dynamic, 4)
+    for (int64_t j = 0; j < (int64_t)height; ++j) {
+        for (int64_t i = 0; i < (int64_t)width; ++i) {
+            size_t p = (size_t)j * width + (size_t)i;
+            double v[3], Y[VSO_MAX_COEF];
+            view_dir(cam, (int)i, (int)j, v);
+            vso_sh_basis((int)sh_degree, v, Y);
+            /* forward, keeping what the backward needs */
+            double rgb[VSO_MAX_LAYERS][3], sig3[VSO_MAX_LAYERS], aw[VSO_MAX_LAYERS], A[VSO_MAX_LAYERS], Tl[VSO_MAX_LAYERS];
+            double wq[VSO_MAX_LAYERS][4];
+            int64_t tx[VSO_MAX_LAYERS][4], ty[VSO_MAX_LAYERS][4];
+            int order[VSO_MAX_LAYERS], cnt = 0;
+            double T = 1.0;
+            for (uint32_t l = 0; l < k; ++l) {
+                uint32_t id = ids[(size_t)l * P + p];
+                if (id == VSO_MISS) continue;
+                const vso_layer* L = &layers[l];
+                vso_tri tri;
+                int64_t E[3];
+                vso_setup(vtx[l], L->indices + 3 * (size_t)id, &tri);
+                vso_covers(&tri, (int)i, (int)j, E);
+                double g[3], gs = 0.0, uu = 0.0, vv = 0.0;
+                for (int c = 0; c < 3; ++c) { g[c] = (double)E[c] * (double)tri.q[c]; gs += g[c]; }
+                for (int c = 0; c < 3; ++c) {
+                    double b = g[c] / gs;
+                    uu += b * (double)L->uvs[2 * (size_t)tri.vi[c] + 0];
+                    vv += b * (double)L->uvs[2 * (size_t)tri.vi[c] + 1];
+                }
+                /* A.6 footprint and weights */
+                double x = uu * (double)L->tex_w - 0.5, y = vv * (double)L->tex_h - 0.5;
+                double x0 = floor(x), y0 = floor(y), a = x - x0, b = y - y0;
+                int64_t ix0 = clampi((int64_t)x0, 0, (int64_t)L->tex_w - 1), ix1 = clampi((int64_t)x0 + 1, 0, (int64_t)L->tex_w - 1);
+                int64_t iy0 = clampi((int64_t)y0, 0, (int64_t)L->tex_h - 1), iy1 = clampi((int64_t)y0 + 1, 0, (int64_t)L->tex_h - 1);
+                tx[l][0] = ix0; ty[l][0] = iy0; wq[l][0] = (1.0 - b) * (1.0 - a);
+                tx[l][1] = ix1; ty[l][1] = iy0; wq[l][1] = (1.0 - b) * a;
+                tx[l][2] = ix0; ty[l][2] = iy1; wq[l][2] = b * (1.0 - a);
+                tx[l][3] = ix1; ty[l][3] = iy1; wq[l][3] = b * a;
+                double sch[4] = {0.0, 0.0, 0.0, 0.0};
+                for (uint32_t c = 0; c < n; ++c)
+                    for (int ch = 0; ch < 4; ++ch) {
+                        double t = 0.0;
+                        for (int q = 0; q < 4; ++q) t += wq[l][q] * tex_fetch(L->texture, tex_dtype, L->tex_w, n, tx[l][q], ty[l][q], 4 * c + ch);
+                        sch[ch] += Y[c] * t;
+                    }
+                for (int ch = 0; ch < 3; ++ch) rgb[l][ch] = 1.0 / (1.0 + exp(-sch[ch]));
+                sig3[l] = 1.0 / (1.0 + exp(-sch[3]));
+                aw[l] = 1.0;
+                if (attenuate) {
+                    const uint32_t* ix = L->indices + 3 * (size_t)id;
+                    double nrm[3];
+                    vso_face_normal(L->positions + 3 * (size_t)ix[0], L->positions + 3 * (size_t)ix[1], L->positions + 3 * (size_t)ix[2], nrm);
+                    aw[l] = vso_alpha_attenuation(v, nrm);
+                }
+                A[l] = sig3[l] * aw[l];
+                Tl[l] = T;
+                order[cnt++] = (int)l;
+                T *= (1.0 - A[l]);
+                if (T < t_min) break;
+            }
+            /* backward */
+            const double* go = grad_out + p * 4;
+            double R = bg[0] * go[0] + bg[1] * go[1] + bg[2] * go[2] - go[3];
+            for (int o = cnt - 1; o >= 0; --o) {
+                int l = order[o];
+                double cg = rgb[l][0] * go[0] + rgb[l][1] * go[1] + rgb[l][2] * go[2];
+                double ds[4];
+                for (int ch = 0; ch < 3; ++ch) ds[ch] = Tl[l] * A[l] * go[ch] * rgb[l][ch] * (1.0 - rgb[l][ch]);
+                ds[3] = Tl[l] * (cg - R) * aw[l] * sig3[l] * (1.0 - sig3[l]);
+                R = A[l] * cg + (1.0 - A[l]) * R;
+                const vso_layer* L = &layers[l];
+                for (int q = 0; q < 4; ++q)
+                    for (uint32_t c = 0; c < n; ++c)
+                        for (int ch = 0; ch < 4; ++ch) {
+                            double* slot = grad_tex[l] + (((size_t)ty[l][q] * L->tex_w + (size_t)tx[l][q]) * n + c) * 4 + ch;
+                            double add = wq[l][q] * Y[c] * ds[ch];
+#pragma omp atomic
+                            *slot += add;
+                        }
+            }
+        }
+    }
+    for (uint32_t l = 0; l < k; ++l) free(vtx[l]);
+    free(vtx);
+    return 0;
+}
+
 int vso_max_threads(void)
 {
 #ifdef _OPENMP
