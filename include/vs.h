@@ -227,6 +227,23 @@ typedef struct {
 vs_status vs_render_aov(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
                         const vs_render_params* params, float* out_rgba, const vs_aov_buffers* aov, void* cuda_stream);
 
+/*
+ * vs_render_backward -- backward pass to the texels (§4.5: the texture values are optimised through
+ * the lookup the real-time renderer performs).  For the same scene, cameras and
+ * params as a vs_render call, and an upstream gradient dL/d(out_rgba), ACCUMULATES dL/d(texture coefficient), summed
+ * over the cameras, by the chain rule through the blend (S7), the sigmoids and SH dot (S6) and the bilinear weights (S5);
+ * VS_FLAG_ATTENUATION's alpha_w and the t_min early exit are constants of the differentiation (layers behind the exit get
+ * no gradient); coverage and UVs do not depend on the textures.
+ *   grad_rgba      DEVICE [num_cameras][height][width][4] float
+ *   grad_textures  HOST array of num_layers DEVICE pointers, layer l: [tex_h][tex_w][(deg+1)^2][4] float (the API layout
+ *                  of vs_layer_desc.texture, always fp32); the caller zeroes them; sums are fp32 atomics in no fixed order
+ *   Float-texture scenes only (VS_ERR_UNSUPPORTED on banded scenes and with VS_FLAG_REFERENCE_PATH / TILED / COUNT).
+ *   Runs S1-S4 again (nothing of the forward call is kept) and k_backward in place of k_shade; returns when done.
+ */
+vs_status vs_render_backward(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
+                             const vs_render_params* params, const float* grad_rgba, float* const* grad_textures,
+                             void* cuda_stream);
+
 /* Counters of the last completed render on this scene. */
 vs_status vs_query_last_render(vs_scene* scene, vs_render_stats* out_stats);
 

@@ -21,7 +21,7 @@ VS_FLAG_REFERENCE_PATH, VS_FLAG_KERNEL_TIMING, VS_FLAG_COUNT_TEXELS, VS_FLAG_TIL
 VS_FLAG_ATTENUATION = 16
 MISS = 0xFFFFFFFF
 
-EXPORTS = ["vs_scene_create", "vs_scene_create_banded", "vs_render", "vs_render_aov", "vs_render_host", "vs_query_last_render", "vs_scene_destroy",
+EXPORTS = ["vs_scene_create", "vs_scene_create_banded", "vs_render", "vs_render_aov", "vs_render_backward", "vs_render_host", "vs_query_last_render", "vs_scene_destroy",
            "vs_last_error", "vs_version"]
 
 
@@ -106,6 +106,9 @@ def load_library(build_if_missing: bool = True):
     L.vs_render_aov.restype = C.c_int
     L.vs_render_aov.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(vs_render_params), C.c_void_p,
                                 C.POINTER(vs_aov_buffers), C.c_void_p]
+    L.vs_render_backward.restype = C.c_int
+    L.vs_render_backward.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(vs_render_params), C.c_void_p,
+                                     C.POINTER(C.c_void_p), C.c_void_p]
     L.vs_query_last_render.restype = C.c_int
     L.vs_query_last_render.argtypes = [C.c_void_p, C.POINTER(vs_render_stats)]
     L.vs_scene_destroy.restype = None
@@ -249,6 +252,18 @@ def vs_render_aov(scene: int, cameras, params: vs_render_params, out_rgba, tri_i
             setattr(a, name, t.data_ptr())
     _check(load_library().vs_render_aov(scene, cams.ctypes.data, cams.shape[0], C.byref(params), out_rgba.data_ptr(),
                                         C.byref(a), _stream_ptr(stream)))
+
+
+def vs_render_backward(scene: int, cameras, params: vs_render_params, grad_rgba, grad_textures, stream=None):
+    """grad_rgba: CUDA float32 [B,H,W,4]; grad_textures: list of k CUDA float32 tensors [tex_h,tex_w,n,4], accumulated into."""
+    cams = _cams(cameras)
+    assert grad_rgba.is_cuda and grad_rgba.is_contiguous() and grad_rgba.numel() == cams.shape[0] * params.width * params.height * 4
+    import torch
+    for t in grad_textures:
+        assert t.is_cuda and t.is_contiguous() and t.dtype == torch.float32
+    ptrs = (C.c_void_p * len(grad_textures))(*[t.data_ptr() for t in grad_textures])
+    _check(load_library().vs_render_backward(scene, cams.ctypes.data, cams.shape[0], C.byref(params), grad_rgba.data_ptr(),
+                                             ptrs, _stream_ptr(stream)))
 
 
 def vs_render_host(scene: int, cameras, params: vs_render_params, out_rgba, out_tri_ids=None, stream=None):

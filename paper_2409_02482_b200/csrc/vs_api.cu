@@ -357,7 +357,8 @@ static vs_status span_end(vs_scene* s, bool on, cudaStream_t st)
 
 // Render `views` cameras starting at cams[0] into device outputs.  All work on `st`, no host sync.
 static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views, const vs_render_params* p,
-                              float* out_rgba, uint32_t* out_ids, cudaStream_t st)
+                              float* out_rgba, uint32_t* out_ids, cudaStream_t st, const float* grad_out = nullptr,
+                              const VsGradTex* grad_tex = nullptr)
 {
     VsFrame fr;
     fr.width = p->width; fr.height = p->height;
@@ -449,7 +450,12 @@ static vs_status render_chunk(vs_scene* s, const vs_camera* cams, uint32_t views
         CU(vs_launch_raster_direct(s->dev, fr, ch, st));
         if ((r = span_end(s, timing, st)) != VS_OK) return r;
         if ((r = span_begin(s, timing, 3, st)) != VS_OK) return r;
-        CU(s->dev.banded ? vs_launch_shade_banded(s->dev, fr, ch, st) : vs_launch_shade(s->dev, s->tex_f16, fr, ch, st));
+        if (grad_out) {   // vs_render_backward: k_backward consumes the key image in place of k_shade
+            ch.grad_out = grad_out; ch.grad_tex = *grad_tex;
+            CU(vs_launch_backward(s->dev, s->tex_f16, fr, ch, st));
+        } else {
+            CU(s->dev.banded ? vs_launch_shade_banded(s->dev, fr, ch, st) : vs_launch_shade(s->dev, s->tex_f16, fr, ch, st));
+        }
         if ((r = span_end(s, timing, st)) != VS_OK) return r;
         s->keys_dirty = false;
         s->launches += (s->dev.t_total ? 2 : 0) + 1;
@@ -545,6 +551,35 @@ extern "C" vs_status vs_render(vs_scene* scene, const vs_camera* cameras, uint32
         if (!retry) return VS_OK;
     }
     return fail(VS_ERR_CUDA, "triangle reference list kept overflowing");
+}
+
+extern "C" vs_status vs_render_backward(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
+                                        const vs_render_params* params, const float* grad_rgba,
+                                        float* const* grad_textures, void* cuda_stream)
+{
+    g_err[0] = 0;
+    vs_status r = validate_render(scene, cameras, num_cameras, params, grad_rgba);
+    if (r != VS_OK) return r;
+    if (!grad_textures) return fail(VS_ERR_INVALID_ARG, "NULL argument");
+    if (scene->dev.banded) return fail(VS_ERR_UNSUPPORTED, "vs_render_backward: float textures only (banded scenes are baked, not fitted)");
+    if (params->flags & (VS_FLAG_REFERENCE_PATH | VS_FLAG_TILED_PATH | VS_FLAG_COUNT_TEXELS))
+        return fail(VS_ERR_UNSUPPORTED, "vs_render_backward runs on the default (direct) raster path only");
+    VsGradTex gt{};
+    for (uint32_t l = 0; l < scene->dev.k; ++l) {
+        if (!grad_textures[l]) return fail(VS_ERR_INVALID_ARG, "grad_textures[%u] is NULL", l);
+        gt.p[l] = grad_textures[l];
+    }
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const uint32_t chunk = pick_chunk(scene, params, num_cameras, false);
+    const size_t px = (size_t)params->width * params->height;
+    if ((r = begin_render(scene, st)) != VS_OK) return r;
+    for (uint32_t v0 = 0; v0 < num_cameras; v0 += chunk) {
+        const uint32_t nv = num_cameras - v0 < chunk ? num_cameras - v0 : chunk;
+        r = render_chunk(scene, cameras + v0, nv, params, nullptr, nullptr, st, grad_rgba + (size_t)v0 * px * 4, &gt);
+        if (r != VS_OK) return r;
+    }
+    bool retry = false;
+    return finish_render(scene, st, &retry);
 }
 
 extern "C" vs_status vs_render_aov(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,

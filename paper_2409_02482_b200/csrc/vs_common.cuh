@@ -263,6 +263,8 @@ __device__ __forceinline__ void vs_fragment_uv(const VsSceneDev& sc, const int4*
 }
 
 // ---- host-side launchers (vs_kernels_*.cu) ------------------------------------------------------
+struct VsGradTex { float* p[VS_MAX_LAYERS]; };   // per layer [tex_h][tex_w][n_coef][4] fp32 gradient accumulators (API texture layout)
+
 struct VsChunk {                 // one pass over `views` cameras
     uint32_t views;
     const VsCamDev* cams;        // DEVICE [views]
@@ -278,6 +280,8 @@ struct VsChunk {                 // one pass over `views` cameras
     int ids_is_output;           // ids is the caller's AOV: empty tiles must be filled with MISS too
     float* out_rgba;             // DEVICE [views][H][W][4]
     uint32_t* texel_bits;        // DEVICE [views][tex_bit_off[k] / 32] or nullptr (VS_FLAG_COUNT_TEXELS)
+    const float* grad_out;       // DEVICE [views][H][W][4] upstream gradient: vs_render_backward runs k_backward instead of k_shade
+    VsGradTex grad_tex;
     int count_fragments;         // banded scenes under VS_FLAG_COUNT_TEXELS: count shaded fragments only
     // direct (untiled) path: non-null keys selects it in vs_launch_shade
     unsigned long long* keys;    // DEVICE [views][k][H][W] max keys, zero between passes
@@ -302,6 +306,7 @@ cudaError_t vs_launch_pack_tris(const uint32_t* indices, const float* layer_posi
                                 uint32_t vtx_off, uint32_t layer, uint4* out, float4* out_normals, uint32_t* error_flag, cudaStream_t st);
 cudaError_t vs_launch_pack_band(const unsigned char* src, uint32_t n_texels, uint32_t band, unsigned char* dst, cudaStream_t st);
 cudaError_t vs_launch_shade_banded(const VsSceneDev& sc, const VsFrame& fr, const struct VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_backward(const VsSceneDev& sc, int f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_layer_aov(const VsSceneDev& sc, int f16, const VsFrame& fr, uint32_t views, const VsCamDev* cams, const int4* vtx,
                                 const uint32_t* ids, float* layer_rgba, float* layer_uv, float* layer_normal, cudaStream_t st);
 cudaError_t vs_launch_check_finite(const float* v, size_t n, uint32_t* error_flag, cudaStream_t st);

@@ -1,0 +1,114 @@
+// vs_kernels_backward.cu -- backward pass to the texels (§4.5: the textures are
+// fitted through the very lookup the renderer performs).  Given dL/d(out_rgba) of a batch of views it
+// accumulates dL/d(texture coefficient) of every layer, by the chain rule through S7 blend -> S6 sigmoid / SH dot ->
+// S5 bilinear weights.  S1-S4 (transform, coverage, nearest fragment) run unchanged before it: this kernel takes the
+// place of k_shade and consumes (and clears) the same key image.
+//
+// One lane = one pixel.  Pass 1 re-shades the pixel's fragments front to back with the plain routine of vs_plain.cuh and
+// keeps (rgb, sigma, alpha_w, T) of every layer it composites; pass 2 walks them back to front with the recurrence
+//   R_end = bg . g_rgb - g_a ;  dL/dA_l = T_l (rgb_l . g_rgb - R_l) ;  R_{l-1} = A_l (rgb_l . g_rgb) + (1 - A_l) R_l
+// and scatters w_q Y_c dL/ds_ch into the gradient textures ([texel][c][ch] fp32 = the API layout of the textures) with
+// fire-and-forget vector reductions: one RED.ADD.v4.F32 per (texel, coefficient), 4 (deg + 1)^2 per fragment.
+// The scatter is the cost: 64 x 16-byte reductions per fragment at degree 3 against 512 bytes read -- bound by the L2's
+// reduction rate, not by HBM or the ALUs.  fp32 sums in arbitrary order: parity is to a relative tolerance.
+#include "vs_common.cuh"
+#include "vs_plain.cuh"
+
+__device__ __forceinline__ void vs_red_add4(float* p, float a, float b, float c, float d)
+{
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+
+template <int F16>
+__global__ void __launch_bounds__(256)
+k_backward(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams, const int4* __restrict__ vtx,
+           const uint32_t* __restrict__ tile_mask, unsigned long long* __restrict__ keys, const float* __restrict__ grad_out,
+           VsGradTex gt)
+{
+    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t tile = blockIdx.x, view = blockIdx.y;
+    const uint32_t tiles = fr.tiles_x * fr.tiles_y;
+    const int W = (int)fr.width, H = (int)fr.height;
+    const int lx = (int)(warp & 1) * 8 + (int)(lane & 7), ly = (int)(warp >> 1) * 4 + (int)(lane >> 3);
+    const int px = (int)(tile % fr.tiles_x) * VS_TILE_W + lx, py = (int)(tile / fr.tiles_x) * VS_TILE_H + ly;
+    const uint32_t lmask = tile_mask[view * tiles + tile];
+    if (lmask == 0u || px >= W || py >= H) return;
+    const size_t plane = (size_t)W * H;
+    const size_t pix0 = (size_t)view * sc.k * plane + (size_t)py * W + px;
+    const int4* __restrict__ vv = vtx + (size_t)view * sc.v_total;
+
+    float Y[VS_MAX_COEF];
+    float vx, vy, vz;
+    vs_view_dir(cams[view], px, py, vx, vy, vz);
+    vs_sh_basis<3>(vx, vy, vz, Y);
+
+    // pass 1: forward, front to back
+    uint32_t ids[VS_MAX_LAYERS];
+    float rgb[VS_MAX_LAYERS][3], sig3[VS_MAX_LAYERS], aw[VS_MAX_LAYERS], Tl[VS_MAX_LAYERS];
+    uint32_t used = 0;                       // layers that were composited (bit l)
+    float Tr = 1.0f;
+    bool alive = true;
+    for (uint32_t l = 0; l < sc.k; ++l) {
+        ids[l] = VS_MISS;
+        if (!((lmask >> l) & 1u)) continue;
+        const unsigned long long key = keys[pix0 + (size_t)l * plane];
+        if (!key) continue;
+        keys[pix0 + (size_t)l * plane] = 0ull;   // cleared for the next pass over this buffer, as k_shade does
+        if (!alive) continue;
+        const uint32_t lid = 0xFFFFFFFFu - (uint32_t)key;
+        float s[4], uv[2];
+        vs_plain_logits<F16>(sc, vv, l, lid, px, py, Y, s, uv);
+        ids[l] = lid;
+        rgb[l][0] = vs_sigmoid(s[0]); rgb[l][1] = vs_sigmoid(s[1]); rgb[l][2] = vs_sigmoid(s[2]);
+        sig3[l] = vs_sigmoid(s[3]);
+        aw[l] = fr.attenuate ? vs_alpha_w(vx, vy, vz, sc.tri_nrm[sc.tri_off[l] + lid]) : 1.0f;
+        Tl[l] = Tr;
+        used |= 1u << l;
+        Tr *= (1.0f - sig3[l] * aw[l]);
+        if (Tr < fr.t_min) alive = false;
+    }
+    if (!used) return;
+
+    // pass 2: backward, back to front
+    const float4 g = reinterpret_cast<const float4*>(grad_out)[((size_t)view * H + py) * W + px];
+    float R = fr.bg[0] * g.x + fr.bg[1] * g.y + fr.bg[2] * g.z - g.w;
+    for (int l = (int)sc.k - 1; l >= 0; --l) {
+        if (!((used >> l) & 1u)) continue;
+        const float A = sig3[l] * aw[l];
+        const float cg = rgb[l][0] * g.x + rgb[l][1] * g.y + rgb[l][2] * g.z;
+        const float TA = Tl[l] * A;
+        float ds[4];
+        ds[0] = TA * g.x * rgb[l][0] * (1.0f - rgb[l][0]);
+        ds[1] = TA * g.y * rgb[l][1] * (1.0f - rgb[l][1]);
+        ds[2] = TA * g.z * rgb[l][2] * (1.0f - rgb[l][2]);
+        ds[3] = Tl[l] * (cg - R) * aw[l] * sig3[l] * (1.0f - sig3[l]);
+        R = A * cg + (1.0f - A) * R;
+        // footprint of the fragment (same arithmetic as the forward)
+        const uint4 tri = __ldg(&sc.tris[sc.tri_off[l] + ids[l]]);
+        float u0, du, v0, dv;
+        vs_fragment_uv(sc, vv, tri, px, py, u0, du, v0, dv);
+        const int Wt = (int)sc.tex_w[l], Ht = (int)sc.tex_h[l];
+        uint32_t cx0, cx1, cy0, cy1;
+        float fa, fb;
+        vs_texel_coord(u0, du, (float)Wt, Wt, cx0, cx1, fa);
+        vs_texel_coord(v0, dv, (float)Ht, Ht, cy0, cy1, fb);
+        const size_t texel[4] = {(size_t)cy0 * Wt + cx0, (size_t)cy0 * Wt + cx1, (size_t)cy1 * Wt + cx0, (size_t)cy1 * Wt + cx1};
+        const float ws[4] = {(1.0f - fa) * (1.0f - fb), fa * (1.0f - fb), (1.0f - fa) * fb, fa * fb};
+        float* __restrict__ gl = gt.p[l];
+        for (int q = 0; q < 4; ++q) {
+            float* gq = gl + texel[q] * (size_t)(4 * sc.n_coef);
+            for (uint32_t c = 0; c < sc.n_coef; ++c) {
+                const float wy = ws[q] * Y[c];
+                vs_red_add4(gq + 4 * c, wy * ds[0], wy * ds[1], wy * ds[2], wy * ds[3]);
+            }
+        }
+    }
+}
+
+cudaError_t vs_launch_backward(const VsSceneDev& sc, int f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
+{
+    dim3 grid(fr.tiles_x * fr.tiles_y, ch.views);
+    if (f16) k_backward<1><<<grid, 256, 0, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_mask, ch.keys, ch.grad_out, ch.grad_tex);
+    else k_backward<0><<<grid, 256, 0, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_mask, ch.keys, ch.grad_out, ch.grad_tex);
+    return cudaGetLastError();
+}

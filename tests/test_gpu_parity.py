@@ -232,6 +232,76 @@ def test_aov_reduced_config4(env, banded):
     check_aov(env, sc, range(3), attenuation=True, views_per_chunk=2)
 
 
+# ---- backward pass to the texels through vs_render_backward ----
+def check_backward(env, sc, views, attenuation=False, t_min=None, background=None, views_per_chunk=0):
+    """GPU gradient textures (fp32 atomics, any order) against the oracle's fp64 ones: max abs error <= 1e-4 of the
+    largest gradient magnitude of the layer + exact zeros where the oracle has exact zeros."""
+    if env.path_flags:
+        pytest.skip("vs_render_backward runs on the direct raster path only")
+    b, torch = env.binding, env.torch
+    rng = np.random.default_rng(21)
+    B, H, W = len(views), sc.height, sc.width
+    g = rng.normal(size=(B, H, W, 4)).astype(np.float32)
+    t_min = sc.t_min if t_min is None else t_min
+    background = sc.background if background is None else background
+    p = b.make_params(W, H, sc.near_plane, t_min, background, b.VS_FLAG_ATTENUATION if attenuation else 0, views_per_chunk)
+    r = b.Renderer(sc)
+    grads = [torch.zeros(ly.texture.shape, dtype=torch.float32, device="cuda") for ly in sc.layers]
+    b.vs_render_backward(r.handle, sc.cameras[list(views)], p, torch.from_numpy(g).cuda(), grads)
+    torch.cuda.synchronize()
+    # the scene is untouched by the backward call: a forward render afterwards still matches the oracle
+    rgba, ids = r.render(sc.cameras[list(views)], p, want_ids=True)
+    torch.cuda.synchronize()
+    r.close()
+    want = None
+    for n, v in enumerate(views):
+        ref = env.oracle.render_scene(sc, [v], t_min=t_min, background=background, attenuation=attenuation)[0]
+        assert np.array_equal(ids[n].cpu().numpy().view(np.uint32), ref["ids"])
+        want = env.oracle.render_backward(sc.layers, sc.sh_degree, sc.cameras[v], W, H, ref["ids"], g[n].astype(np.float64),
+                                          want, near_plane=sc.near_plane, t_min=t_min, background=background,
+                                          attenuation=attenuation)
+    worst = 0.0
+    for l in range(sc.k):
+        got = grads[l].cpu().numpy().astype(np.float64)
+        scale = max(np.abs(want[l]).max(), 1e-30)
+        err = np.abs(got - want[l]).max() / scale
+        worst = max(worst, err)
+        assert err <= 1e-4, "layer %d: relative gradient error %.3e" % (l, err)
+        assert np.all(got[want[l] == 0.0] == 0.0)
+    return worst, want
+
+
+def test_backward_config1(env):
+    sc = env.synth.make_config(1)
+    worst, want = check_backward(env, sc, range(4), views_per_chunk=3)
+    assert all(np.abs(w).max() > 1e-2 for w in want)
+    check_backward(env, sc, [2], attenuation=True, background=(0.3, 0.6, 0.1), t_min=0.0)
+    print("C1 backward: worst relative gradient error %.3e" % worst)
+
+
+def test_backward_reduced_config4_fp16(env):
+    sc = env.synth.make_config(4, mesh_n=48, width=320, height=180, tex_size=128, num_cameras=3, k=9)
+    worst, _ = check_backward(env, sc, range(3), views_per_chunk=2)
+    print("C4 reduced backward: worst relative gradient error %.3e" % worst)
+
+
+def test_backward_early_exit_and_errors(env):
+    b, torch = env.binding, env.torch
+    sc = env.synth.make_config(1, width=100, height=60, num_cameras=1, tex_size=64)
+    for ly in sc.layers:
+        ly.texture[:, :, 0, 3] += 60.0                      # opaque outer layer: nothing behind it gets a gradient
+    _, want = check_backward(env, sc, [0], t_min=2.0 ** -6)
+    assert np.all(want[1] == 0.0) and np.all(want[2] == 0.0) and np.abs(want[0]).max() > 1e-3
+    if not env.path_flags:
+        banded = env.synth.make_config(1, width=32, height=32, num_cameras=1, banded=True)
+        r = b.Renderer(banded)
+        with pytest.raises(b.VsError) as e:
+            b.vs_render_backward(r.handle, banded.cameras, b.make_params(32, 32), torch.zeros((1, 32, 32, 4), device="cuda"),
+                                 [torch.zeros((1,), device="cuda")] * 3)
+        assert e.value.status == b.VS_ERR_UNSUPPORTED
+        r.close()
+
+
 def test_determinism_and_chunking(env):
     sc = env.synth.make_config(2, mesh_n=30, width=200, height=150, tex_size=128, num_cameras=6)
     a = gpu_render(env, sc, range(6), views_per_chunk=1)
