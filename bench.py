@@ -175,8 +175,26 @@ def run_ours(args):
     b_fb = W * H * 16 * B
     alg_bytes_step = b_tex + b_geom + b_fb
 
+    if args.backward:
+        # step = one vs_render_backward call (S1-S4 + k_backward) over the batch; the fp32 gradient textures are
+        # accumulated into across steps (zeroed once, outside the timed region)
+        gen = torch.Generator(device=dev).manual_seed(1234)
+        gout = torch.randn((B, H, W, 4), dtype=torch.float32, device=dev, generator=gen)
+        grads = [torch.zeros(ly.texture.shape, dtype=torch.float32, device=dev) for ly in sc.layers]
+        b_grad = cstats["unique_texels"] * sc.n_coef * 16 * 2          # fp32 gradient texel read + written once per view
+        b_fb = W * H * 16 * B                                           # the upstream gradient is read instead of an image written
+        alg_bytes_step = b_tex + b_grad + b_geom + b_fb
+
+        def run_step():
+            binding.vs_render_backward(renderer.handle, sc.cameras, params, gout, grads)
+    else:
+        b_grad = 0
+
+        def run_step():
+            binding.vs_render(renderer.handle, sc.cameras, params, out)
+
     for _ in range(max(args.warmup, 0)):
-        binding.vs_render(renderer.handle, sc.cameras, params, out)
+        run_step()
     torch.cuda.synchronize()
 
     sampler = ClockSampler(local) if rank == 0 else None
@@ -187,7 +205,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     ev0.record(stream)
     for _ in range(args.steps):
-        binding.vs_render(renderer.handle, sc.cameras, params, out)
+        run_step()
         st = renderer.stats()                      # per-kernel CUDA-event times of the finished call
         shade_ms += st["ms_shade"]; raster_ms += st["ms_raster"]; bin_ms += st["ms_binning"]; xf_ms += st["ms_transform"]
         shade_launches += st["shade_launches"]; launches += st["kernel_launches"]
@@ -224,12 +242,12 @@ def run_ours(args):
     # bytes are B_tex + B_fb of the views one launch processes (B_geom belongs to the geometry kernels
     # and is counted in `whole_step`, which divides ALL algorithmic bytes by the whole step's time).
     per_launch_ms = shade_ms / max(shade_launches, 1)
-    bytes_per_launch = (b_tex + b_fb) * args.steps / max(shade_launches, 1)
+    bytes_per_launch = (b_tex + b_grad + b_fb) * args.steps / max(shade_launches, 1)
     achieved = bytes_per_launch / (per_launch_ms * 1e-3) / 1e9 if per_launch_ms > 0 else 0.0
     step_achieved = alg_bytes_step * world / (secs_max / args.steps) / 1e9
-    roofline = {"bound": "hbm", "kernel": "k_shade", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"bound": "hbm", "kernel": "k_backward" if args.backward else "k_shade", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": (NCU_TRAFFIC_BYTES_PER_VIEW[args.config] * B * args.steps / max(shade_launches, 1)
-                            if args.config in NCU_TRAFFIC_BYTES_PER_VIEW and not args.tiled else None),
+                            if args.config in NCU_TRAFFIC_BYTES_PER_VIEW and not (args.tiled or args.backward or args.attenuation) else None),
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_per_launch,
                 "launch_ms": per_launch_ms, "views_per_launch": B * args.steps / max(shade_launches, 1),
                 "kernel_share_of_step": shade_ms / (secs * 1e3),
@@ -277,6 +295,7 @@ def run_ours(args):
                        "raster_path": "tiled (binning + per-tile shared-memory keys)" if args.tiled
                        else "direct (triangle-parallel, 64-bit max keys in HBM/L2)",
                        "attenuation": bool(args.attenuation),
+                       "pass": "backward to texels (vs_render_backward)" if args.backward else "forward (vs_render)",
                        "parallelism": "views sharded, scene replicated (dp%d)" % world,
                        "l2": "no flush: %.2f GiB of textures streamed per step >> 126 MB L2" % (
                            sum(sum(t.nbytes for t in ly.band_textures) if banded else ly.texture.nbytes for ly in sc.layers) / 2 ** 30),
@@ -302,6 +321,7 @@ def main():
     ap.add_argument("--chunk", type=int, default=0, help="views per internal pass (0 = automatic)")
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="oracle work of the cpu_baseline sample (whole views)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--backward", action="store_true", help="time vs_render_backward (gradients to the texels, PAPER.md:L441-443) instead of vs_render (not the headline workload)")
     ap.add_argument("--banded", action="store_true", help="the paper's 8-bit mixed-resolution textures on the same geometry (PAPER.md:L445-459; not the headline workload)")
     ap.add_argument("--attenuation", action="store_true", help="render with VS_FLAG_ATTENUATION (PAPER.md:L279-286; not the headline workload)")
     ap.add_argument("--tiled", action="store_true", help="time the per-tile raster path (VS_FLAG_TILED_PATH) instead of the default direct one")

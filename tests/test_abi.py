@@ -29,6 +29,9 @@ def test_struct_layouts_match_header():
     assert C.sizeof(binding.vs_layer_desc) == 56
     assert C.sizeof(binding.vs_scene_desc) == 24
     assert C.sizeof(binding.vs_render_stats) == 104
+    assert C.sizeof(binding.vs_layer_desc_banded) == 104      # 5 geometry fields (40) + 4 pointers + 2 x 4 uint32
+    assert C.sizeof(binding.vs_scene_desc_banded) == 32
+    assert C.sizeof(binding.vs_aov_buffers) == 32
 
 
 def test_argument_validation_happens_before_any_cuda_work():
