@@ -1,7 +1,7 @@
 // vs_plain.cuh -- plain (one thread per fragment, no cooperation) S5-S6 for every texture format: the four channel
 // logits of the fragment of triangle `lid` of layer l at pixel (px, py).  Used by the brute-force kernel
 // (VS_FLAG_REFERENCE_PATH) and by the per-layer render-buffer kernel (vs_render_aov); same arithmetic contract
-// as the fast kernels, written for clarity, not speed.
+// as the fast kernels, written for clarity first (16-byte texel loads, nothing else).
 #pragma once
 #include "vs_common.cuh"
 
@@ -44,15 +44,31 @@ __device__ inline void vs_plain_logits(const VsSceneDev& sc, const int4* __restr
     const uint32_t nv = sc.texel_vecs;
     const uint32_t offs[4] = {(f.cy0 * Wt + f.cx0) * nv, (f.cy0 * Wt + f.cx1) * nv, (f.cy1 * Wt + f.cx0) * nv, (f.cy1 * Wt + f.cx1) * nv};
     const float ws[4] = {(1.0f - f.a) * (1.0f - f.b), f.a * (1.0f - f.b), (1.0f - f.a) * f.b, f.a * f.b};
-    for (uint32_t c = 0; c < sc.n_coef; ++c)
-        for (int ch = 0; ch < 4; ++ch) {
-            float v = 0.0f;
-            for (int q = 0; q < 4; ++q) {
-                float tv;
-                if (F16) tv = __half2float(reinterpret_cast<const __half*>(sc.tex[l] + offs[q])[ch * sc.np_pad + c]);
-                else tv = reinterpret_cast<const float*>(sc.tex[l] + offs[q])[ch * sc.np_pad + c];
-                v += ws[q] * tv;
+    // internal texel layout [ch][np_pad]: 16-byte vectors of consecutive coefficients of one channel
+    const uint32_t vpc = nv >> 2;   // vectors per channel
+    for (int ch = 0; ch < 4; ++ch)
+        for (uint32_t v = 0; v < vpc; ++v) {
+            uint4 t[4];
+            for (int q = 0; q < 4; ++q) t[q] = __ldg(sc.tex[l] + offs[q] + ch * vpc + v);
+            constexpr int EPV = F16 ? 8 : 4;
+#pragma unroll
+            for (int e = 0; e < EPV; ++e) {
+                const uint32_t c = v * EPV + e;
+                if (c >= sc.n_coef) break;   // zero padding
+                float val = 0.0f;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t w = (F16 ? (e >> 1) : e) == 0 ? t[q].x : (F16 ? (e >> 1) : e) == 1 ? t[q].y : (F16 ? (e >> 1) : e) == 2 ? t[q].z : t[q].w;
+                    float tv;
+                    if (F16) {
+                        const __half2 h = *reinterpret_cast<const __half2*>(&w);
+                        tv = (e & 1) ? __high2float(h) : __low2float(h);
+                    } else {
+                        tv = __uint_as_float(w);
+                    }
+                    val += ws[q] * tv;
+                }
+                s[ch] += Y[c] * val;
             }
-            s[ch] += Y[c] * v;
         }
 }
