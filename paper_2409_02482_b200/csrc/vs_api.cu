@@ -567,6 +567,8 @@ extern "C" vs_status vs_render_backward(vs_scene* scene, const vs_camera* camera
     VsGradTex gt{};
     for (uint32_t l = 0; l < scene->dev.k; ++l) {
         if (!grad_textures[l]) return fail(VS_ERR_INVALID_ARG, "grad_textures[%u] is NULL", l);
+        if ((uint64_t)scene->dev.tex_w[l] * scene->dev.tex_h[l] * scene->dev.n_coef >= (1ull << 32))
+            return fail(VS_ERR_UNSUPPORTED, "layer %u: gradient texture too large", l);
         gt.p[l] = grad_textures[l];
     }
     cudaStream_t st = (cudaStream_t)cuda_stream;
