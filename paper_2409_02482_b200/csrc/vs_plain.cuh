@@ -45,20 +45,29 @@ __device__ inline void vs_plain_logits(const VsSceneDev& sc, const int4* __restr
     const uint32_t offs[4] = {(f.cy0 * Wt + f.cx0) * nv, (f.cy0 * Wt + f.cx1) * nv, (f.cy1 * Wt + f.cx0) * nv, (f.cy1 * Wt + f.cx1) * nv};
     const float ws[4] = {(1.0f - f.a) * (1.0f - f.b), f.a * (1.0f - f.b), (1.0f - f.a) * f.b, f.a * f.b};
     // internal texel layout [ch][np_pad]: 16-byte vectors of consecutive coefficients of one channel
-    const uint32_t vpc = nv >> 2;   // vectors per channel
-    for (int ch = 0; ch < 4; ++ch)
-        for (uint32_t v = 0; v < vpc; ++v) {
-            uint4 t[4];
-            for (int q = 0; q < 4; ++q) t[q] = __ldg(sc.tex[l] + offs[q] + ch * vpc + v);
+    const uint32_t vpc = nv >> 2;   // vectors per channel: 1, 2 or 4
+#pragma unroll 1
+    for (int ch = 0; ch < 4; ++ch) {
+        // all vectors of this channel row of the four texels are requested before the first is used
+        uint4 t[4][4];
+#pragma unroll
+        for (int v = 0; v < 4; ++v)
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+                t[v][q] = (uint32_t)v < vpc ? __ldg(sc.tex[l] + offs[q] + ch * vpc + v) : make_uint4(0, 0, 0, 0);
+        float acc = 0.0f;
+#pragma unroll
+        for (int v = 0; v < 4; ++v) {
             constexpr int EPV = F16 ? 8 : 4;
 #pragma unroll
             for (int e = 0; e < EPV; ++e) {
-                const uint32_t c = v * EPV + e;
-                if (c >= sc.n_coef) break;   // zero padding
+                const int c = v * EPV + e;                     // zero padding adds 0
+                if ((uint32_t)v >= vpc || c >= VS_MAX_COEF) continue;
                 float val = 0.0f;
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    const uint32_t w = (F16 ? (e >> 1) : e) == 0 ? t[q].x : (F16 ? (e >> 1) : e) == 1 ? t[q].y : (F16 ? (e >> 1) : e) == 2 ? t[q].z : t[q].w;
+                    const int wi = F16 ? (e >> 1) : e;
+                    const uint32_t w = wi == 0 ? t[v][q].x : wi == 1 ? t[v][q].y : wi == 2 ? t[v][q].z : t[v][q].w;
                     float tv;
                     if (F16) {
                         const __half2 h = *reinterpret_cast<const __half2*>(&w);
@@ -68,7 +77,9 @@ __device__ inline void vs_plain_logits(const VsSceneDev& sc, const int4* __restr
                     }
                     val += ws[q] * tv;
                 }
-                s[ch] += Y[c] * val;
+                acc += ((uint32_t)c < sc.n_coef ? Y[c] : 0.0f) * val;
             }
         }
+        s[ch] = acc;
+    }
 }
