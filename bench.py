@@ -303,7 +303,8 @@ def run_ours(args):
                        "tile_refs_per_view": cstats["tile_refs"] / B},
             "clocks": clocks, "roofline": roofline, "cpu_baseline": cpu_baseline,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(sc.cameras.nbytes),
-                    "d2h_bytes_per_step": int(host_out.numel() * 4), "steps": e2e_steps},
+                    "d2h_bytes_per_step": int(host_out.numel() * 4), "steps": e2e_steps,
+                    "pass": "forward (vs_render_host)"},
             "gpu_launches": int(launches)}
     print(json.dumps(line))
     renderer.close()

@@ -20,7 +20,7 @@ __device__ __forceinline__ void vs_red_add4(float* p, float a, float b, float c,
 }
 
 template <int F16>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, 3)
 k_backward(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams, const int4* __restrict__ vtx,
            const uint32_t* __restrict__ tile_mask, unsigned long long* __restrict__ keys, const float* __restrict__ grad_out,
            VsGradTex gt)
