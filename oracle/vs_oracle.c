@@ -25,8 +25,12 @@
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): closed-form full-screen quad; hand-counted top-left
  * fixtures (tests/golden/); double-precision ray-triangle brute force; scipy sph_harm; torch
  * grid_sample; numpy float16; SPEC.md:L478 blend example; analytic constant-layer compositing;
- * depth-sorted blend equivalence.  No function here is "parity unpinned" except the choice of a
- * sigmoid on the colour channels (reading Q2 in DESIGN.md), which the paper does not state.
+ * depth-sorted blend equivalence; attenuation: SPEC.md:L468-470 values, tanh(5x), closed-form tilted quads;
+ * banded 8-bit format: SPEC.md:L361-378 values, grid_sample per band, float-twin renders, affine mixed-resolution
+ * bands; render buffers: closed-form quad, sphere normals; backward: central finite differences of the forward.
+ * "Parity unpinned" by the paper (readings): the sigmoid on the colour channels (Q2), the SH sign
+ * convention (Q3), which normal the transparency attenuation uses (Q13: the geometric face normal) and the raw
+ * (unencoded) form of the render buffers (Q13b) -- each is pinned only against its own stated definition.
  */
 #include <math.h>
 #include <stdint.h>
