@@ -138,6 +138,39 @@ def test_config4_full_banded(env):
     print("C4 full size, banded: worst rgba err %.3e" % worst)
 
 
+def test_config4_backward_full_resolution(env):
+    """SURVEY.md §8(f) NEXT-4 at the headline geometry, image size and layer count (k = 9, ~300k triangles per layer,
+    1920x1080): vs_render_backward over two views against the oracle's fp64 gradients.  Textures are 512^2 here (the
+    oracle's fp64 gradient textures of the 2048^2 scene would take 19 GB): magnified texels, so thousands of fragments
+    reduce into the same gradient texel -- the hard case for the atomic scatter."""
+    b, torch = env.binding, env.torch
+    sc = env.synth.make_config(4, tex_size=512, num_cameras=64)
+    views = [0, 63]
+    W, H = sc.width, sc.height
+    g = np.random.default_rng(33).normal(size=(len(views), H, W, 4)).astype(np.float32)
+    r = b.Renderer(sc)
+    p = b.make_params(W, H, sc.near_plane, sc.t_min, sc.background)
+    grads = [torch.zeros(ly.texture.shape, dtype=torch.float32, device="cuda") for ly in sc.layers]
+    b.vs_render_backward(r.handle, sc.cameras[views], p, torch.from_numpy(g).cuda(), grads)
+    torch.cuda.synchronize()
+    r.close()
+    want = None
+    for n, v in enumerate(views):
+        ref = env.oracle.render_scene(sc, [v])[0]
+        want = env.oracle.render_backward(sc.layers, sc.sh_degree, sc.cameras[v], W, H, ref["ids"], g[n].astype(np.float64), want,
+                                          near_plane=sc.near_plane, t_min=sc.t_min, background=sc.background)
+    worst = 0.0
+    for l in range(sc.k):
+        got = grads[l].cpu().numpy().astype(np.float64)
+        scale = np.abs(want[l]).max()
+        assert scale > 1e-2
+        err = np.abs(got - want[l]).max() / scale
+        worst = max(worst, err)
+        assert err <= 1e-4, "layer %d: relative gradient error %.3e" % (l, err)
+        assert np.all(got[want[l] == 0.0] == 0.0)
+    print("C4 geometry at 1920x1080, 512^2 textures, backward over 2 views: worst relative gradient error %.3e" % worst)
+
+
 def test_config5_full(env):
     # even views are far cameras (r = 3), odd views close-ups (r = 1.6) that fill the frame
     _check_config(env, 5, [0, 1, 15], [0, 1])
