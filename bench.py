@@ -52,7 +52,7 @@ def geometry_bytes_per_view(sc):
 
 
 class ClockSampler:
-    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+    FIELDS = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
               "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
               "clocks_event_reasons.sw_power_cap")
 
@@ -61,12 +61,15 @@ class ClockSampler:
         self.proc = None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", "-i", str(gpu_index), "--query-gpu=" + self.FIELDS,
-                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                          "--format=csv,noheader,nounits", "-lms", "20"],
                                          stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
         except Exception:
             self.proc = None
 
-    def stop(self):
+    def stop(self, t0=None, t1=None):
+        """Median SM clock, maximum clock, power and throttle reasons of the samples taken between the wall-clock times
+        t0 and t1 (the timed region); the sampler is started before the warm-up so that it is already running then."""
+        import datetime
         out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
         if self.proc is None:
             return out
@@ -75,25 +78,34 @@ class ClockSampler:
             self.proc.wait(timeout=5)
         except Exception:
             self.proc.kill()
-        sm, mx, reasons, power = [], [], set(), []
+        rows = []
         try:
             for line in open(self.path):
                 f = [x.strip() for x in line.split(",")]
-                if len(f) < 8:
+                if len(f) < 9:
                     continue
                 try:
-                    sm.append(float(f[0])); mx.append(float(f[1])); power.append(float(f[2]))
+                    ts = datetime.datetime.strptime(f[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                except ValueError:
+                    ts = None
+                try:
+                    rows.append((ts, float(f[1]), float(f[2]), float(f[3]), f[5:9]))
                 except ValueError:
                     continue
-                for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), f[4:8]):
-                    if val.lower().startswith("active"):
-                        reasons.add(name)
             os.unlink(self.path)
         except Exception:
             pass
+        inside = [r for r in rows if t0 is not None and r[0] is not None and t0 - 0.02 <= r[0] <= t1 + 0.02]
+        window = "timed region" if inside else "warm-up + timed region"
+        sm, mx, reasons, power = [], [], set(), []
+        for _, a_sm, a_mx, a_pw, flags in (inside or rows):
+            sm.append(a_sm); mx.append(a_mx); power.append(a_pw)
+            for name, val in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), flags):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
         if sm:
             out = {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
-                   "samples": len(sm), "power_w_max": max(power) if power else None}
+                   "samples": len(sm), "window": window, "power_w_max": max(power) if power else None}
         return out
 
 
@@ -193,16 +205,17 @@ def run_ours(args):
         def run_step():
             binding.vs_render(renderer.handle, sc.cameras, params, out)
 
+    sampler = ClockSampler(local) if rank == 0 else None   # started before the warm-up: nvidia-smi takes a moment to come up
     for _ in range(max(args.warmup, 0)):
         run_step()
     torch.cuda.synchronize()
 
-    sampler = ClockSampler(local) if rank == 0 else None
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     shade_ms = raster_ms = bin_ms = xf_ms = 0.0
     shade_launches = launches = 0
     vsdist.barrier()
     torch.cuda.synchronize()
+    wall0 = time.time()
     ev0.record(stream)
     for _ in range(args.steps):
         run_step()
@@ -213,7 +226,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     vsdist.barrier()
     secs = ev0.elapsed_time(ev1) / 1e3
-    clocks = sampler.stop() if sampler else None
+    clocks = sampler.stop(wall0, time.time()) if sampler else None
     secs_max = vsdist.max_over_ranks(secs, dev)
     pixels_all = vsdist.sum_over_ranks(float(B * W * H * args.steps), dev)
     value = pixels_all / secs_max / 1e6
@@ -314,7 +327,7 @@ def run_ours(args):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=4, choices=[1, 2, 3, 4, 5])
