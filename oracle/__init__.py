@@ -66,6 +66,9 @@ def lib():
         L.vso_transform_vertex.argtypes = [C.c_void_p, C.c_float, C.c_void_p, C.c_void_p, C.c_void_p,
                                            C.c_void_p, C.c_void_p]
         L.vso_max_threads.restype = C.c_int
+        L.vso_count_footprints.restype = C.c_int
+        L.vso_count_footprints.argtypes = [C.POINTER(_Layer), C.c_uint32, C.c_uint32, C.c_uint32, C.c_double, C.c_void_p,
+                                           C.c_void_p, C.c_void_p, C.POINTER(C.c_void_p), C.c_void_p]
         _lib = L
     return _lib
 
@@ -192,6 +195,34 @@ def render_backward(layers, sh_degree: int, camera, width: int, height: int, ids
     if rc != 0:
         raise ValueError("vso_render_backward rejected its arguments (rc=%d)" % rc)
     return grad_tex
+
+
+def count_footprints(layers, width: int, height: int, view, *, t_min: float = 2.0 ** -14, marks=None):
+    """Footprint census of one rendered view (SURVEY.md §8(d) "counted, not assumed"): `view` is the dict returned by
+    render_view(..., want_layer_rgba=True, want_layer_uv=True) with the same t_min.  `marks`: list of uint8 [tex_h, tex_w]
+    arrays (one per layer; zeros are created if None) that accumulate the referenced texels.
+    Returns (composited_fragments, newly_marked_texels, marks)."""
+    k = len(layers)
+    arr = (_Layer * k)()
+    sizes = []
+    for i, L in enumerate(layers):
+        th, tw = (L.band_textures[0].shape[:2] if getattr(L, "band_textures", None) is not None else L.texture.shape[:2])
+        sizes.append((th, tw))
+        arr[i] = _Layer(None, None, None, None, 0, 0, tw, th)
+    if marks is None:
+        marks = [np.zeros(s, dtype=np.uint8) for s in sizes]
+    for m, s in zip(marks, sizes):
+        assert m.dtype == np.uint8 and m.flags.c_contiguous and m.shape == s
+    mptr = (C.c_void_p * k)(*[m.ctypes.data for m in marks])
+    ids = np.ascontiguousarray(view["ids"], dtype=np.uint32)
+    lrgba = np.ascontiguousarray(view["layer_rgba"], dtype=np.float64)
+    luv = np.ascontiguousarray(view["layer_uv"], dtype=np.float64)
+    assert ids.shape == (k, height, width) and lrgba.shape == (k, height, width, 4) and luv.shape == (k, height, width, 2)
+    out = np.zeros(2, dtype=np.uint64)
+    rc = lib().vso_count_footprints(arr, k, width, height, float(t_min), _ptr(ids), _ptr(lrgba), _ptr(luv), mptr, _ptr(out))
+    if rc != 0:
+        raise ValueError("vso_count_footprints rejected its arguments (rc=%d)" % rc)
+    return int(out[0]), int(out[1]), marks
 
 
 def render_scene(scene, views=None, **kw):

@@ -27,7 +27,8 @@
  * grid_sample; numpy float16; SPEC.md:L478 blend example; analytic constant-layer compositing;
  * depth-sorted blend equivalence; attenuation: SPEC.md:L468-470 values, tanh(5x), closed-form tilted quads;
  * banded 8-bit format: SPEC.md:L361-378 values, grid_sample per band, float-twin renders, affine mixed-resolution
- * bands; render buffers: closed-form quad, sphere normals; backward: central finite differences of the forward.
+ * bands; render buffers: closed-form quad, sphere normals; backward: central finite differences of the forward;
+ * footprint census (vso_count_footprints): hand-counted texels of pixel-aligned quads, early-exit and clamp cases.
  * "Parity unpinned" by the paper (readings): the sigmoid on the colour channels (Q2), the SH sign
  * convention (Q3), which normal the transparency attenuation uses (Q13: the geometric face normal) and the raw
  * (unencoded) form of the render buffers (Q13b) -- each is pinned only against its own stated definition.
@@ -617,6 +618,48 @@ int vso_render_backward(const vso_layer* layers, uint32_t k, uint32_t sh_degree,
     }
     for (uint32_t l = 0; l < k; ++l) free(vtx[l]);
     free(vtx);
+    return 0;
+}
+
+/*
+ * Footprint census of ONE rendered view -- the numerator of the roofline (B_tex = "unique texels referenced by
+ * the 2x2 footprints of *shaded* fragments ... counted, not assumed: an instrumented pass or the oracle").
+ * Inputs are what vso_render produced for the view: ids [k][H][W], layer_rgba [k][H][W][4] (alpha = the blend weight A of
+ * A.8, after alpha_w if it was enabled) and layer_uv [k][H][W][2].  Per pixel, the layers are walked in blend order with the
+ * A.8 recurrence (T *= 1 - A; stop once T < t_min): every hit layer reached before the stop -- the stopping layer included --
+ * is a COMPOSITED fragment.  Each composited fragment marks the four texels of its A.6 footprint (x = u W - 0.5, floor,
+ * clamp-to-edge; texels of weight 0 count: they are fetched) in marks[l] ([tex_h][tex_w] bytes, set to 1, never cleared
+ * here, so several views may be accumulated).  out[0] += composited fragments, out[1] += texels newly marked by this call.
+ * Returns 0, or -1 on bad arguments.
+ */
+int vso_count_footprints(const vso_layer* layers, uint32_t k, uint32_t width, uint32_t height, double t_min,
+                         const uint32_t* ids, const double* layer_rgba, const double* layer_uv, uint8_t* const* marks,
+                         uint64_t* out)
+{
+    if (!layers || k < 1 || k > VSO_MAX_LAYERS || !ids || !layer_rgba || !layer_uv || !marks || !out) return -1;
+    const size_t P = (size_t)width * height;
+    uint64_t frags = 0, fresh = 0;
+    for (size_t p = 0; p < P; ++p) {
+        double T = 1.0;
+        for (uint32_t l = 0; l < k; ++l) {
+            if (ids[(size_t)l * P + p] == VSO_MISS) continue;
+            const vso_layer* L = &layers[l];
+            frags++;
+            double u = layer_uv[((size_t)l * P + p) * 2], v = layer_uv[((size_t)l * P + p) * 2 + 1];
+            double x0 = floor(u * (double)L->tex_w - 0.5), y0 = floor(v * (double)L->tex_h - 0.5);
+            int64_t ix[2] = {clampi((int64_t)x0, 0, (int64_t)L->tex_w - 1), clampi((int64_t)x0 + 1, 0, (int64_t)L->tex_w - 1)};
+            int64_t iy[2] = {clampi((int64_t)y0, 0, (int64_t)L->tex_h - 1), clampi((int64_t)y0 + 1, 0, (int64_t)L->tex_h - 1)};
+            for (int b = 0; b < 2; ++b)
+                for (int a = 0; a < 2; ++a) {
+                    uint8_t* m = &marks[l][(size_t)iy[b] * L->tex_w + (size_t)ix[a]];
+                    if (!*m) { *m = 1; fresh++; }
+                }
+            T *= (1.0 - layer_rgba[((size_t)l * P + p) * 4 + 3]);
+            if (T < t_min) break;
+        }
+    }
+    out[0] += frags;
+    out[1] += fresh;
     return 0;
 }
 
