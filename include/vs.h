@@ -93,6 +93,10 @@ enum {
     VS_FLAG_COUNT_TEXELS   = 1u << 2, /* measurement aid: count shaded fragments and, per view, the UNIQUE
                                          texels their 2x2 footprints reference (the algorithmic texture
                                          bytes of DESIGN.md §8); slower, not for timed runs                */
+    VS_FLAG_OVERLAP        = 1u << 5, /* experiment: run S1-S4 of the next chunk of cameras on an internal
+                                         high-priority stream, in one resident CTA per SM, beside S5-S7 of the current
+                                         chunk instead of back to back on `cuda_stream`; same outputs bit for bit
+                                         (measured slower on B200; off by default)                            */
     VS_FLAG_ATTENUATION    = 1u << 4  /* transparency attenuation (§4.2 "Transparency
                                          Attenuation"): every fragment's opacity is multiplied by
                                          alpha_w = 2 Sigmoid(10 |v . n|) - 1 before blending, v = the pixel's

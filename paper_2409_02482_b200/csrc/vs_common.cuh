@@ -24,6 +24,7 @@ struct VsSceneDev {
     uint32_t k, sh_degree, n_coef;
     uint32_t texel_vecs;                  // 16-byte vectors per texel in the internal layout (= 4 * np_pad * elem / 16)
     uint32_t np_pad;                      // coefficients per channel row of the internal layout [texel][ch][np_pad]
+    uint32_t frag_layout;                 // 1: fp16 texels of 16 (padded) coefficients stored in mma A-fragment order (see below)
     uint32_t tri_off[VS_MAX_LAYERS + 1];  // global triangle id of each layer's triangle 0
     uint32_t vtx_off[VS_MAX_LAYERS + 1];  // global vertex index of each layer's vertex 0
     const uint4* tex[VS_MAX_LAYERS];      // [tex_h][tex_w][texel_vecs] 16-byte vectors
@@ -295,7 +296,7 @@ cudaError_t vs_launch_transform(const VsSceneDev& sc, const VsFrame& fr, const V
 cudaError_t vs_launch_bin_count(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_bin_scan(const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_bin_scatter(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
-cudaError_t vs_launch_raster_direct(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_raster_direct(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st, uint32_t resident_ctas);
 cudaError_t vs_launch_raster(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_shade(const VsSceneDev& sc, int tex_f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_popcount(const uint32_t* words, size_t n, unsigned long long* counter, cudaStream_t st);
@@ -310,11 +311,19 @@ cudaError_t vs_launch_backward(const VsSceneDev& sc, int f16, const VsFrame& fr,
 cudaError_t vs_launch_layer_aov(const VsSceneDev& sc, int f16, const VsFrame& fr, uint32_t views, const VsCamDev* cams, const int4* vtx,
                                 const uint32_t* ids, float* layer_rgba, float* layer_uv, float* layer_normal, cudaStream_t st);
 cudaError_t vs_launch_check_finite(const float* v, size_t n, uint32_t* error_flag, cudaStream_t st);
-cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, uint32_t n_coef, uint32_t np_pad,
+cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, uint32_t n_coef, uint32_t np_pad, uint32_t frag_layout,
                                    uint4* dst, cudaStream_t st);
 
 // Internal texel layout: [texel][ch = 0..3][np_pad] elements, channel-major, every channel row
 // padded to np_pad = 16-byte vectors-per-channel (1, 2 or 4) * elements per vector coefficients.
+// fp16 textures with np_pad == 16 (SH degree 2 and 3; VsSceneDev::frag_layout) permute the 64 halves of a texel into the
+// A-fragment order of mma.sync.m16n8k16 instead, so that lane oi = 0..7 of an octet loads the four registers of its A
+// fragment as ONE 16-byte vector: vector v = (ch & 1) * 4 + ((c & 7) >> 1), half ((c >> 3) * 2 + (ch >> 1)) * 2 + (c & 1)
+// of that vector (A row = 2 f + (ch & 1) + 8 (ch >> 1) for the fragment f of the octet, A column = c).
+__host__ __device__ inline uint32_t vs_frag_half_index(uint32_t c, uint32_t ch)
+{
+    return ((ch & 1u) * 4u + ((c & 7u) >> 1)) * 8u + ((c >> 3) * 2u + (ch >> 1)) * 2u + (c & 1u);
+}
 __host__ __device__ inline uint32_t vs_vecs_per_channel(int f16, uint32_t n_coef)
 {
     const uint32_t epv = f16 ? 8u : 4u;

@@ -77,22 +77,29 @@ __device__ __forceinline__ void vs_direct_large(int X0, int Y0, int X1, int Y1, 
     }
 }
 
-#ifndef VS_RD_MIN_CTAS
-#define VS_RD_MIN_CTAS 4
+#ifndef VS_RD_THREADS
+#define VS_RD_THREADS 256
 #endif
-__global__ void __launch_bounds__(256, VS_RD_MIN_CTAS)
+#ifndef VS_RD_MIN_CTAS
+#define VS_RD_MIN_CTAS (1024 / VS_RD_THREADS)
+#endif
+__global__ void __launch_bounds__(VS_RD_THREADS, VS_RD_MIN_CTAS)
 k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, unsigned long long* __restrict__ keys,
                 uint32_t* __restrict__ tile_mask, uint2* __restrict__ big_list, uint32_t* __restrict__ big_count, uint32_t big_capacity,
-                unsigned long long* __restrict__ counters)
+                unsigned long long* __restrict__ counters, uint32_t blocks_per_view, uint32_t total_blocks)
 {
-    __shared__ __align__(16) int slab[8 * VS_RD_WARP_WORDS];
+    __shared__ __align__(16) int slab[(VS_RD_THREADS / 32) * VS_RD_WARP_WORDS];
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t view = blockIdx.y;
-    const uint32_t gt = blockIdx.x * 256u + tid;
     const int W = (int)fr.width, H = (int)fr.height;
     const size_t plane_px = (size_t)W * H;
     int4* rec4 = reinterpret_cast<int4*>(slab + warp * VS_RD_WARP_WORDS);                 // [vector][lane]
     unsigned short* queue = reinterpret_cast<unsigned short*>(slab + warp * VS_RD_WARP_WORDS + VS_RD_FIELDS * 32);   // [512]
+    // work item = (view, block of VS_RD_THREADS consecutive triangles).  The grid either has one CTA per item or, when the
+    // kernel runs beside the previous chunk's k_shade, a few resident CTAs per SM that stride over the items
+    for (uint32_t item = blockIdx.x; item < total_blocks; item += gridDim.x) {
+    __syncwarp();   // the previous item's phase 2 has finished reading this warp's slab
+    const uint32_t view = item / blocks_per_view;
+    const uint32_t gt = (item - view * blocks_per_view) * (uint32_t)VS_RD_THREADS + tid;
     const int4* __restrict__ vv = vtx + (size_t)view * sc.v_total;
     unsigned long long* __restrict__ vkeys = keys + (size_t)view * sc.k * plane_px;
 
@@ -116,6 +123,7 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
             large = valid && !(narrow && i1 - i0 < 8 && j1 - j0 < 8);
         }
     }
+#ifndef VS_EXP_NOMASK
     {
         // layer bit of every 16x16 tile the box touches: k_shade skips the tiles and layers nothing was drawn into.
         // A warp's 32 consecutive triangles share a handful of tiles: the lanes that report the same (tile, layer)
@@ -135,6 +143,7 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
             for (int ty = ty0; ty <= ty1; ++ty)
                 for (int tx = tx0; tx <= tx1; ++tx) atomicOr(&tm[(size_t)ty * fr.tiles_x + tx], 1u << layer);
     }
+#endif
     {
         const unsigned dropped = __popc(__ballot_sync(0xFFFFFFFFu, status == 1));
         const unsigned degen = __popc(__ballot_sync(0xFFFFFFFFu, status == 2));
@@ -269,6 +278,7 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
         else if (lin) vs_direct_large<long long, true>(X0, Y0, X1, Y1, X2, Y2, q0, q1, q2, fA, bi0, bi1, bj0, bj1, W, plane, blid, lane, 0u, 1u);
         else vs_direct_large<long long, false>(X0, Y0, X1, Y1, X2, Y2, q0, q1, q2, fA, bi0, bi1, bj0, bj1, W, plane, blid, lane, 0u, 1u);
     }
+    }   // items
 }
 
 // Triangles with very large clipped boxes (full-screen quads, close-ups of coarse meshes): every entry of
@@ -300,15 +310,20 @@ k_raster_big(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx
     }
 }
 
-cudaError_t vs_launch_raster_direct(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
+cudaError_t vs_launch_raster_direct(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st, uint32_t resident_ctas)
 {
     if (sc.t_total == 0) return cudaSuccess;
     // key offsets inside one view are carried as uint32
     if ((unsigned long long)sc.k * fr.width * fr.height >= (1ull << 32)) return cudaErrorInvalidValue;
-    dim3 grid((sc.t_total + 255) / 256, ch.views);
-    k_raster_direct<<<grid, 256, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.tile_mask, ch.big_list, ch.big_count, ch.big_capacity, ch.counters);
+    const uint32_t bpv = (sc.t_total + VS_RD_THREADS - 1) / VS_RD_THREADS;
+    const unsigned long long total = (unsigned long long)bpv * ch.views;
+    if (total >= (1ull << 31)) return cudaErrorInvalidValue;
+    // resident_ctas != 0: that many CTAs stride over the work items (the kernel shares the SMs with another one)
+    const uint32_t grid = resident_ctas && resident_ctas < total ? resident_ctas : (uint32_t)total;
+    k_raster_direct<<<grid, VS_RD_THREADS, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.tile_mask, ch.big_list, ch.big_count, ch.big_capacity,
+                                                   ch.counters, bpv, (uint32_t)total);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
-    k_raster_big<<<148 * 4, 256, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.big_list, ch.big_count, ch.big_capacity);
+    k_raster_big<<<resident_ctas ? 148 : 148 * 4, 256, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.big_list, ch.big_count, ch.big_capacity);
     return cudaGetLastError();
 }

@@ -32,8 +32,9 @@ __global__ void k_check_finite(const float* __restrict__ v, size_t n, uint32_t* 
 
 // API layout [texel][c][ch] (float or half) -> internal [texel][ch][np_pad]: channel-major so that a
 // 16-byte vector holds consecutive coefficients of ONE channel; rows zero-padded to np_pad.
+// frag: the mma A-fragment order of vs_common.cuh (fp16, np_pad == 16) instead of the channel-major one.
 template <typename T>
-__global__ void k_pack_texture(const T* __restrict__ src, uint32_t n_texels, uint32_t n_coef, uint32_t np_pad,
+__global__ void k_pack_texture(const T* __restrict__ src, uint32_t n_texels, uint32_t n_coef, uint32_t np_pad, uint32_t frag,
                                T* __restrict__ dst)
 {
     const uint32_t dst_elems = 4 * np_pad, src_elems = n_coef * 4;
@@ -42,6 +43,11 @@ __global__ void k_pack_texture(const T* __restrict__ src, uint32_t n_texels, uin
         size_t texel = i / dst_elems;
         uint32_t e = (uint32_t)(i - texel * dst_elems);
         uint32_t ch = e / np_pad, c = e - ch * np_pad;
+        if (frag) {   // inverse of vs_frag_half_index
+            const uint32_t v = e >> 3, r = e & 7u;
+            ch = (v >> 2) + 2u * ((r >> 1) & 1u);
+            c = (v & 3u) * 2u + (r & 1u) + 8u * (r >> 2);
+        }
         dst[i] = c < n_coef ? src[texel * src_elems + 4 * c + ch] : T(0);
     }
 }
@@ -80,14 +86,14 @@ cudaError_t vs_launch_check_finite(const float* v, size_t n, uint32_t* error_fla
     return cudaGetLastError();
 }
 
-cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, uint32_t n_coef, uint32_t np_pad,
+cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, uint32_t n_coef, uint32_t np_pad, uint32_t frag_layout,
                                    uint4* dst, cudaStream_t st)
 {
     const int blocks = 148 * 16;
     if (f16)
-        k_pack_texture<__half><<<blocks, 256, 0, st>>>((const __half*)src, n_texels, n_coef, np_pad, (__half*)dst);
+        k_pack_texture<__half><<<blocks, 256, 0, st>>>((const __half*)src, n_texels, n_coef, np_pad, frag_layout, (__half*)dst);
     else
-        k_pack_texture<float><<<blocks, 256, 0, st>>>((const float*)src, n_texels, n_coef, np_pad, (float*)dst);
+        k_pack_texture<float><<<blocks, 256, 0, st>>>((const float*)src, n_texels, n_coef, np_pad, 0u, (float*)dst);
     return cudaGetLastError();
 }
 

@@ -33,6 +33,27 @@ __device__ __forceinline__ void vs_prefetch_l2(const void* p)
 {
     asm volatile("prefetch.global.L2 [%0];" ::"l"(p));
 }
+#ifndef VS_SHADE_PFMODE
+#define VS_SHADE_PFMODE 0     // 0: one prefetch.global.L2 per texel; 1: one bulk prefetch per footprint row; 2: same, 256-byte aligned blocks
+#endif
+__device__ __forceinline__ void vs_prefetch_l2_bulk(const void* p, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes));
+}
+__device__ __forceinline__ uint4 vs_ldg_tex(const char* base, uint32_t vec_off, int slot)
+{
+#ifdef VS_EXP_TEXMASK   // timing experiment only (wrong images): confine the texel addresses to a cache-resident window
+    vec_off &= (uint32_t)VS_EXP_TEXMASK;
+#endif
+    const uint4* p = reinterpret_cast<const uint4*>(base + (unsigned long long)vec_off * 16ull) + slot;
+#ifdef VS_SHADE_LD256
+    uint4 r;
+    asm volatile("ld.global.nc.L2::256B.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(r.x), "=r"(r.y), "=r"(r.z), "=r"(r.w) : "l"(p));
+    return r;
+#else
+    return __ldg(p);
+#endif
+}
 
 // ---- packed fp32 pairs (sm_100: FFMA2 / FMUL2) -------------------------------------------------
 typedef unsigned long long f32x2;
@@ -92,13 +113,34 @@ struct VsShadeShape {
     static constexpr int NACT = NVEC / SLOTS;                          // octet lanes that hold data (4 or 8)
     static constexpr int NE = SLOTS * EPV;                             // coefficients per lane (4 or 8)
     static constexpr int PPV = EPV / 2;                                // fp32 pairs per vector
+    // fp16 texels of 16 (padded) coefficients: stored in mma A-fragment order (VsSceneDev::frag_layout) and contracted on
+    // the tensor cores, 4 fragments x 4 channels x 16 coefficients per mma.sync.m16n8k16
+    static constexpr bool MMA = F16 && NCOEF > 8;
 };
 
-template <int F16, int DEG, bool COUNT>
-#ifndef VS_SHADE_MIN_CTAS
-#define VS_SHADE_MIN_CTAS 3
+// D (16x8, fp32) = A (16x16, fp16, row) x B (16x8, fp16, col), C = 0
+__device__ __forceinline__ void vs_mma_16816(float& d0, float& d1, float& d2, float& d3, const uint4& a, uint32_t b0, uint32_t b1)
+{
+    asm volatile("mma.sync.aligned.m16n8k16.row.col.f32.f16.f16.f32 {%0, %1, %2, %3}, {%4, %5, %6, %7}, {%8, %9}, {%10, %10, %10, %10};"
+                 : "=f"(d0), "=f"(d1), "=f"(d2), "=f"(d3)
+                 : "r"(a.x), "r"(a.y), "r"(a.z), "r"(a.w), "r"(b0), "r"(b1), "f"(0.0f));
+}
+
+// A CTA shades a 16-pixel-wide strip of VS_SHADE_WARPS / 2 warp rows (8x4-pixel warp blocks) of one 16x16 mask tile:
+// 8 warps = the whole tile, 4 warps = its upper or lower half (smaller CTAs pack the register file more tightly).
+#ifndef VS_SHADE_WARPS
+#define VS_SHADE_WARPS 8
 #endif
-__global__ void __launch_bounds__(256, VS_SHADE_MIN_CTAS)
+#ifndef VS_SHADE_MIN_CTAS
+#define VS_SHADE_MIN_CTAS (24 / VS_SHADE_WARPS)
+#endif
+#ifndef VS_SHADE_DEPTH
+#define VS_SHADE_DEPTH 2      // register buffers of texel vectors per lane (one is being consumed)
+#endif
+#define VS_SHADE_PIX (VS_SHADE_WARPS * 32)
+#define VS_SHADE_SUBTILES (8 / VS_SHADE_WARPS)
+template <int F16, int DEG, bool COUNT>
+__global__ void __launch_bounds__(VS_SHADE_PIX, VS_SHADE_MIN_CTAS)
 k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams, const int4* __restrict__ vtx,
         const uint32_t* __restrict__ tile_off, const uint32_t* __restrict__ ids, unsigned long long* __restrict__ keys,
         uint32_t* __restrict__ out_ids, float* __restrict__ out_rgba,
@@ -108,18 +150,18 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     constexpr int SLOTS = S::SLOTS, LPC = S::LPC, NACT = S::NACT, NE = S::NE, PPV = S::PPV;
 
     extern __shared__ __align__(16) unsigned char smem[];
-    // [k][256] packed texel coordinates, then [k][256] float2 fractions (a < 0: no fragment)
+    // [k][pixels] packed texel coordinates, then [k][pixels] float2 fractions (a < 0: no fragment)
     uint32_t* rec_xy = reinterpret_cast<uint32_t*>(smem);
-    float2* rec_ab = reinterpret_cast<float2*>(smem + (size_t)sc.k * VS_TILE_PIX * 4);
-    unsigned char* per_warp = smem + (size_t)sc.k * VS_TILE_PIX * 12;  // 8 x (2 KB basis + 1 KB records + 512 B logits)
-    float* rec_aw = reinterpret_cast<float*>(per_warp + 8 * 3584);      // [k][256] attenuation weights (only if fr.attenuate)
+    float2* rec_ab = reinterpret_cast<float2*>(smem + (size_t)sc.k * VS_SHADE_PIX * 4);
+    unsigned char* per_warp = smem + (size_t)sc.k * VS_SHADE_PIX * 12;  // per warp: 2 KB basis + 1 KB records + 512 B logits
+    float* rec_aw = reinterpret_cast<float*>(per_warp + VS_SHADE_WARPS * 3584);   // [k][pixels] attenuation weights (only if fr.attenuate)
 
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t tile = blockIdx.x, view = blockIdx.y;
+    const uint32_t tile = blockIdx.x / VS_SHADE_SUBTILES, sub = blockIdx.x % VS_SHADE_SUBTILES, view = blockIdx.y;
     const uint32_t tiles = fr.tiles_x * fr.tiles_y;
     const int W = (int)fr.width, H = (int)fr.height;
     // lane -> pixel of the warp's 8x4 block: column = lane & 7, row = lane >> 3
-    const int lx = (int)(warp & 1) * 8 + (int)(lane & 7), ly = (int)(warp >> 1) * 4 + (int)(lane >> 3);
+    const int lx = (int)(warp & 1) * 8 + (int)(lane & 7), ly = (int)(sub * (VS_SHADE_WARPS / 2) + (warp >> 1)) * 4 + (int)(lane >> 3);
     const int px = (int)(tile % fr.tiles_x) * VS_TILE_W + lx, py = (int)(tile / fr.tiles_x) * VS_TILE_H + ly;
     const bool inimg = px < W && py < H;
     const size_t pix = ((size_t)view * H + py) * W + px;
@@ -170,7 +212,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
 #pragma unroll
             for (int u = 0; u < VS_MAX_LAYERS; ++u)
                 if (u < (int)sc.k && id[u] != VS_MISS)
-                    rec_aw[u * VS_TILE_PIX + tid] = vs_alpha_w(vx, vy, vz, __ldg(&sc.tri_nrm[sc.tri_off[u] + id[u]]));
+                    rec_aw[u * VS_SHADE_PIX + tid] = vs_alpha_w(vx, vy, vz, __ldg(&sc.tri_nrm[sc.tri_off[u] + id[u]]));
         }
 #pragma unroll
         for (int u = 0; u < VS_MAX_LAYERS; ++u) {
@@ -184,23 +226,39 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
                     ab = make_float2(f.a, f.b);
                     any_hit = true;
                 }
-                rec_xy[u * VS_TILE_PIX + tid] = xy;
-                rec_ab[u * VS_TILE_PIX + tid] = ab;
+                rec_xy[u * VS_SHADE_PIX + tid] = xy;
+                rec_ab[u * VS_SHADE_PIX + tid] = ab;
             }
         }
     }
     // each thread reads back only its own records: no barrier needed
     // pull the footprint of this pixel in layer `ln` into L2 (issued VS_SHADE_PF_DIST layers ahead of its use)
     auto prefetch_layer = [&](uint32_t ln) {
-        const float2 abn = rec_ab[ln * VS_TILE_PIX + tid];
+#ifdef VS_EXP_TEXMASK
+        return;
+#endif
+        const float2 abn = rec_ab[ln * VS_SHADE_PIX + tid];
         if (abn.x >= 0.0f) {
-            const uint32_t xy = rec_xy[ln * VS_TILE_PIX + tid];
+            const uint32_t xy = rec_xy[ln * VS_SHADE_PIX + tid];
             const uint32_t cx0 = xy & 0x7FFFu, cy0 = (xy >> 16) & 0x7FFFu, Wt = sc.tex_w[ln];
             const uint4* p0 = sc.tex[ln] + (size_t)(cy0 * Wt + cx0) * S::NVEC;
             const uint4* p1 = p0 + ((xy >> 31) ? (size_t)Wt * S::NVEC : (size_t)0);
             const uint32_t dx = ((xy >> 15) & 1u) * S::NVEC;
-            vs_prefetch_l2(p0); vs_prefetch_l2(p1);
-            if (VS_SHADE_PREFETCH > 1) { vs_prefetch_l2(p0 + dx); vs_prefetch_l2(p1 + dx); }
+            if (VS_SHADE_PFMODE == 0) {
+                vs_prefetch_l2(p0); vs_prefetch_l2(p1);
+                if (VS_SHADE_PREFETCH > 1) { vs_prefetch_l2(p0 + dx); vs_prefetch_l2(p1 + dx); }
+            } else if (VS_SHADE_PFMODE == 1) {
+                const uint32_t bytes = (S::NVEC + dx) * 16u;
+                vs_prefetch_l2_bulk(p0, bytes);
+                if (xy >> 31) vs_prefetch_l2_bulk(p1, bytes);
+            } else {
+                // the 256-byte aligned blocks that hold the row's one or two texels (texture allocations are padded to 256 bytes)
+                const unsigned long long a0 = (unsigned long long)p0, a1 = (unsigned long long)p1;
+                const unsigned long long s0 = a0 & ~255ull, s1 = a1 & ~255ull;
+                const uint32_t bytes = (uint32_t)(((a0 + (S::NVEC + dx) * 16u + 255ull) & ~255ull) - s0);
+                vs_prefetch_l2_bulk((const void*)s0, bytes);
+                if (xy >> 31) vs_prefetch_l2_bulk((const void*)s1, bytes);
+            }
         }
     };
     if (VS_SHADE_PREFETCH)
@@ -213,7 +271,10 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
 
     // ---------------- phase B: shade + composite ----------------
     const uint32_t oct = lane >> 3, oi = lane & 7;  // octet index (= pixel row) / lane within octet
-    float4* ysm = reinterpret_cast<float4*>(per_warp + warp * 3584);                // [j][oct][4 chunks of 4 floats], swizzled
+    // SH basis of the warp's 32 pixels: pixel (row r, column c) owns the four 16-byte chunks of slot r * 8 + (c ^ (r & 1)) and
+    // keeps chunk q at position (q + (r >> 1) + (c >> 1)) & 3 -- both the owners' stores (8 columns of a row per quarter warp)
+    // and the octets' loads (2 chunks x the 4 rows of one column) then touch every bank group exactly once
+    float4* ysm = reinterpret_cast<float4*>(per_warp + warp * 3584);
     // record / logit slabs, one 16-byte chunk per pixel, pixel (row o, column j) at chunk 8 o + ((j + 2 o) & 7):
     // the owners' stores (8 columns of one row) and the octets' accesses (4 rows of one column) are both conflict free
     uint4* rec_o = reinterpret_cast<uint4*>(per_warp + warp * 3584 + 2048);         // texel offsets
@@ -221,17 +282,39 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     float4* part = reinterpret_cast<float4*>(per_warp + warp * 3584 + 3072);        // 4 channel logits
     const uint32_t own_slot = (lane & 24u) + (((lane & 7u) + 2u * (lane >> 3)) & 7u);
     {
-        // SH basis of the owner's pixel -> row (j = column, oct = row); chunk q stored at q ^ (row >> 1) so that
-        // the four octets' reads of one chunk fall into distinct banks
+        // SH basis of the owner's pixel (layout: see ysm above)
         float Y[16];
 #pragma unroll
         for (int c = 0; c < 16; ++c) Y[c] = 0.0f;
         float vx, vy, vz;
         vs_view_dir(cams[view], px, py, vx, vy, vz);
         vs_sh_basis<DEG>(vx, vy, vz, Y);
-        float4* row = ysm + ((lane & 7) * 4 + (lane >> 3)) * 4;
+        const uint32_t yr = lane >> 3, yc = lane & 7;
+        float4* row = ysm + (yr * 8 + (yc ^ (yr & 1))) * 4;
+        if (S::MMA) {
+            // B operand of the mma: Y_c = hi_c + lo_c in fp16 (|error| < 2^-22 |Y_c|), chunk i = hilo * 2 + (t >> 1) holds the
+            // halves {x[2t], x[2t+1], x[2t+8], x[2t+9]} of t = 2 (i & 1) and t + 1: lane oi of an octet reads 8 bytes at 8 oi
+            __half hi[16], lo[16];
 #pragma unroll
-        for (int q = 0; q < 4; ++q) row[q ^ (int)(lane >> 4)] = make_float4(Y[4 * q], Y[4 * q + 1], Y[4 * q + 2], Y[4 * q + 3]);
+            for (int c = 0; c < 16; ++c) {
+                hi[c] = __float2half_rn(Y[c]);
+                lo[c] = __float2half_rn(Y[c] - __half2float(hi[c]));
+            }
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const __half* x = (i >> 1) ? lo : hi;
+                const int t0 = 2 * (i & 1);
+                const __half2 h0 = __halves2half2(x[2 * t0], x[2 * t0 + 1]), h1 = __halves2half2(x[2 * t0 + 8], x[2 * t0 + 9]);
+                const __half2 h2 = __halves2half2(x[2 * t0 + 2], x[2 * t0 + 3]), h3 = __halves2half2(x[2 * t0 + 10], x[2 * t0 + 11]);
+                uint4 u;
+                u.x = *reinterpret_cast<const uint32_t*>(&h0); u.y = *reinterpret_cast<const uint32_t*>(&h1);
+                u.z = *reinterpret_cast<const uint32_t*>(&h2); u.w = *reinterpret_cast<const uint32_t*>(&h3);
+                reinterpret_cast<uint4*>(row)[(i + (yr >> 1) + (yc >> 1)) & 3] = u;
+            }
+        } else {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) row[(q + (yr >> 1) + (yc >> 1)) & 3] = make_float4(Y[4 * q], Y[4 * q + 1], Y[4 * q + 2], Y[4 * q + 3]);
+        }
     }
     const uint32_t ychunk0 = ((oi % LPC) * NE) >> 2;   // first 16-byte chunk of this lane's coefficients
     const bool lane_on = oi < (uint32_t)NACT;
@@ -239,14 +322,14 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     float Tr = 1.0f, Cr = 0.0f, Cg = 0.0f, Cb = 0.0f;
     bool alive = true;
     for (uint32_t l = 0; l < sc.k; ++l) {
-        const float2 ab = rec_ab[l * VS_TILE_PIX + tid];
+        const float2 ab = rec_ab[l * VS_SHADE_PIX + tid];
         const bool shade = ab.x >= 0.0f && alive;
         const unsigned m = __ballot_sync(0xFFFFFFFFu, shade);
         if (m == 0) continue;  // warp-uniform
         VsFragRec r;
         r.o00 = r.o01 = r.o10 = r.o11 = 0; r.w00 = r.w01 = r.w10 = r.w11 = 0.0f;
         if (shade) {
-            const uint32_t xy = rec_xy[l * VS_TILE_PIX + tid];
+            const uint32_t xy = rec_xy[l * VS_SHADE_PIX + tid];
             const uint32_t cx0 = xy & 0x7FFFu, cy0 = (xy >> 16) & 0x7FFFu;
             const uint32_t Wt = sc.tex_w[l], nv = (uint32_t)S::NVEC;
             const uint32_t row0 = cy0 * Wt, row1 = row0 + ((xy >> 31) ? Wt : 0u);
@@ -268,38 +351,67 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
         rec_o[own_slot] = make_uint4(r.o00, r.o01, r.o10, r.o11);
         rec_w[own_slot] = make_float4(r.w00, r.w01, r.w10, r.w11);
         __syncwarp();
-        const uint4* __restrict__ tb = sc.tex[l] + SLOTS * oi;
+        // address = per-lane base + 16 * (32-bit texel-vector offset): one IMAD.WIDE.U32 per load
+        const char* __restrict__ tb = reinterpret_cast<const char*>(sc.tex[l] + SLOTS * oi);
 
-        uint4 tv[2][SLOTS][4];
+        uint4 tv[VS_SHADE_DEPTH][SLOTS][4];   // ring of texel vectors: columns j .. j + VS_SHADE_DEPTH - 2 are in flight
         auto issue = [&](int j, int b) {
             const uint4 o = rec_o[8 * oct + ((j + 2 * oct) & 7)];
 #pragma unroll
             for (int s = 0; s < SLOTS; ++s) {
                 if (lane_on) {
-                    tv[b][s][0] = __ldg(tb + o.x + s); tv[b][s][1] = __ldg(tb + o.y + s);
-                    tv[b][s][2] = __ldg(tb + o.z + s); tv[b][s][3] = __ldg(tb + o.w + s);
+                    tv[b][s][0] = vs_ldg_tex(tb, o.x, s); tv[b][s][1] = vs_ldg_tex(tb, o.y, s);
+                    tv[b][s][2] = vs_ldg_tex(tb, o.z, s); tv[b][s][3] = vs_ldg_tex(tb, o.w, s);
                 } else {
                     tv[b][s][0] = tv[b][s][1] = tv[b][s][2] = tv[b][s][3] = make_uint4(0, 0, 0, 0);
                 }
             }
         };
-        issue(0, 0);
+#pragma unroll
+        for (int j = 0; j < VS_SHADE_DEPTH - 1; ++j) issue(j, j);
         if (VS_SHADE_PREFETCH && l + VS_SHADE_PF_DIST < sc.k && alive) prefetch_layer(l + VS_SHADE_PF_DIST);
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-            if (j + 1 < 8) issue(j + 1, (j + 1) & 1);
-            const int b = j & 1;
+            if (j + VS_SHADE_DEPTH - 1 < 8) issue(j + VS_SHADE_DEPTH - 1, (j + VS_SHADE_DEPTH - 1) % VS_SHADE_DEPTH);
+            const int b = j % VS_SHADE_DEPTH;
             const uint32_t slot = 8 * oct + ((j + 2 * oct) & 7);
             const float4 w = rec_w[slot];
+            if (S::MMA) {
+                // rows of A = (fragment f = octet, channel), columns of B = (fragment, hi | lo): lane (g = lane >> 2, t = lane & 3)
+                // gets D[g][2t .. 2t+1] and D[g+8][..]; the entries of its OWN fragment are those of t == f
+                const uint2 bf = *reinterpret_cast<const uint2*>(reinterpret_cast<const unsigned char*>(ysm) +
+                    (oct * 8 + ((uint32_t)j ^ (oct & 1))) * 64 + ((((oi >> 2) * 2 + ((oi & 3) >> 1)) + (oct >> 1) + (j >> 1)) & 3) * 16 + (oi & 1) * 8);
+                float d0, d1, d2, d3, sa, sb;
+                vs_mma_16816(d0, d1, d2, d3, tv[b][0][0], bf.x, bf.y);
+                sa = w.x * (d0 + d1); sb = w.x * (d2 + d3);
+                vs_mma_16816(d0, d1, d2, d3, tv[b][0][1], bf.x, bf.y);
+                sa = fmaf(w.y, d0 + d1, sa); sb = fmaf(w.y, d2 + d3, sb);
+                vs_mma_16816(d0, d1, d2, d3, tv[b][0][2], bf.x, bf.y);
+                sa = fmaf(w.z, d0 + d1, sa); sb = fmaf(w.z, d2 + d3, sb);
+                vs_mma_16816(d0, d1, d2, d3, tv[b][0][3], bf.x, bf.y);
+                sa = fmaf(w.w, d0 + d1, sa); sb = fmaf(w.w, d2 + d3, sb);
+                // lane (g, t == f) holds channels g & 1 (sa) and (g & 1) + 2 (sb) of its fragment: part = {ch0, ch2, ch1, ch3}
+                if ((lane & 3u) == oct) reinterpret_cast<float2*>(part)[slot * 2 + ((lane >> 2) & 1u)] = make_float2(sa, sb);
+            } else {
             const f32x2 W00 = vs_pack2(w.x, w.x), W01 = vs_pack2(w.y, w.y), W10 = vs_pack2(w.z, w.z), W11 = vs_pack2(w.w, w.w);
-            const float4* yrow = ysm + (j * 4 + oct) * 4;
+            const float4* yrow = ysm + (oct * 8 + ((uint32_t)j ^ (oct & 1))) * 4;
             f32x2 acc2 = 0ull;
+#ifdef VS_EXP_NOMATH   // timing experiment only (wrong images): keep the loads, drop conversions + bilinear + SH arithmetic
+            {
+                uint32_t x = 0;
+#pragma unroll
+                for (int s = 0; s < SLOTS; ++s)
+#pragma unroll
+                    for (int q4 = 0; q4 < 4; ++q4) x ^= tv[b][s][q4].x ^ tv[b][s][q4].y ^ tv[b][s][q4].z ^ tv[b][s][q4].w;
+                acc2 = vs_pack2(__uint_as_float(x & 0x3F800000u) * w.x, yrow[ychunk0 & 3].x);
+            }
+#else
 #pragma unroll
             for (int s = 0; s < SLOTS; ++s) {
 #pragma unroll
                 for (int h = 0; h < PPV / 2; ++h) {   // 16-byte chunk of 4 basis values <-> 2 element pairs
                     const int e = s * PPV + 2 * h;    // element pair index within the lane's coefficients
-                    const float4 y = yrow[(ychunk0 + (e >> 1)) ^ (oct >> 1)];
+                    const float4 y = yrow[(ychunk0 + (e >> 1) + (oct >> 1) + (j >> 1)) & 3];
 #pragma unroll
                     for (int g = 0; g < 2; ++g) {
                         const int q = 2 * h + g;
@@ -311,17 +423,20 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
                     }
                 }
             }
+#endif
             float a0, a1;
             vs_unpack2(acc2, a0, a1);
             float acc = a0 + a1;
             if (LPC == 2) acc += __shfl_xor_sync(0xFFFFFFFFu, acc, 1);
             if (lane_on && (oi % LPC) == 0) reinterpret_cast<float*>(part)[slot * 4 + oi / LPC] = acc;
+            }
         }
         __syncwarp();
         if (shade) {
-            const float4 s4 = part[own_slot];
+            float4 s4 = part[own_slot];
+            if (S::MMA) { const float t = s4.y; s4.y = s4.z; s4.z = t; }   // stored as {ch0, ch2, ch1, ch3}
             float A = vs_sigmoid(s4.w);
-            if (fr.attenuate) A *= rec_aw[l * VS_TILE_PIX + tid];
+            if (fr.attenuate) A *= rec_aw[l * VS_SHADE_PIX + tid];
             const float TA = Tr * A;
             Cr += TA * vs_sigmoid(s4.x); Cg += TA * vs_sigmoid(s4.y); Cb += TA * vs_sigmoid(s4.z);
             Tr *= (1.0f - A);
@@ -336,7 +451,7 @@ template <int F16, int DEG, bool COUNT>
 static cudaError_t launch_sh2(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
 {
     if (sc.texel_vecs != (uint32_t)VsShadeShape<F16, DEG>::NVEC) return cudaErrorInvalidValue;
-    const size_t smem = (size_t)sc.k * VS_TILE_PIX * (fr.attenuate ? 16 : 12) + 8 * 3584;
+    const size_t smem = (size_t)sc.k * VS_SHADE_PIX * (fr.attenuate ? 16 : 12) + VS_SHADE_WARPS * 3584;
     auto kern = k_shade<F16, DEG, COUNT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -344,12 +459,12 @@ static cudaError_t launch_sh2(const VsSceneDev& sc, const VsFrame& fr, const VsC
     e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, VS_SHADE_CARVEOUT);
     if (e != cudaSuccess) return e;
 #endif
-    dim3 grid(fr.tiles_x * fr.tiles_y, ch.views);
+    dim3 grid(fr.tiles_x * fr.tiles_y * VS_SHADE_SUBTILES, ch.views);
     if (ch.keys)
-        kern<<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_mask, nullptr, ch.keys, ch.ids_is_output ? ch.ids : nullptr,
+        kern<<<grid, VS_SHADE_PIX, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_mask, nullptr, ch.keys, ch.ids_is_output ? ch.ids : nullptr,
                                       ch.out_rgba, ch.texel_bits, ch.counters);
     else
-        kern<<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_off, ch.ids, nullptr, nullptr, ch.out_rgba, ch.texel_bits,
+        kern<<<grid, VS_SHADE_PIX, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_off, ch.ids, nullptr, nullptr, ch.out_rgba, ch.texel_bits,
                                       ch.counters);
     return cudaGetLastError();
 }

@@ -44,6 +44,28 @@ __device__ inline void vs_plain_logits(const VsSceneDev& sc, const int4* __restr
     const uint32_t nv = sc.texel_vecs;
     const uint32_t offs[4] = {(f.cy0 * Wt + f.cx0) * nv, (f.cy0 * Wt + f.cx1) * nv, (f.cy1 * Wt + f.cx0) * nv, (f.cy1 * Wt + f.cx1) * nv};
     const float ws[4] = {(1.0f - f.a) * (1.0f - f.b), f.a * (1.0f - f.b), (1.0f - f.a) * f.b, f.a * f.b};
+    if (F16 && sc.frag_layout) {
+        // mma A-fragment order (vs_common.cuh): vector v holds channels (v >> 2) and (v >> 2) + 2, coefficients 2t, 2t+1, 2t+8, 2t+9
+#pragma unroll
+        for (int v = 0; v < 8; ++v) {   // fully unrolled: every index below is a constant
+            uint4 t[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) t[q] = __ldg(sc.tex[l] + offs[q] + v);
+#pragma unroll
+            for (int r = 0; r < 8; ++r) {
+                const int ch = (v >> 2) + 2 * ((r >> 1) & 1), c = (v & 3) * 2 + (r & 1) + 8 * (r >> 2);
+                float val = 0.0f;
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    const uint32_t w = (r >> 1) == 0 ? t[q].x : (r >> 1) == 1 ? t[q].y : (r >> 1) == 2 ? t[q].z : t[q].w;
+                    const __half2 h = *reinterpret_cast<const __half2*>(&w);
+                    val += ws[q] * ((r & 1) ? __high2float(h) : __low2float(h));
+                }
+                s[ch] += ((uint32_t)c < sc.n_coef ? Y[c] : 0.0f) * val;
+            }
+        }
+        return;
+    }
     // internal texel layout [ch][np_pad]: 16-byte vectors of consecutive coefficients of one channel
     const uint32_t vpc = nv >> 2;   // vectors per channel: 1, 2 or 4
 #pragma unroll 1
