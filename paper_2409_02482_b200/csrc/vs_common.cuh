@@ -219,21 +219,26 @@ __device__ __forceinline__ void vs_texel_coord(float u0, float du, float fW, int
     c1 = (uint32_t)min(max(i0 + 1, 0), Wt - 1);
 }
 
+// Perspective-correct barycentrics b'_1, b'_2 of the sample of pixel (px, py) in the triangle of the transformed vertices a, b, c
+// (b'_i ~ E_i q_i).  The oracle orients the triangle first (swap of vertices 1, 2 when A2 < 0); without the swap
+// every E_i changes sign, and so do the g_i and their sum: the quotients are the same bit for bit, so the setup is skipped here.
+__device__ __forceinline__ void vs_barycentrics(const int4& a, const int4& b, const int4& c, int px, int py, float& b1, float& b2)
+{
+    const int Sx = 256 * px + 128, Sy = 256 * py + 128;
+    const long long E0 = vs_edge(b.x, b.y, c.x, c.y, Sx, Sy), E1 = vs_edge(c.x, c.y, a.x, a.y, Sx, Sy), E2 = vs_edge(a.x, a.y, b.x, b.y, Sx, Sy);
+    const float g0 = __ll2float_rn(E0) * __int_as_float(a.z), g1 = __ll2float_rn(E1) * __int_as_float(b.z), g2 = __ll2float_rn(E2) * __int_as_float(c.z);
+    const float inv = __fdividef(1.0f, g0 + g1 + g2);
+    b1 = g1 * inv; b2 = g2 * inv;
+}
+
 // `tri` = index record of the winning triangle of layer l
 __device__ __forceinline__ void vs_fragment_setup_tri(const VsSceneDev& sc, const int4* __restrict__ vv, uint32_t l,
                                                       const uint4 tri, int px, int py, VsFrag& f)
 {
     const int4 a = __ldg(&vv[tri.x]), b = __ldg(&vv[tri.y]), c = __ldg(&vv[tri.z]);
-    const float2 uva = __ldg(&sc.uvs[tri.x]), uvb = __ldg(&sc.uvs[tri.y]), uvc = __ldg(&sc.uvs[tri.z]);
-    VsTri T;
-    vs_setup_tri(a, b, c, T);
-    const float2 uv0 = uva, uv1 = T.swapped ? uvc : uvb, uv2 = T.swapped ? uvb : uvc;
-    VsEdges e;
-    vs_edges_at(T, px, py, e);
-    // perspective-correct barycentrics b'_i ~ E_i q_i
-    const float g0 = __ll2float_rn(e.E0) * T.q0, g1 = __ll2float_rn(e.E1) * T.q1, g2 = __ll2float_rn(e.E2) * T.q2;
-    const float inv = __fdividef(1.0f, g0 + g1 + g2);
-    const float b1 = g1 * inv, b2 = g2 * inv;
+    const float2 uv0 = __ldg(&sc.uvs[tri.x]), uv1 = __ldg(&sc.uvs[tri.y]), uv2 = __ldg(&sc.uvs[tri.z]);
+    float b1, b2;
+    vs_barycentrics(a, b, c, px, py, b1, b2);
     const int Wt = (int)sc.tex_w[l], Ht = (int)sc.tex_h[l];
     vs_texel_coord(uv0.x, b1 * (uv1.x - uv0.x) + b2 * (uv2.x - uv0.x), (float)Wt, Wt, f.cx0, f.cx1, f.a);
     vs_texel_coord(uv0.y, b1 * (uv1.y - uv0.y) + b2 * (uv2.y - uv0.y), (float)Ht, Ht, f.cy0, f.cy1, f.b);
@@ -250,15 +255,9 @@ __device__ __forceinline__ void vs_fragment_uv(const VsSceneDev& sc, const int4*
                                                float& u0, float& du, float& v0, float& dv)
 {
     const int4 a = __ldg(&vv[tri.x]), b = __ldg(&vv[tri.y]), c = __ldg(&vv[tri.z]);
-    const float2 uva = __ldg(&sc.uvs[tri.x]), uvb = __ldg(&sc.uvs[tri.y]), uvc = __ldg(&sc.uvs[tri.z]);
-    VsTri T;
-    vs_setup_tri(a, b, c, T);
-    const float2 uv1 = T.swapped ? uvc : uvb, uv2 = T.swapped ? uvb : uvc;
-    VsEdges e;
-    vs_edges_at(T, px, py, e);
-    const float g0 = __ll2float_rn(e.E0) * T.q0, g1 = __ll2float_rn(e.E1) * T.q1, g2 = __ll2float_rn(e.E2) * T.q2;
-    const float inv = __fdividef(1.0f, g0 + g1 + g2);
-    const float b1 = g1 * inv, b2 = g2 * inv;
+    const float2 uva = __ldg(&sc.uvs[tri.x]), uv1 = __ldg(&sc.uvs[tri.y]), uv2 = __ldg(&sc.uvs[tri.z]);
+    float b1, b2;
+    vs_barycentrics(a, b, c, px, py, b1, b2);
     u0 = uva.x; du = b1 * (uv1.x - uva.x) + b2 * (uv2.x - uva.x);
     v0 = uva.y; dv = b1 * (uv1.y - uva.y) + b2 * (uv2.y - uva.y);
 }

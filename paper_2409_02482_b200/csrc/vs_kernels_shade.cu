@@ -129,13 +129,13 @@ __device__ __forceinline__ void vs_mma_16816(float& d0, float& d1, float& d2, fl
 // A CTA shades a 16-pixel-wide strip of VS_SHADE_WARPS / 2 warp rows (8x4-pixel warp blocks) of one 16x16 mask tile:
 // 8 warps = the whole tile, 4 warps = its upper or lower half (smaller CTAs pack the register file more tightly).
 #ifndef VS_SHADE_WARPS
-#define VS_SHADE_WARPS 8
+#define VS_SHADE_WARPS 4
 #endif
 #ifndef VS_SHADE_MIN_CTAS
 #define VS_SHADE_MIN_CTAS (24 / VS_SHADE_WARPS)
 #endif
 #ifndef VS_SHADE_DEPTH
-#define VS_SHADE_DEPTH 2      // register buffers of texel vectors per lane (one is being consumed)
+#define VS_SHADE_DEPTH 3      // tensor-core path: register buffers of texel vectors per lane (one is being consumed); others: 2
 #endif
 #define VS_SHADE_PIX (VS_SHADE_WARPS * 32)
 #define VS_SHADE_SUBTILES (8 / VS_SHADE_WARPS)
@@ -354,7 +354,8 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
         // address = per-lane base + 16 * (32-bit texel-vector offset): one IMAD.WIDE.U32 per load
         const char* __restrict__ tb = reinterpret_cast<const char*>(sc.tex[l] + SLOTS * oi);
 
-        uint4 tv[VS_SHADE_DEPTH][SLOTS][4];   // ring of texel vectors: columns j .. j + VS_SHADE_DEPTH - 2 are in flight
+        constexpr int DEPTH = S::MMA ? VS_SHADE_DEPTH : 2;
+        uint4 tv[DEPTH][SLOTS][4];   // ring of texel vectors: columns j .. j + VS_SHADE_DEPTH - 2 are in flight
         auto issue = [&](int j, int b) {
             const uint4 o = rec_o[8 * oct + ((j + 2 * oct) & 7)];
 #pragma unroll
@@ -368,12 +369,12 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             }
         };
 #pragma unroll
-        for (int j = 0; j < VS_SHADE_DEPTH - 1; ++j) issue(j, j);
+        for (int j = 0; j < DEPTH - 1; ++j) issue(j, j);
         if (VS_SHADE_PREFETCH && l + VS_SHADE_PF_DIST < sc.k && alive) prefetch_layer(l + VS_SHADE_PF_DIST);
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
-            if (j + VS_SHADE_DEPTH - 1 < 8) issue(j + VS_SHADE_DEPTH - 1, (j + VS_SHADE_DEPTH - 1) % VS_SHADE_DEPTH);
-            const int b = j % VS_SHADE_DEPTH;
+            if (j + DEPTH - 1 < 8) issue(j + DEPTH - 1, (j + DEPTH - 1) % DEPTH);
+            const int b = j % DEPTH;
             const uint32_t slot = 8 * oct + ((j + 2 * oct) & 7);
             const float4 w = rec_w[slot];
             if (S::MMA) {
