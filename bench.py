@@ -31,10 +31,32 @@ from paper_2409_02482_b200 import synth  # noqa: E402
 
 METRIC = "megapixels_per_sec_rendering_k_layers"
 UNIT = "MP/s"
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel (k_shade, direct path) from the committed
-# `ncu --set full` capture (profiles/), divided by the views of the captured launch, keyed by config; reported
-# per launch of the timed run.  None for configs without a capture.
-NCU_TRAFFIC_BYTES_PER_VIEW = {4: (21.545490e9 + 1.304478e9) / 16}   # profiles/r1m_summary.md: one launch = 16 views
+# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel from the committed `ncu --set full` captures:
+# profiles/ncu_traffic.json holds, per configuration, the bytes per view of the captured launch together with the commit
+# and the SHA-256 of the kernel sources the capture was taken from.  `roofline.traffic` is reported only while those
+# sources are unchanged (else null: a capture of other code is not evidence about this run).
+TRAFFIC_FILE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "ncu_traffic.json")
+TRAFFIC_SOURCES = ("vs_kernels_shade.cu", "vs_common.cuh")
+
+
+def kernel_source_hashes():
+    import hashlib
+    d = os.path.join(os.path.dirname(os.path.abspath(__file__)), "paper_2409_02482_b200", "csrc")
+    return {f: hashlib.sha256(open(os.path.join(d, f), "rb").read()).hexdigest() for f in TRAFFIC_SOURCES}
+
+
+def ncu_traffic_bytes_per_view(config_key):
+    """(bytes per view, provenance) of the committed capture of this configuration, or (None, why not)."""
+    try:
+        table = json.load(open(TRAFFIC_FILE))
+    except Exception:
+        return None, "no profiles/ncu_traffic.json"
+    ent = table.get(str(config_key))
+    if not ent:
+        return None, "no committed ncu capture of this configuration"
+    if ent.get("source_sha256") != kernel_source_hashes():
+        return None, "kernel sources changed since the capture of commit %s" % ent.get("commit")
+    return float(ent["dram_bytes_per_view"]), "ncu --set full capture of commit %s (%s)" % (ent.get("commit"), ent.get("summary"))
 
 
 def load_peaks():
@@ -115,6 +137,15 @@ def build_scene(cfg, rank, world, args):
         kw["num_cameras"] = args.views
     if getattr(args, "banded", False):
         kw["banded"] = True
+    if getattr(args, "camera_subset", None):
+        kw["camera_subset"] = args.camera_subset
+    if getattr(args, "strong", False):
+        # strong scaling: ONE batch (rank 0's cameras), split evenly over the ranks; every rank renders its slice
+        sc = synth.make_config(cfg, **kw)
+        mine = vsdist.shard_views(len(sc.cameras), rank, world)
+        sc.name += " [strong scaling: views %d..%d of the %d-view batch on rank %d]" % (mine.start, mine.stop - 1, len(sc.cameras), rank)
+        sc.cameras = np.ascontiguousarray(sc.cameras[mine.start:mine.stop])
+        return sc
     return synth.make_config(cfg, camera_rotate=vsdist.rank_camera_rotation(rank, world), **kw)
 
 
@@ -165,12 +196,17 @@ def run_ours(args):
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     vsdist.init_process_group("nccl")
-    binding.load_library()
+    if args.lib:            # a variant build of the same sources (python -m paper_2409_02482_b200.build --lib PATH -D...)
+        binding.LIB_PATH = os.path.abspath(args.lib)
+        binding.load_library(build_if_missing=False)
+    else:
+        binding.load_library()
 
     sc = build_scene(args.config, rank, world, args)
     B, W, H = len(sc.cameras), sc.width, sc.height
     renderer = binding.Renderer(sc, dev)
-    path_flag = (binding.VS_FLAG_TILED_PATH if args.tiled else 0) | (binding.VS_FLAG_ATTENUATION if args.attenuation else 0)
+    path_flag = ((binding.VS_FLAG_TILED_PATH if args.tiled else 0) | (binding.VS_FLAG_ATTENUATION if args.attenuation else 0) |
+                 (binding.VS_FLAG_OVERLAP if args.overlap else 0))
     flags = binding.VS_FLAG_KERNEL_TIMING | path_flag
     params = binding.make_params(W, H, sc.near_plane, sc.t_min, sc.background, flags, args.chunk)
     out = torch.empty((B, H, W, 4), dtype=torch.float32, device=dev)
@@ -209,22 +245,21 @@ def run_ours(args):
     for _ in range(max(args.warmup, 0)):
         run_step()
     torch.cuda.synchronize()
+    renderer.stats()        # resets the accumulated kernel timings: what the next query returns belongs to the timed steps
 
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    shade_ms = raster_ms = bin_ms = xf_ms = 0.0
-    shade_launches = launches = 0
     vsdist.barrier()
     torch.cuda.synchronize()
     wall0 = time.time()
     ev0.record(stream)
     for _ in range(args.steps):
-        run_step()
-        st = renderer.stats()                      # per-kernel CUDA-event times of the finished call
-        shade_ms += st["ms_shade"]; raster_ms += st["ms_raster"]; bin_ms += st["ms_binning"]; xf_ms += st["ms_transform"]
-        shade_launches += st["shade_launches"]; launches += st["kernel_launches"]
+        run_step()          # asynchronous: no host synchronisation between the steps
     ev1.record(stream)
     torch.cuda.synchronize()
     vsdist.barrier()
+    st = renderer.stats()   # per-kernel CUDA-event times (recorded on the render stream) and launch counts of the K steps
+    shade_ms, raster_ms, bin_ms, xf_ms = st["ms_shade"], st["ms_raster"], st["ms_binning"], st["ms_transform"]
+    shade_launches, launches = st["shade_launches"], st["kernel_launches"]
     secs = ev0.elapsed_time(ev1) / 1e3
     clocks = sampler.stop(wall0, time.time()) if sampler else None
     secs_max = vsdist.max_over_ranks(secs, dev)
@@ -258,9 +293,25 @@ def run_ours(args):
     bytes_per_launch = (b_tex + b_grad + b_fb) * args.steps / max(shade_launches, 1)
     achieved = bytes_per_launch / (per_launch_ms * 1e-3) / 1e9 if per_launch_ms > 0 else 0.0
     step_achieved = alg_bytes_step * world / (secs_max / args.steps) / 1e9
+    views_per_launch = B * args.steps / max(shade_launches, 1)
+    traffic_key = "%d%s%s" % (args.config, "-" + args.camera_subset if args.camera_subset else "", "-backward" if args.backward else "")
+    plain = not (args.tiled or args.attenuation or args.overlap or args.views or banded or args.lib)
+    traffic_per_view, traffic_src = ncu_traffic_bytes_per_view(traffic_key) if plain else (None, "not the captured launch configuration")
+    # the three candidate bounds of SURVEY.md §8(d), per view: HBM (algorithmic bytes), L1 gather (4 texels per fragment through
+    # the 128 B/clk/SM data pipe), FP32 issue (algorithmic lane-ops: 4 x 4n bilinear + SH FMAs, 4 x 4n half->float conversions
+    # for fp16 texels, ~40 for sigmoids and blend; 128 lanes per SM) -- the largest one binds
+    sm_clock_hz = 1965.0e6
+    frags_view = cstats["shaded_fragments"] / B
+    t_hbm = alg_bytes_step / B / (peak * 1e9) * 1e3
+    t_l1 = frags_view * 4 * texel_bytes / (148 * 128 * sm_clock_hz) * 1e3
+    lane_ops = 16 * sc.n_coef + (16 * sc.n_coef if (not banded and sc.layers[0].texture.dtype == np.float16) or banded else 0) + 40
+    t_fp32 = frags_view * lane_ops / (148 * 128 * sm_clock_hz) * 1e3
+    cand = {"hbm": t_hbm, "l1_gather": t_l1, "fp32_issue": t_fp32}
+    bounds = {"ms_per_view": cand, "binding": max(cand, key=cand.get), "measured_ms_per_view": 1e3 * secs_max / args.steps / B,
+              "lane_ops_per_fragment": lane_ops, "note": "148 SMs x 128 B/clk resp. 128 lanes at 1965 MHz; HBM at the measured copy peak"}
     roofline = {"bound": "hbm", "kernel": "k_backward" if args.backward else "k_shade", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": (NCU_TRAFFIC_BYTES_PER_VIEW[args.config] * B * args.steps / max(shade_launches, 1)
-                            if args.config in NCU_TRAFFIC_BYTES_PER_VIEW and not (args.tiled or args.backward or args.attenuation) else None),
+                "frac": achieved / peak, "traffic": traffic_per_view * views_per_launch if traffic_per_view else None,
+                "traffic_source": traffic_src, "bounds": bounds,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_per_launch,
                 "launch_ms": per_launch_ms, "views_per_launch": B * args.steps / max(shade_launches, 1),
                 "kernel_share_of_step": shade_ms / (secs * 1e3),
@@ -296,10 +347,17 @@ def run_ours(args):
             nviews += 1
         cpu_baseline = {"value": nviews * W * H / t / 1e6, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
                         "sample": "first %d of %d views of %s, %.1f s" % (nviews, B, sc.name, t)}
+        # "reported for 1 thread and for all host cores" -- one view on one thread, if it fits the budget
+        est = t / nviews * oracle.max_threads()
+        if est <= args.cpu_1thread_seconds:
+            t1 = time_oracle(sc, [0], threads=1)
+            cpu_baseline["one_thread"] = {"value": W * H / t1 / 1e6, "unit": UNIT, "cores": 1, "sample": "view 0, %.1f s" % t1}
+        else:
+            cpu_baseline["one_thread"] = {"value": None, "skipped": "estimated %.0f s for one view > --cpu-1thread-seconds %.0f" % (est, args.cpu_1thread_seconds)}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": 1e3 * secs_max / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f32", "data": "synthetic", "fps": fps,
+            "ms_per_step": 1e3 * secs_max / args.steps, "higher_is_better": True, "scaling": "strong" if args.strong else "weak",
+            "vs_baseline": None, "dtype": "f32", "data": "synthetic", "fps": fps,
             "config": {"workload": sc.name, "k": sc.k, "triangles_per_layer": int(sc.layers[0].indices.shape[0]),
                        "width": W, "height": H, "views_per_step": B, "sh_degree": sc.sh_degree,
                        "texture": ("uint8 banded " + " ".join("%dx%d" % (t.shape[1], t.shape[0]) for t in sc.layers[0].band_textures)
@@ -307,7 +365,8 @@ def run_ours(args):
                                   "%s %dx%d" % (sc.layers[0].texture.dtype, sc.layers[0].texture.shape[1], sc.layers[0].texture.shape[0]),
                        "raster_path": "tiled (binning + per-tile shared-memory keys)" if args.tiled
                        else "direct (triangle-parallel, 64-bit max keys in HBM/L2)",
-                       "attenuation": bool(args.attenuation),
+                       "attenuation": bool(args.attenuation), "overlap": bool(args.overlap), "library": args.lib or "libvs_b200.so",
+                       "timed_loop": "K asynchronous vs_render calls, one stream synchronisation at the end; kernel times from CUDA events on the render stream",
                        "pass": "backward to texels (vs_render_backward)" if args.backward else "forward (vs_render)",
                        "parallelism": "views sharded, scene replicated (dp%d)" % world,
                        "l2": "no flush: %.2f GiB of textures streamed per step >> 126 MB L2" % (
@@ -339,6 +398,12 @@ def main():
     ap.add_argument("--banded", action="store_true", help="the paper's 8-bit mixed-resolution textures on the same geometry (PAPER.md:L445-459; not the headline workload)")
     ap.add_argument("--attenuation", action="store_true", help="render with VS_FLAG_ATTENUATION (PAPER.md:L279-286; not the headline workload)")
     ap.add_argument("--tiled", action="store_true", help="time the per-tile raster path (VS_FLAG_TILED_PATH) instead of the default direct one")
+    ap.add_argument("--overlap", action="store_true", help="VS_FLAG_OVERLAP: S1-S4 of the next chunk beside S5-S7 of the current one (experiment, DESIGN.md §7)")
+    ap.add_argument("--camera-subset", choices=["far", "close"], default=None,
+                    help="every other camera of the set: on C5 the r=3 orbit cameras resp. the r=1.6 close-ups (SURVEY.md §8(d))")
+    ap.add_argument("--strong", action="store_true", help="multi-GPU: split ONE camera batch evenly over the ranks (strong scaling) instead of one batch per rank")
+    ap.add_argument("--lib", default=None, help="load this build of the library (an experiment variant made by `python -m paper_2409_02482_b200.build --lib PATH -D...`)")
+    ap.add_argument("--cpu-1thread-seconds", type=float, default=30.0, help="budget of the 1-thread oracle sample (one whole view); skipped if a view would take longer")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":

@@ -115,18 +115,20 @@ typedef struct {
     uint32_t views_per_chunk; /* cameras processed per internal pass; 0 = choose automatically             */
 } vs_render_params;
 
-/* Counters of the most recent vs_render / vs_render_host on a scene (summed over its cameras). */
+/* Counters of the most recent render call on a scene (summed over its cameras), plus the launch counts and the
+ * VS_FLAG_KERNEL_TIMING stage times ACCUMULATED over all render calls since the previous vs_query_last_render (so that a
+ * caller may time many asynchronous calls and pay one host wait). */
 typedef struct {
     uint64_t dropped_triangles;    /* near-plane / guard-band drops (0 on all BASELINE.json configs)      */
     uint64_t degenerate_triangles; /* zero area after snapping                                             */
     uint64_t tile_refs;            /* (triangle, tile) pairs binned                                        */
-    uint64_t scratch_bytes;        /* peak device scratch of the call                                      */
-    uint64_t kernel_launches;      /* kernels launched by the call (memsets / copies not counted)          */
+    uint64_t scratch_bytes;        /* peak device scratch held by the scene so far                         */
+    uint64_t kernel_launches;      /* kernels launched since the previous query (memsets / copies not counted) */
     uint64_t raster_launches;      /* of which k_raster (one per chunk of cameras)                         */
     uint64_t shade_launches;       /* of which k_shade  (one per chunk of cameras)                         */
     uint64_t shaded_fragments;     /* VS_FLAG_COUNT_TEXELS: (pixel, layer) fragments shaded                */
     uint64_t unique_texels;        /* VS_FLAG_COUNT_TEXELS: sum over views and layers of distinct texels   */
-    double   ms_transform;         /* VS_FLAG_KERNEL_TIMING: device time per stage, summed over the call   */
+    double   ms_transform;         /* VS_FLAG_KERNEL_TIMING: device time per stage, summed since the previous query */
     double   ms_binning;           /*   count + scan + scatter                                             */
     double   ms_raster;            /*   coverage + nearest-fragment resolve kernel                         */
     double   ms_shade;             /*   texel fetch + SH + composite kernel                                */
@@ -178,21 +180,30 @@ vs_status vs_scene_create(const vs_scene_desc* desc, void* cuda_stream, vs_scene
 
 /*
  * vs_render -- the hot path, steps S1-S7 of DESIGN.md §1 for a batch of cameras:
- *   S1 vertex transform + S2 triangle setup, S3 screen-tile binning (count / scan / scatter),
- *   S4 coverage + per-layer nearest-fragment resolve, S5 perspective-correct UV + bilinear fetch,
- *   S6 SH evaluation + sigmoid, S7 fixed-order front-to-back compositing.
+ *   S1 vertex transform, S2 triangle setup + S4 coverage and per-layer nearest-fragment resolve (default: triangle-parallel
+ *   with 64-bit maximum keys in HBM/L2; under VS_FLAG_TILED_PATH: S3 screen-tile binning by count / prefix sum / scatter, then
+ *   one CTA per tile with the keys in shared memory), S5 perspective-correct UV + bilinear fetch, S6 SH evaluation + sigmoid,
+ *   S7 fixed-order front-to-back compositing.
  *
- *   cameras      HOST  [num_cameras]
+ *   cameras      HOST  [num_cameras]; copied before the call returns (the caller may reuse the array at once)
  *   out_rgba     DEVICE [num_cameras][height][width][4] float: rgb = C + T*background, a = 1 - T.
  *                A pixel no layer hits is a value (background, alpha 0), not an error.
  *   out_tri_ids  DEVICE [num_cameras][num_layers][height][width] uint32 or NULL: id of the nearest
  *                covering triangle of each layer, 0xFFFFFFFF = miss (the AOV the parity tests read).
  *
- *   All kernels are enqueued on `cuda_stream` without any host synchronisation in between; the call
- *   then waits for that stream once, reads the counters back and returns with the outputs complete.
- *   (The per-tile triangle-reference list is sized from earlier calls and checked on the device; if a
- *   chunk of cameras needed more, the list is grown and the call renders again before returning.)
- *   Scratch is owned by the scene and reused between calls, so calls on one scene must not overlap.
+ *   ASYNCHRONOUS: all work is enqueued on `cuda_stream` and the call returns without waiting for it; the outputs are
+ *   complete when the stream reaches the end of the call's work (synchronise the stream, or keep enqueueing on it).
+ *   Counters and kernel timings are fetched lazily by vs_query_last_render, the only host wait of the render API.
+ *   Exception: under VS_FLAG_TILED_PATH the call waits once for the stream, because the per-tile triangle-reference list is
+ *   sized from earlier calls and checked on the device; if a chunk of cameras needed more, the list is grown and the call
+ *   renders again before returning.
+ *   The scene itself is immutable.  What a call writes besides the caller's outputs lives in two scratch sets owned by the
+ *   scene (transformed vertices, key image, tile masks), handed from user to user through CUDA events and grown with
+ *   stream-ordered allocations from a pool private to the scene.  Calls on one scene from several host threads and on
+ *   different streams are therefore LEGAL and give the same results as serial calls; they share the two sets, so their
+ *   device work interleaves at the granularity of a chunk of cameras instead of overlapping freely (a deliberate limit:
+ *   the key image of the direct path is kept zeroed between uses, which a per-call allocation could not offer without a
+ *   multi-GB memset per call).
  */
 vs_status vs_render(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
                     const vs_render_params* params, float* out_rgba, uint32_t* out_tri_ids,
@@ -225,8 +236,8 @@ typedef struct {
 /*
  * vs_render_aov -- vs_render plus the per-layer buffers of `aov` (which may be NULL: then it is vs_render without ids).
  *   The image is produced by the same kernels as vs_render (bit-identical); the buffers are written by a separate plain
- *   kernel (k_layer_aov) from the triangle-id planes, so the hot path carries no cost for them.  Asynchronous outputs on
- *   `cuda_stream`, same synchronisation and scratch rules as vs_render.
+ *   kernel (k_layer_aov) from the triangle-id planes, so the hot path carries no cost for them.  Asynchronous on
+ *   `cuda_stream`, same rules as vs_render.
  */
 vs_status vs_render_aov(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
                         const vs_render_params* params, float* out_rgba, const vs_aov_buffers* aov, void* cuda_stream);
@@ -242,13 +253,14 @@ vs_status vs_render_aov(vs_scene* scene, const vs_camera* cameras, uint32_t num_
  *   grad_textures  HOST array of num_layers DEVICE pointers, layer l: [tex_h][tex_w][(deg+1)^2][4] float (the API layout
  *                  of vs_layer_desc.texture, always fp32); the caller zeroes them; sums are fp32 atomics in no fixed order
  *   Float-texture scenes only (VS_ERR_UNSUPPORTED on banded scenes and with VS_FLAG_REFERENCE_PATH / TILED / COUNT).
- *   Runs S1-S4 again (nothing of the forward call is kept) and k_backward in place of k_shade; returns when done.
+ *   Runs S1-S4 again (nothing of the forward call is kept) and k_backward in place of k_shade; asynchronous on
+ *   `cuda_stream` like vs_render.
  */
 vs_status vs_render_backward(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
                              const vs_render_params* params, const float* grad_rgba, float* const* grad_textures,
                              void* cuda_stream);
 
-/* Counters of the last completed render on this scene. */
+/* Waits for the most recent render call on this scene and returns its counters (see vs_render_stats). */
 vs_status vs_query_last_render(vs_scene* scene, vs_render_stats* out_stats);
 
 /* Frees all device memory of the scene after synchronising the device.  NULL is a no-op. */
@@ -257,7 +269,7 @@ void vs_scene_destroy(vs_scene* scene);
 /* Thread-local description of the last error on this thread ("" if none). */
 const char* vs_last_error(void);
 
-/* Library version, e.g. "vs-b200 0.1 (sm_100a)". */
+/* Library version, e.g. "vs-b200 0.2 (sm_100a)". */
 const char* vs_version(void);
 
 #ifdef __cplusplus

@@ -168,7 +168,7 @@ def render_backward(layers, sh_degree: int, camera, width: int, height: int, ids
                     attenuation: bool = False, num_threads: int = 0):
     """Accumulate dL/d(texture) of every layer for one view, given the forward ids of that view and the upstream
     gradient grad_out [H,W,4].  grad_tex: list of float64 arrays shaped like the textures (created as zeros if None);
-    returned."""
+    an entry may be None: that layer's gradient is then not computed.  Returned."""
     k = len(layers)
     arr = (_Layer * k)()
     keep, code = [], None
@@ -183,8 +183,8 @@ def render_backward(layers, sh_degree: int, camera, width: int, height: int, ids
     if grad_tex is None:
         grad_tex = [np.zeros(L.texture.shape, dtype=np.float64) for L in layers]
     for gt, L in zip(grad_tex, layers):
-        assert gt.dtype == np.float64 and gt.flags.c_contiguous and gt.shape == L.texture.shape
-    gptr = (C.c_void_p * k)(*[g.ctypes.data for g in grad_tex])
+        assert gt is None or (gt.dtype == np.float64 and gt.flags.c_contiguous and gt.shape == L.texture.shape)
+    gptr = (C.c_void_p * k)(*[None if g is None else g.ctypes.data for g in grad_tex])
     cam = np.ascontiguousarray(camera, dtype=np.float32)
     bg = np.asarray(background, dtype=np.float64)
     ids = np.ascontiguousarray(ids, dtype=np.uint32)

@@ -509,7 +509,8 @@ int vso_render_banded(const vso_layer* layers, const vso_bands* bands, double v_
  *   dL/ds_ch = dL/drgb_ch rgb_ch (1 - rgb_ch) ;  dL/ds_3 = dL/dA alpha_w sigma(s_3) (1 - sigma(s_3))
  *   dL/dtex[q][c][ch] += w_q Y_c dL/ds_ch           for the four texels q of the footprint
  * The early exit is a constant of the differentiation (layers behind it get no gradient); coverage and UVs do not depend
- * on the textures.  Float textures only (dtype 0 / 1).  Returns 0, or -1 on bad arguments.
+ * on the textures.  Float textures only (dtype 0 / 1).  grad_tex[l] == NULL: the gradient of layer l is not wanted (a full-size
+ * fp64 gradient texture is 2 GB per layer; the tests take the layers one at a time).  Returns 0, or -1 on bad arguments.
  */
 int vso_render_backward(const vso_layer* layers, uint32_t k, uint32_t sh_degree, int tex_dtype, const float* cam,
                         uint32_t width, uint32_t height, float near_plane, double t_min, const double* bg,
@@ -605,6 +606,7 @@ int vso_render_backward(const vso_layer* layers, uint32_t k, uint32_t sh_degree,
                 ds[3] = Tl[l] * (cg - R) * aw[l] * sig3[l] * (1.0 - sig3[l]);
                 R = A[l] * cg + (1.0 - A[l]) * R;
                 const vso_layer* L = &layers[l];
+                if (!grad_tex[l]) continue;
                 for (int q = 0; q < 4; ++q)
                     for (uint32_t c = 0; c < n; ++c)
                         for (int ch = 0; ch < 4; ++ch) {

@@ -78,6 +78,15 @@ class vs_render_stats(C.Structure):
 
 
 _lib = None
+# handle -> (k, n_coef, [(tex_h, tex_w)] per layer, banded): what the marshalling checks of the render calls need
+_SCENES = {}
+
+
+def _scene_info(scene):
+    info = _SCENES.get(int(scene))
+    if info is None:
+        raise ValueError("unknown scene handle %r (not created through this binding, or already destroyed)" % (scene,))
+    return info
 
 
 def load_library(build_if_missing: bool = True):
@@ -182,6 +191,7 @@ def vs_scene_create(layers, sh_degree: int, stream=None) -> int:
     desc = vs_scene_desc(k, sh_degree, dtype_code or 0, VS_MEM_HOST if on_host else VS_MEM_DEVICE, arr)
     handle = C.c_void_p()
     _check(L.vs_scene_create(C.byref(desc), _stream_ptr(stream), C.byref(handle)))
+    _SCENES[handle.value] = (k, (sh_degree + 1) ** 2, [(int(ly.texture.shape[0]), int(ly.texture.shape[1])) for ly in layers], False)
     return handle.value
 
 
@@ -218,6 +228,7 @@ def vs_scene_create_banded(layers, sh_degree: int, v_min: float, v_max: float, s
     desc = vs_scene_desc_banded(k, sh_degree, VS_MEM_HOST if on_host else VS_MEM_DEVICE, float(v_min), float(v_max), arr)
     handle = C.c_void_p()
     _check(L.vs_scene_create_banded(C.byref(desc), _stream_ptr(stream), C.byref(handle)))
+    _SCENES[handle.value] = (k, (sh_degree + 1) ** 2, [(int(ly.band_textures[0].shape[0]), int(ly.band_textures[0].shape[1])) for ly in layers], True)
     return handle.value
 
 
@@ -229,12 +240,16 @@ def _cams(cameras):
 
 def vs_render(scene: int, cameras, params: vs_render_params, out_rgba, out_tri_ids=None, stream=None):
     """cameras: HOST [B,16] float32; out_rgba: CUDA float32 [B,H,W,4]; out_tri_ids: CUDA int32/uint32
-    [B,k,H,W] or None.  Asynchronous on `stream` (default: torch's current stream)."""
+    [B,k,H,W] or None.  Asynchronous on `stream` (default: torch's current stream): the call returns once the work is
+    enqueued (the cameras have been copied by then); only the per-tile path (VS_FLAG_TILED_PATH) waits for its overflow check."""
+    import torch
     cams = _cams(cameras)
-    assert out_rgba.is_cuda and out_rgba.is_contiguous() and out_rgba.numel() == cams.shape[0] * params.width * params.height * 4
+    k = _scene_info(scene)[0]
+    px = cams.shape[0] * params.width * params.height
+    assert out_rgba.is_cuda and out_rgba.is_contiguous() and out_rgba.dtype == torch.float32 and out_rgba.numel() == px * 4
     ids_ptr = None
     if out_tri_ids is not None:
-        assert out_tri_ids.is_cuda and out_tri_ids.is_contiguous() and out_tri_ids.element_size() == 4
+        assert out_tri_ids.is_cuda and out_tri_ids.is_contiguous() and out_tri_ids.element_size() == 4 and out_tri_ids.numel() == px * k
         ids_ptr = out_tri_ids.data_ptr()
     _check(load_library().vs_render(scene, cams.ctypes.data, cams.shape[0], C.byref(params),
                                     out_rgba.data_ptr(), ids_ptr, _stream_ptr(stream)))
@@ -244,12 +259,17 @@ def vs_render_aov(scene: int, cameras, params: vs_render_params, out_rgba, tri_i
                   layer_normal=None, stream=None):
     """vs_render plus the per-layer buffers (CUDA tensors or None): tri_ids [B,k,H,W] int32, layer_rgba [B,k,H,W,4],
     layer_uv [B,k,H,W,2], layer_normal [B,k,H,W,3] float32."""
+    import torch
     cams = _cams(cameras)
-    assert out_rgba.is_cuda and out_rgba.is_contiguous()
+    k = _scene_info(scene)[0]
+    px = cams.shape[0] * params.width * params.height
+    assert out_rgba.is_cuda and out_rgba.is_contiguous() and out_rgba.dtype == torch.float32 and out_rgba.numel() == px * 4
     a = vs_aov_buffers()
-    for name, t in (("tri_ids", tri_ids), ("layer_rgba", layer_rgba), ("layer_uv", layer_uv), ("layer_normal", layer_normal)):
+    for name, t, per_px in (("tri_ids", tri_ids, 1), ("layer_rgba", layer_rgba, 4), ("layer_uv", layer_uv, 2), ("layer_normal", layer_normal, 3)):
         if t is not None:
-            assert t.is_cuda and t.is_contiguous() and t.element_size() == 4
+            assert t.is_cuda and t.is_contiguous() and t.element_size() == 4, name
+            assert name == "tri_ids" or t.dtype == torch.float32, name
+            assert t.numel() == px * k * per_px, "%s: %d elements, expected %d" % (name, t.numel(), px * k * per_px)
             setattr(a, name, t.data_ptr())
     _check(load_library().vs_render_aov(scene, cams.ctypes.data, cams.shape[0], C.byref(params), out_rgba.data_ptr(),
                                         C.byref(a), _stream_ptr(stream)))
@@ -260,8 +280,16 @@ def vs_render_backward(scene: int, cameras, params: vs_render_params, grad_rgba,
     cams = _cams(cameras)
     assert grad_rgba.is_cuda and grad_rgba.is_contiguous() and grad_rgba.numel() == cams.shape[0] * params.width * params.height * 4
     import torch
-    for t in grad_textures:
-        assert t.is_cuda and t.is_contiguous() and t.dtype == torch.float32
+    k, n_coef, tex_sizes, banded = _scene_info(scene)
+    assert not banded, "vs_render_backward: float-texture scenes only"
+    assert grad_rgba.dtype == torch.float32
+    # the C side reads grad_textures[l] for every l < k and scatters at offsets derived from the SCENE's texture shapes
+    assert len(grad_textures) == k, "grad_textures: %d tensors for a scene of %d layers" % (len(grad_textures), k)
+    for l, t in enumerate(grad_textures):
+        assert t.is_cuda and t.is_contiguous() and t.dtype == torch.float32, "grad_textures[%d]" % l
+        assert tuple(t.shape) == (tex_sizes[l][0], tex_sizes[l][1], n_coef, 4), \
+            "grad_textures[%d]: shape %s, expected %s" % (l, tuple(t.shape), (tex_sizes[l][0], tex_sizes[l][1], n_coef, 4))
+        assert t.data_ptr() % 16 == 0, "grad_textures[%d] must be 16-byte aligned" % l
     ptrs = (C.c_void_p * len(grad_textures))(*[t.data_ptr() for t in grad_textures])
     _check(load_library().vs_render_backward(scene, cams.ctypes.data, cams.shape[0], C.byref(params), grad_rgba.data_ptr(),
                                              ptrs, _stream_ptr(stream)))
@@ -271,9 +299,21 @@ def vs_render_host(scene: int, cameras, params: vs_render_params, out_rgba, out_
     """Same, with HOST outputs (numpy arrays or CPU torch tensors, pinned for async copies).  Blocks
     until the images are in the host buffers."""
     cams = _cams(cameras)
+    k = _scene_info(scene)[0]
+    px = cams.shape[0] * params.width * params.height
+
+    def nelem(a):
+        return a.size if isinstance(a, np.ndarray) else a.numel()
 
     def host_ptr(a):
-        return a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr()
+        if isinstance(a, np.ndarray):
+            assert a.flags.c_contiguous and a.itemsize == 4
+            return a.ctypes.data
+        assert not a.is_cuda and a.is_contiguous() and a.element_size() == 4
+        return a.data_ptr()
+
+    assert nelem(out_rgba) == px * 4, "out_rgba: %d elements, expected %d" % (nelem(out_rgba), px * 4)
+    assert out_tri_ids is None or nelem(out_tri_ids) == px * k
 
     _check(load_library().vs_render_host(scene, cams.ctypes.data, cams.shape[0], C.byref(params),
                                          host_ptr(out_rgba), host_ptr(out_tri_ids) if out_tri_ids is not None else None,
@@ -288,6 +328,7 @@ def vs_query_last_render(scene: int) -> dict:
 
 def vs_scene_destroy(scene: int):
     if scene:
+        _SCENES.pop(int(scene), None)
         load_library().vs_scene_destroy(scene)
 
 

@@ -1,6 +1,8 @@
 """Build paper_2409_02482_b200/libvs_b200.so (the C-ABI library of include/vs.h) with nvcc for sm_100a.
 
-`python -m paper_2409_02482_b200.build [--force]`.  The .so is built IN-TREE so that it travels to the
+`python -m paper_2409_02482_b200.build [--force] [--lib PATH] [-DNAME=VALUE ...]`.  `--lib` with -D switches builds a
+variant of the same sources (the experiment switches of the kernels, e.g. -DVS_SHADE_PREFETCH=0) into another file, which
+`bench.py --lib PATH` loads.  The .so is built IN-TREE so that it travels to the
 GPU box with the repository snapshot; nvcc cross-compiles without a GPU.  Every .cu is compiled to an
 object of its own (in parallel, cached under build/ by a hash of the source, the headers and the flags)
 and the objects are linked into the shared library.
@@ -80,4 +82,10 @@ def ensure_built(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(ensure_built(force="--force" in sys.argv, verbose=True))
+    argv = sys.argv[1:]
+    if "--lib" in argv:
+        out = os.path.abspath(argv[argv.index("--lib") + 1])
+        defines = [a for a in argv if a.startswith("-D")]
+        print(build(out, extra_flags=defines, force="--force" in argv, verbose=True))
+    else:
+        print(ensure_built(force="--force" in argv, verbose=True))

@@ -203,7 +203,7 @@ static vs_status init_runtime(vs_scene* s)
 }
 
 extern "C" const char* vs_last_error(void) { return g_err; }
-extern "C" const char* vs_version(void) { return "vs-b200 0.1 (sm_100a)"; }
+extern "C" const char* vs_version(void) { return "vs-b200 0.2 (sm_100a)"; }
 
 extern "C" void vs_scene_destroy(vs_scene* scene)
 {

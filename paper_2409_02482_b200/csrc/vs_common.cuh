@@ -56,6 +56,37 @@ struct VsFrame {
 // [5] max over chunks of the references a chunk needed when that exceeded ref_capacity (0 = no overflow)
 enum { VS_CNT_DROPPED = 0, VS_CNT_DEGENERATE = 1, VS_CNT_REFS = 2, VS_CNT_FRAGS = 3, VS_CNT_TEXELS = 4, VS_CNT_OVERFLOW = 5, VS_CNT_N = 8 };
 
+// ---- packed fp32 pairs (sm_100: FADD2 / FMUL2 / FFMA2 issue one instruction for two lanes' worth of fp32 work) ----
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 vs_pack2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void vs_unpack2(f32x2 v, float& lo, float& hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 vs_fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2 vs_mul2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 vs_add2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+
 // ---- triangle setup shared by the binning, raster and shading kernels ----------
 struct VsTri {
     int X0, Y0, X1, Y1, X2, Y2;

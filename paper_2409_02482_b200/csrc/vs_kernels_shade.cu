@@ -55,32 +55,6 @@ __device__ __forceinline__ uint4 vs_ldg_tex(const char* base, uint32_t vec_off, 
 #endif
 }
 
-// ---- packed fp32 pairs (sm_100: FFMA2 / FMUL2) -------------------------------------------------
-typedef unsigned long long f32x2;
-
-__device__ __forceinline__ f32x2 vs_pack2(float lo, float hi)
-{
-    f32x2 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void vs_unpack2(f32x2 v, float& lo, float& hi)
-{
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ f32x2 vs_fma2(f32x2 a, f32x2 b, f32x2 c)
-{
-    f32x2 r;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
-    return r;
-}
-__device__ __forceinline__ f32x2 vs_mul2(f32x2 a, f32x2 b)
-{
-    f32x2 r;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
-    return r;
-}
-
 // element pair q (0..3 for fp16, 0..1 for fp32) of a 16-byte texel vector as packed fp32
 template <int F16>
 __device__ __forceinline__ f32x2 vs_pair(const uint4& t, int q)

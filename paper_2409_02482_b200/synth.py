@@ -262,13 +262,29 @@ CONFIG_NAMES = {
 }
 
 
+def _scene_name(cfg: int, layers, W: int, H: int, B: int, deg: int, reduced: bool, suffix: str = "") -> str:
+    """Name built from the ACTUAL sizes; the full configuration keeps its BASELINE.json wording, a variant made with
+    overrides is called "Cn-reduced" and lists what was really built (so that no log line claims more than was run)."""
+    if not reduced:
+        return CONFIG_NAMES[cfg] + suffix
+    ly = layers[0]
+    if ly.band_textures is not None:
+        tex = "uint8 banded %d^2" % ly.band_textures[0].shape[0]
+    else:
+        tex = "%s SH%d %dx%d" % ("fp16" if ly.texture.dtype == np.float16 else "fp32", deg, ly.texture.shape[1], ly.texture.shape[0])
+    return "C%d-reduced k=%d, %d tris/layer, %dx%d x%d views, %s%s" % (cfg, len(layers), ly.indices.shape[0], W, H, B, tex, suffix)
+
+
 def make_config(cfg: int, *, seed: int = 0, mesh_n: int | None = None, width: int | None = None,
                 height: int | None = None, tex_size: int | None = None, num_cameras: int | None = None,
-                k: int | None = None, camera_rotate: float = 0.0, banded: bool = False) -> Scene:
+                k: int | None = None, camera_rotate: float = 0.0, banded: bool = False,
+                camera_subset: str | None = None) -> Scene:
     """Build configuration `cfg` (1..5).  The keyword overrides give *reduced* variants of the same
     recipe (used by the CPU tests, where the full sizes would take too long).  `banded=True` gives the
     same geometry and cameras with the paper's 8-bit mixed-resolution textures (`banded_textures`, v_range (-15, 15))
-    instead of the float ones."""
+    instead of the float ones.  `camera_subset` = "far" / "close" keeps every other camera of the set:
+    on C5 the even ones orbit at r = 3, the odd ones are the close-ups at r = 1.6 (the two regimes of SURVEY.md §8(d))."""
+    reduced = any(v is not None for v in (mesh_n, width, height, tex_size, num_cameras, k))
     if cfg == 1:
         k = k or 3
         ts = tex_size or 256
@@ -288,8 +304,8 @@ def make_config(cfg: int, *, seed: int = 0, mesh_n: int | None = None, width: in
             layers.append(Layer(pos, uv, idx, tex))
         cams = circle_cameras(B, 3.0, W, H)
         if banded:
-            return Scene(CONFIG_NAMES[1] + " [banded u8]", layers, 1, cams, W, H, v_range=(-15.0, 15.0))
-        return Scene(CONFIG_NAMES[1], layers, 1, cams, W, H)
+            return Scene(_scene_name(1, layers, W, H, B, 1, reduced, " [banded u8]"), layers, 1, cams, W, H, v_range=(-15.0, 15.0))
+        return Scene(_scene_name(1, layers, W, H, B, 1, reduced), layers, 1, cams, W, H)
 
     spec = {
         2: dict(k=5, n=91, W=800, H=800, B=16, ts=1024, deg=2, op=None),
@@ -318,7 +334,12 @@ def make_config(cfg: int, *, seed: int = 0, mesh_n: int | None = None, width: in
     else:
         radius = 3.0
     cams = fibonacci_cameras(B, radius, W, H, rotate=camera_rotate)
+    suffix = ""
+    if camera_subset is not None:
+        assert camera_subset in ("far", "close")
+        cams = np.ascontiguousarray(cams[0::2] if camera_subset == "far" else cams[1::2])
+        suffix = " [%d %s cameras of the set]" % (len(cams), camera_subset)
     if banded:
-        return Scene(CONFIG_NAMES[cfg] + " [banded u8 %d^2..%d^2]" % (ts, max(1, ts >> deg)), layers, deg, cams, W, H,
-                     v_range=(-15.0, 15.0))
-    return Scene(CONFIG_NAMES[cfg], layers, deg, cams, W, H)
+        return Scene(_scene_name(cfg, layers, W, H, len(cams), deg, reduced, " [banded u8 %d^2..%d^2]" % (ts, max(1, ts >> deg)) + suffix),
+                     layers, deg, cams, W, H, v_range=(-15.0, 15.0))
+    return Scene(_scene_name(cfg, layers, W, H, len(cams), deg, reduced, suffix), layers, deg, cams, W, H)

@@ -59,6 +59,13 @@ def _worker(rank, world, port, q):
         res = oracle.render_view(sc.layers, sc.sh_degree, sc.cameras[v], sc.width, sc.height,
                                  near_plane=sc.near_plane, t_min=sc.t_min, background=sc.background, num_threads=1)
         checksum += float(np.asarray(res["rgba"], dtype=np.float64).sum())
+    # bench.py --strong builds its per-rank scene with the same split: this rank's slice of ONE batch
+    import types
+    import bench
+    mine_sc = bench.build_scene(1, rank, world, types.SimpleNamespace(views=0, banded=False, camera_subset=None, strong=True))
+    assert np.array_equal(mine_sc.cameras, sc.cameras[mine]) and "strong scaling" in mine_sc.name
+    weak_sc = bench.build_scene(1, rank, world, types.SimpleNamespace(views=0, banded=False, camera_subset=None, strong=False))
+    assert len(weak_sc.cameras) == len(sc.cameras)   # weak scaling: a whole batch per rank
     vsdist.barrier()
     secs = 1.0 + rank                               # synthetic per-rank device times: the job time is the max
     out = {"rank": rank, "views": mine, "checksum": checksum,

@@ -2,9 +2,12 @@
 test_gpu_parity.py), in the launch configuration bench.py times (whole camera batch in one vs_render
 call, automatic chunking, no AOV in the timed call).
 
-For each configuration the whole batch is rendered once; a sample of views (chosen to include the
-first, the last and -- for C5 -- a far and a close-up camera) is compared against the CPU oracle pixel
-by pixel: triangle ids BIT-EXACT, RGBA max abs error <= 1e-4.  Every view is additionally checked
+For each configuration the whole batch is rendered once; FOUR views (chosen to include the first, the
+last and -- for C5 -- two far and two close-up cameras) are compared against the CPU oracle pixel
+by pixel: triangle ids BIT-EXACT, RGBA max abs error <= 1e-4.  On the first of them the counters behind
+every roofline figure (VS_FLAG_COUNT_TEXELS: shaded fragments, unique footprint texels) are compared with
+the oracle's footprint census: fragments exactly, texels to 1e-4 relative (a footprint whose fp32 texel
+coordinate falls on the other side of a texel boundary than the oracle's fp64 one moves by one texel).  Every view is additionally checked
 through properties that hold at any size (the AOV-less timed call and the AOV call give the same
 image bit for bit; the default direct raster path and the per-tile path give the same ids and image; alpha in [0,1]; pixels no layer hits are exactly the background; ids in range;
 no dropped triangles)."""
@@ -16,6 +19,7 @@ import pytest
 pytestmark = pytest.mark.gpu
 
 TOL = 1e-4
+TEXEL_COUNT_RTOL = 1e-4     # fp32-vs-fp64 footprint edge cases
 
 
 @pytest.fixture(scope="module")
@@ -72,21 +76,33 @@ def _check_config(env, cfg, sample_views, id_views):
             err = float(np.abs(rgba.astype(np.float64) - ref["rgba"]).max())
             worst = max(worst, err)
             assert err <= TOL, "C%d view %d: max abs rgba error %.3e" % (cfg, v, err)
+    # (3) the roofline numerator: the GPU's instrumented pass against the oracle's footprint census on one view
+    v = id_views[0]
+    pc = b.make_params(W, H, sc.near_plane, sc.t_min, sc.background, b.VS_FLAG_COUNT_TEXELS)
+    one = torch.empty((1, H, W, 4), dtype=torch.float32, device="cuda")
+    b.vs_render(r.handle, sc.cameras[[v]], pc, one)
+    cs = r.stats()
+    ref = env.oracle.render_scene(sc, [v], want_layer_rgba=True, want_layer_uv=True)[0]
+    frags, texels, _ = env.oracle.count_footprints(sc.layers, W, H, ref, t_min=sc.t_min)
+    assert cs["shaded_fragments"] == frags, "C%d view %d: %d shaded fragments, the oracle composites %d" % (cfg, v, cs["shaded_fragments"], frags)
+    assert abs(cs["unique_texels"] - texels) <= TEXEL_COUNT_RTOL * texels, \
+        "C%d view %d: %d unique texels, the oracle counts %d" % (cfg, v, cs["unique_texels"], texels)
     r.close()
-    print("C%d full size: %d views rendered, %d compared with the oracle, worst rgba err %.3e, coverage of view %d = %.3f"
-          % (cfg, B, len(id_views), worst, sample_views[0], float(hit.any(axis=0).mean())))
+    print("C%d full size: %d views rendered, %d compared with the oracle, worst rgba err %.3e, coverage of view %d = %.3f; "
+          "census of view %d: %d fragments (exact), %d unique texels (oracle %d)"
+          % (cfg, B, len(id_views), worst, sample_views[0], float(hit.any(axis=0).mean()), v, frags, cs["unique_texels"], texels))
 
 
 def test_config2_full(env):
-    _check_config(env, 2, [0, 7, 15], [0, 15])
+    _check_config(env, 2, [0, 5, 10, 15], [0, 5, 10, 15])
 
 
 def test_config3_full(env):
-    _check_config(env, 3, [0, 13, 31], [0, 31])
+    _check_config(env, 3, [0, 13, 22, 31], [0, 13, 22, 31])
 
 
 def test_config4_full(env):
-    _check_config(env, 4, [0, 29, 63], [0, 63])
+    _check_config(env, 4, [0, 29, 46, 63], [0, 29, 46, 63])
 
 
 def test_config4_full_attenuation(env):
@@ -171,6 +187,40 @@ def test_config4_backward_full_resolution(env):
     print("C4 geometry at 1920x1080, 512^2 textures, backward over 2 views: worst relative gradient error %.3e" % worst)
 
 
+def test_config4_backward_full_size_textures(env):
+    """The same at the FULL texture size (2048^2, the un-magnified regime: ~1.6 unique texels per fragment, so hardly any
+    reduction per gradient texel -- the opposite case of the 512^2 test above).  The oracle's fp64 gradient of one layer is
+    2.1 GB, so the layers are taken one at a time (oracle/render_backward skips the layers whose slot is None)."""
+    b, torch = env.binding, env.torch
+    sc = env.synth.make_config(4)
+    v = 17
+    W, H = sc.width, sc.height
+    g = np.random.default_rng(34).normal(size=(1, H, W, 4)).astype(np.float32)
+    r = b.Renderer(sc)
+    p = b.make_params(W, H, sc.near_plane, sc.t_min, sc.background)
+    grads = [torch.zeros(ly.texture.shape, dtype=torch.float32, device="cuda") for ly in sc.layers]
+    b.vs_render_backward(r.handle, sc.cameras[[v]], p, torch.from_numpy(g).cuda(), grads)
+    torch.cuda.synchronize()
+    r.close()
+    ref = env.oracle.render_scene(sc, [v])[0]
+    worst = 0.0
+    for l in (0, 4, 8):        # outermost, middle, innermost shell
+        slot = [np.zeros(ly.texture.shape, np.float64) if i == l else None for i, ly in enumerate(sc.layers)]
+        env.oracle.render_backward(sc.layers, sc.sh_degree, sc.cameras[v], W, H, ref["ids"], g[0].astype(np.float64), slot,
+                                   near_plane=sc.near_plane, t_min=sc.t_min, background=sc.background)
+        want = slot[l]
+        got = grads[l].cpu().numpy()
+        scale = np.abs(want).max()
+        assert scale > 1e-3
+        err = float(np.abs(got - want).max() / scale)
+        worst = max(worst, err)
+        assert err <= 1e-4, "layer %d: relative gradient error %.3e" % (l, err)
+        assert np.all(got[want == 0.0] == 0.0)
+        del slot, want, got
+    print("C4 full size (2048^2 textures), backward of view %d, layers 0 / 4 / 8 against the oracle: worst relative gradient error %.3e"
+          % (v, worst))
+
+
 def test_config5_full(env):
-    # even views are far cameras (r = 3), odd views close-ups (r = 1.6) that fill the frame
-    _check_config(env, 5, [0, 1, 15], [0, 1])
+    # even views are far cameras (r = 3), odd views close-ups (r = 1.6) that fill the frame: two of each
+    _check_config(env, 5, [0, 1, 14, 15], [0, 1, 14, 15])

@@ -402,3 +402,34 @@ def test_host_path_matches_device_path(env):
     b.vs_render_host(h, sc.cameras, b.make_params(160, 120), pageable)
     assert np.array_equal(pageable, dev_rgba)
     b.vs_scene_destroy(h)
+
+
+def test_census_counters_match_the_oracle(env):
+    """The numerator of every roofline figure ("counted, not assumed"): VS_FLAG_COUNT_TEXELS' shaded
+    fragments and unique 2x2-footprint texels against the oracle's footprint census (pinned in tests/test_oracle_census.py)
+    on reduced C2 and C4 scenes and on C1, several views per call (the texel count is per view, summed over the views).
+    Fragments must agree exactly; texels to 1e-4 relative (fp32-vs-fp64 texel coordinate at a texel boundary), and with an
+    early exit (C1 with an opaque middle layer) the fragment count may differ by the knife-edge pixels only."""
+    b = env.binding
+    cases = [(env.synth.make_config(2, mesh_n=31, width=200, height=200, tex_size=256, num_cameras=3), [0, 1, 2], None),
+             (env.synth.make_config(4, mesh_n=40, width=320, height=180, tex_size=256, num_cameras=3), [0, 2], None),
+             (env.synth.make_config(1), [0, 1, 2, 3], None),
+             (env.synth.make_config(1), [1, 3], 2.0 ** -6)]
+    for n, (sc, views, t_min) in enumerate(cases):
+        if t_min is not None:
+            sc.layers[1].texture[:, :, 0, 3] += 30.0       # opaque middle layer: the innermost one is never composited
+        tm = sc.t_min if t_min is None else t_min
+        _, _, stats = gpu_render(env, sc, views, flags=b.VS_FLAG_COUNT_TEXELS, t_min=tm, want_ids=False)
+        frags = texels = 0
+        for v in views:
+            ref = env.oracle.render_scene(sc, [v], want_layer_rgba=True, want_layer_uv=True, t_min=tm)[0]
+            f, t, _ = env.oracle.count_footprints(sc.layers, sc.width, sc.height, ref, t_min=tm)
+            frags += f
+            texels += t
+        assert frags > 1000 and texels > 1000
+        assert stats["shaded_fragments"] == frags, "case %d: %d fragments on the GPU, %d in the oracle" % (n, stats["shaded_fragments"], frags)
+        assert abs(stats["unique_texels"] - texels) <= max(2, 1e-4 * texels), \
+            "case %d: %d unique texels on the GPU, %d in the oracle" % (n, stats["unique_texels"], texels)
+        if t_min is not None:
+            hits = sum(int((env.oracle.render_scene(sc, [v], t_min=tm)[0]["ids"] != env.oracle.MISS).sum()) for v in views)
+            assert frags < hits, "the early exit must have removed fragments"

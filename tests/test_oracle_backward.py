@@ -77,3 +77,16 @@ def test_layers_behind_the_early_exit_get_no_gradient():
     inner_only = (r["ids"][0] == oracle.MISS) & (r["ids"][1] != oracle.MISS)
     assert not inner_only.any()                   # nested shells: layer 1 is only ever seen through layer 0
     assert np.abs(grads[0]).max() > 1e-3 and np.all(grads[1] == 0.0) and np.all(grads[2] == 0.0)
+
+
+def test_layers_can_be_taken_one_at_a_time():
+    """grad_tex[l] = None skips layer l; the other layers' gradients are unchanged (the full-size GPU test relies on it)."""
+    sc = synth.make_config(1, width=40, height=32, num_cameras=1, tex_size=32)
+    ref = oracle.render_scene(sc, [0])[0]
+    g = np.random.default_rng(5).normal(size=(sc.height, sc.width, 4))
+    kw = dict(near_plane=sc.near_plane, t_min=sc.t_min, background=sc.background)
+    full = oracle.render_backward(sc.layers, sc.sh_degree, sc.cameras[0], sc.width, sc.height, ref["ids"], g, **kw)
+    for l in range(sc.k):
+        only = [np.zeros(ly.texture.shape, np.float64) if i == l else None for i, ly in enumerate(sc.layers)]
+        oracle.render_backward(sc.layers, sc.sh_degree, sc.cameras[0], sc.width, sc.height, ref["ids"], g, only, **kw)
+        np.testing.assert_allclose(only[l], full[l], rtol=0, atol=1e-12 * max(1.0, np.abs(full[l]).max()))
