@@ -281,12 +281,13 @@ def vs_render_backward(scene: int, cameras, params: vs_render_params, grad_rgba,
     assert grad_rgba.is_cuda and grad_rgba.is_contiguous() and grad_rgba.numel() == cams.shape[0] * params.width * params.height * 4
     import torch
     k, n_coef, tex_sizes, banded = _scene_info(scene)
-    assert not banded, "vs_render_backward: float-texture scenes only"
     assert grad_rgba.dtype == torch.float32
     # the C side reads grad_textures[l] for every l < k and scatters at offsets derived from the SCENE's texture shapes
     assert len(grad_textures) == k, "grad_textures: %d tensors for a scene of %d layers" % (len(grad_textures), k)
     for l, t in enumerate(grad_textures):
         assert t.is_cuda and t.is_contiguous() and t.dtype == torch.float32, "grad_textures[%d]" % l
+        if banded:
+            continue          # the library rejects banded scenes itself (VS_ERR_UNSUPPORTED) before touching any tensor
         assert tuple(t.shape) == (tex_sizes[l][0], tex_sizes[l][1], n_coef, 4), \
             "grad_textures[%d]: shape %s, expected %s" % (l, tuple(t.shape), (tex_sizes[l][0], tex_sizes[l][1], n_coef, 4))
         assert t.data_ptr() % 16 == 0, "grad_textures[%d] must be 16-byte aligned" % l

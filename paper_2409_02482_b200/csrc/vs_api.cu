@@ -56,25 +56,45 @@ struct DeviceGuard {
 
 // Device buffer that only grows.  Growth is stream-ordered (cudaFreeAsync + cudaMallocFromPoolAsync on the stream that
 // uses the buffer next): no cudaFree / cudaMalloc, hence no implicit device synchronisation inside a render call.
+// Every buffer sits between two guard bands of VS_GUARD_BYTES filled with 0xA5 at allocation; vs_query_last_render checks
+// them (compute-sanitizer is not available on the target pool: an out-of-bounds WRITE of a kernel into scratch is caught here).
+#define VS_GUARD_BYTES 4096
 struct DevBuf {
-    void* p = nullptr;
-    size_t cap = 0;
+    void* p = nullptr;     // first usable byte
+    size_t cap = 0;        // usable bytes
     cudaError_t reserve(size_t bytes, cudaMemPool_t pool, cudaStream_t st, bool* grew = nullptr)
     {
         if (bytes <= cap) return cudaSuccess;
-        if (p) cudaFreeAsync(p, st);
+        if (p) cudaFreeAsync((char*)p - VS_GUARD_BYTES, st);
         p = nullptr; cap = 0;
-        size_t want = bytes + bytes / 8;
-        cudaError_t e = cudaMallocFromPoolAsync(&p, want, pool, st);
+        size_t want = (bytes + bytes / 8 + 255) & ~(size_t)255;
+        void* base = nullptr;
+        cudaError_t e = cudaMallocFromPoolAsync(&base, want + 2 * VS_GUARD_BYTES, pool, st);
         if (e != cudaSuccess) {
             cudaGetLastError();   // clear the failed attempt: the exact-size retry below may succeed
-            want = bytes;
-            e = cudaMallocFromPoolAsync(&p, want, pool, st);
+            want = (bytes + 255) & ~(size_t)255;
+            e = cudaMallocFromPoolAsync(&base, want + 2 * VS_GUARD_BYTES, pool, st);
         }
-        if (e == cudaSuccess) { cap = want; if (grew) *grew = true; } else { p = nullptr; cudaGetLastError(); }
+        if (e != cudaSuccess) { cudaGetLastError(); return e; }
+        p = (char*)base + VS_GUARD_BYTES; cap = want;
+        if (grew) *grew = true;
+        e = cudaMemsetAsync(base, 0xA5, VS_GUARD_BYTES, st);
+        if (e == cudaSuccess) e = cudaMemsetAsync((char*)p + cap, 0xA5, VS_GUARD_BYTES, st);
         return e;
     }
-    void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }   // after a device synchronisation only
+    // after a device synchronisation only: true if both guard bands still hold their pattern
+    bool guards_intact() const
+    {
+        if (!p) return true;
+        unsigned char h[2][VS_GUARD_BYTES];
+        if (cudaMemcpy(h[0], (char*)p - VS_GUARD_BYTES, VS_GUARD_BYTES, cudaMemcpyDeviceToHost) != cudaSuccess) return false;
+        if (cudaMemcpy(h[1], (char*)p + cap, VS_GUARD_BYTES, cudaMemcpyDeviceToHost) != cudaSuccess) return false;
+        for (int g = 0; g < 2; ++g)
+            for (int i = 0; i < VS_GUARD_BYTES; ++i)
+                if (h[g][i] != 0xA5) return false;
+        return true;
+    }
+    void release() { if (p) cudaFree((char*)p - VS_GUARD_BYTES); p = nullptr; cap = 0; }   // after a device synchronisation only
 };
 
 #define VS_NUM_SETS 2      // scratch sets; a call ping-pongs between them
@@ -93,6 +113,16 @@ struct ScratchSet {
     cudaEvent_t ev_raster = nullptr;   // S1-S4 of the chunk in this set have been enqueued up to here
     cudaEvent_t ev_done = nullptr;     // the last consumer of the set (shade / backward / aov kernel) ends here
     bool used = false;                 // ev_done has been recorded at least once
+    const DevBuf* named(int i, const char** name) const
+    {
+        static const char* names[] = {"vtx", "keys", "tile_count", "big_list", "big_count", "tri_tiles", "tile_off", "tile_cursor",
+                                      "tile_tris", "ids", "texel_bits", "aov_ids"};
+        const DevBuf* bufs[] = {&vtx, &keys, &tile_count, &big_list, &big_count, &tri_tiles, &tile_off, &tile_cursor, &tile_tris, &ids,
+                                &texel_bits, &aov_ids};
+        if (i < 0 || i >= 12) return nullptr;
+        *name = names[i];
+        return bufs[i];
+    }
     size_t bytes() const
     {
         return vtx.cap + keys.cap + tile_count.cap + big_list.cap + big_count.cap + tri_tiles.cap + tile_off.cap + tile_cursor.cap +
@@ -946,6 +976,21 @@ extern "C" vs_status vs_query_last_render(vs_scene* scene, vs_render_stats* out)
     out->shaded_fragments = h[VS_CNT_FRAGS];
     out->unique_texels = h[VS_CNT_TEXELS];
     out->scratch_bytes = scene->scratch_peak;
+    // guard bands of every scratch buffer (written by no kernel unless it runs out of bounds); the streams of OTHER calls may
+    // still be running, so wait for the device first -- this is the statistics call, not the hot path
+    CU(cudaDeviceSynchronize());
+    for (int si = 0; si < VS_NUM_SETS; ++si)
+        for (int bi = 0;; ++bi) {
+            const char* name = "";
+            const DevBuf* db = scene->sets[si].named(bi, &name);
+            if (!db) break;
+            if (!db->guards_intact()) return fail(VS_ERR_CUDA, "scratch guard band of %s (set %d) was overwritten: a kernel wrote out of bounds", name, si);
+        }
+    for (int ti = 0; ti < VS_NUM_TICKETS; ++ti)
+        if (!scene->tickets[ti].cams.guards_intact()) return fail(VS_ERR_CUDA, "scratch guard band of the camera buffer was overwritten");
+    for (int i = 0; i < 2; ++i)
+        if (!scene->stage_rgba[i].guards_intact() || !scene->stage_ids[i].guards_intact())
+            return fail(VS_ERR_CUDA, "scratch guard band of a staging buffer was overwritten");
     out->kernel_launches = scene->launches;
     out->raster_launches = scene->raster_launches;
     out->shade_launches = scene->shade_launches;

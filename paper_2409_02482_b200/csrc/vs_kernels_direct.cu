@@ -125,23 +125,33 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
     }
 #ifndef VS_EXP_NOMASK
     {
-        // layer bit of every 16x16 tile the box touches: k_shade skips the tiles and layers nothing was drawn into.
-        // A warp's 32 consecutive triangles share a handful of tiles: the lanes that report the same (tile, layer)
-        // elect one of them (match.any), so the L2 sees a few atomics per warp instead of one per triangle.
+        // layer bit of every 16x16 tile the box touches: k_shade skips the tiles and layers nothing was drawn into.  The mask
+        // only has to be a SUPERSET (a set bit costs k_shade a read of zero keys, nothing else).  A warp's 32 consecutive
+        // triangles form a compact patch, so the warp marks the tiles of the bounding box of its boxes with the union of its
+        // layer bits: five warp reductions and at most one atomic per lane.  Warps whose patch is spread over more than 32
+        // tiles (a mesh whose index order jumps) fall back to exact per-triangle marks.
         uint32_t* __restrict__ tm = tile_mask + (size_t)view * fr.tiles_x * fr.tiles_y;
         const int tx0 = i0 / VS_TILE_W, tx1 = i1 / VS_TILE_W, ty0 = j0 / VS_TILE_H, ty1 = j1 / VS_TILE_H;
+        const int wx0 = __reduce_min_sync(0xFFFFFFFFu, valid ? tx0 : 0x7FFFFFFF), wx1 = __reduce_max_sync(0xFFFFFFFFu, valid ? tx1 : -1);
+        const int wy0 = __reduce_min_sync(0xFFFFFFFFu, valid ? ty0 : 0x7FFFFFFF), wy1 = __reduce_max_sync(0xFFFFFFFFu, valid ? ty1 : -1);
+        const uint32_t wl = __reduce_or_sync(0xFFFFFFFFu, valid ? (1u << layer) : 0u);
+        const int nx = wx1 - wx0 + 1, nt = nx * (wy1 - wy0 + 1);
+        if (wl != 0u && nt <= 32) {
+            if ((int)lane < nt) atomicOr(&tm[(size_t)(wy0 + (int)lane / nx) * fr.tiles_x + (wx0 + (int)lane % nx)], wl);
+        } else if (wl != 0u) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) {  // the four corner tiles; a box of at most 8x8 samples touches no other
-            const int tx = (c & 1) ? tx1 : tx0, ty = (c & 2) ? ty1 : ty0;
-            const bool fresh = valid && !((c & 1) && tx1 == tx0) && !((c & 2) && ty1 == ty0);
-            const uint32_t tile = (uint32_t)ty * fr.tiles_x + (uint32_t)tx;
-            const uint32_t key = fresh ? tile * 16u + layer : 0xFFFFFFFFu;
-            const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key);
-            if (fresh && (uint32_t)(__ffs(peers) - 1) == lane) atomicOr(&tm[tile], 1u << layer);
+            for (int c = 0; c < 4; ++c) {  // the four corner tiles; a box of at most 8x8 samples touches no other
+                const int tx = (c & 1) ? tx1 : tx0, ty = (c & 2) ? ty1 : ty0;
+                const bool fresh = valid && !((c & 1) && tx1 == tx0) && !((c & 2) && ty1 == ty0);
+                const uint32_t tile = (uint32_t)ty * fr.tiles_x + (uint32_t)tx;
+                const uint32_t key = fresh ? tile * 16u + layer : 0xFFFFFFFFu;
+                const uint32_t peers = __match_any_sync(0xFFFFFFFFu, key);
+                if (fresh && (uint32_t)(__ffs(peers) - 1) == lane) atomicOr(&tm[tile], 1u << layer);
+            }
+            if (large && (tx1 - tx0 > 1 || ty1 - ty0 > 1))  // the tiles between the corners
+                for (int ty = ty0; ty <= ty1; ++ty)
+                    for (int tx = tx0; tx <= tx1; ++tx) atomicOr(&tm[(size_t)ty * fr.tiles_x + tx], 1u << layer);
         }
-        if (large && (tx1 - tx0 > 1 || ty1 - ty0 > 1))  // the tiles between the corners
-            for (int ty = ty0; ty <= ty1; ++ty)
-                for (int tx = tx0; tx <= tx1; ++tx) atomicOr(&tm[(size_t)ty * fr.tiles_x + tx], 1u << layer);
     }
 #endif
     {

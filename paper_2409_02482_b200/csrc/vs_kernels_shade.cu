@@ -112,6 +112,7 @@ __device__ __forceinline__ void vs_mma_16816(float& d0, float& d1, float& d2, fl
 #define VS_SHADE_DEPTH 3      // tensor-core path: register buffers of texel vectors per lane (one is being consumed); others: 2
 #endif
 #define VS_SHADE_PIX (VS_SHADE_WARPS * 32)
+#define VS_SHADE_WARP_BYTES 3072   // shared memory per warp: SH basis 2048 + fragment records 512 + logits 512
 #define VS_SHADE_SUBTILES (8 / VS_SHADE_WARPS)
 template <int F16, int DEG, bool COUNT>
 __global__ void __launch_bounds__(VS_SHADE_PIX, VS_SHADE_MIN_CTAS)
@@ -127,8 +128,8 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     // [k][pixels] packed texel coordinates, then [k][pixels] float2 fractions (a < 0: no fragment)
     uint32_t* rec_xy = reinterpret_cast<uint32_t*>(smem);
     float2* rec_ab = reinterpret_cast<float2*>(smem + (size_t)sc.k * VS_SHADE_PIX * 4);
-    unsigned char* per_warp = smem + (size_t)sc.k * VS_SHADE_PIX * 12;  // per warp: 2 KB basis + 1 KB records + 512 B logits
-    float* rec_aw = reinterpret_cast<float*>(per_warp + VS_SHADE_WARPS * 3584);   // [k][pixels] attenuation weights (only if fr.attenuate)
+    unsigned char* per_warp = smem + (size_t)sc.k * VS_SHADE_PIX * 12;  // per warp: 2 KB basis + 512 B records + 512 B logits
+    float* rec_aw = reinterpret_cast<float*>(per_warp + VS_SHADE_WARPS * VS_SHADE_WARP_BYTES);   // [k][pixels] attenuation weights (only if fr.attenuate)
 
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t tile = blockIdx.x / VS_SHADE_SUBTILES, sub = blockIdx.x % VS_SHADE_SUBTILES, view = blockIdx.y;
@@ -248,12 +249,11 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     // SH basis of the warp's 32 pixels: pixel (row r, column c) owns the four 16-byte chunks of slot r * 8 + (c ^ (r & 1)) and
     // keeps chunk q at position (q + (r >> 1) + (c >> 1)) & 3 -- both the owners' stores (8 columns of a row per quarter warp)
     // and the octets' loads (2 chunks x the 4 rows of one column) then touch every bank group exactly once
-    float4* ysm = reinterpret_cast<float4*>(per_warp + warp * 3584);
+    float4* ysm = reinterpret_cast<float4*>(per_warp + warp * VS_SHADE_WARP_BYTES);
     // record / logit slabs, one 16-byte chunk per pixel, pixel (row o, column j) at chunk 8 o + ((j + 2 o) & 7):
     // the owners' stores (8 columns of one row) and the octets' accesses (4 rows of one column) are both conflict free
-    uint4* rec_o = reinterpret_cast<uint4*>(per_warp + warp * 3584 + 2048);         // texel offsets
-    float4* rec_w = reinterpret_cast<float4*>(per_warp + warp * 3584 + 2560);       // bilinear weights
-    float4* part = reinterpret_cast<float4*>(per_warp + warp * 3584 + 3072);        // 4 channel logits
+    uint4* rec_o = reinterpret_cast<uint4*>(per_warp + warp * VS_SHADE_WARP_BYTES + 2048);    // fragment records
+    float4* part = reinterpret_cast<float4*>(per_warp + warp * VS_SHADE_WARP_BYTES + 2560);   // 4 channel logits
     const uint32_t own_slot = (lane & 24u) + (((lane & 7u) + 2u * (lane >> 3)) & 7u);
     {
         // SH basis of the owner's pixel (layout: see ysm above)
@@ -322,16 +322,23 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             }
         }
         if (COUNT && lane == 0) atomicAdd(&counters[VS_CNT_FRAGS], (unsigned long long)__popc(m));
-        rec_o[own_slot] = make_uint4(r.o00, r.o01, r.o10, r.o11);
-        rec_w[own_slot] = make_float4(r.w00, r.w01, r.w10, r.w11);
+        // one 16-byte record per fragment: {offset of texel 00 | "the footprint has a second column", offset of texel 10, a, b}
+        // (offsets are multiples of NVEC >= 4: the low bits are free); the octets rebuild the other two offsets and the four
+        // weights -- half the shared-memory wavefronts of two records
+        rec_o[own_slot] = make_uint4(r.o00 | (r.o01 != r.o00 ? 1u : 0u), r.o10, __float_as_uint(shade ? ab.x : 0.0f), __float_as_uint(shade ? ab.y : 0.0f));
         __syncwarp();
         // address = per-lane base + 16 * (32-bit texel-vector offset): one IMAD.WIDE.U32 per load
         const char* __restrict__ tb = reinterpret_cast<const char*>(sc.tex[l] + SLOTS * oi);
 
         constexpr int DEPTH = S::MMA ? VS_SHADE_DEPTH : 2;
         uint4 tv[DEPTH][SLOTS][4];   // ring of texel vectors: columns j .. j + VS_SHADE_DEPTH - 2 are in flight
+        float fa[DEPTH], fb[DEPTH];  // and the bilinear fractions of their fragments
         auto issue = [&](int j, int b) {
-            const uint4 o = rec_o[8 * oct + ((j + 2 * oct) & 7)];
+            const uint4 rec = rec_o[8 * oct + ((j + 2 * oct) & 7)];
+            const uint32_t dxo = (rec.x & 1u) * (uint32_t)S::NVEC;
+            uint4 o;
+            o.x = rec.x & ~3u; o.y = o.x + dxo; o.z = rec.y; o.w = rec.y + dxo;
+            fa[b] = __uint_as_float(rec.z); fb[b] = __uint_as_float(rec.w);
 #pragma unroll
             for (int s = 0; s < SLOTS; ++s) {
                 if (lane_on) {
@@ -350,7 +357,9 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             if (j + DEPTH - 1 < 8) issue(j + DEPTH - 1, (j + DEPTH - 1) % DEPTH);
             const int b = j % DEPTH;
             const uint32_t slot = 8 * oct + ((j + 2 * oct) & 7);
-            const float4 w = rec_w[slot];
+            float4 w;
+            w.x = (1.0f - fa[b]) * (1.0f - fb[b]); w.y = fa[b] * (1.0f - fb[b]);
+            w.z = (1.0f - fa[b]) * fb[b];          w.w = fa[b] * fb[b];
             if (S::MMA) {
                 // rows of A = (fragment f = octet, channel), columns of B = (fragment, hi | lo): lane (g = lane >> 2, t = lane & 3)
                 // gets D[g][2t .. 2t+1] and D[g+8][..]; the entries of its OWN fragment are those of t == f
@@ -426,7 +435,7 @@ template <int F16, int DEG, bool COUNT>
 static cudaError_t launch_sh2(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
 {
     if (sc.texel_vecs != (uint32_t)VsShadeShape<F16, DEG>::NVEC) return cudaErrorInvalidValue;
-    const size_t smem = (size_t)sc.k * VS_SHADE_PIX * (fr.attenuate ? 16 : 12) + VS_SHADE_WARPS * 3584;
+    const size_t smem = (size_t)sc.k * VS_SHADE_PIX * (fr.attenuate ? 16 : 12) + VS_SHADE_WARPS * VS_SHADE_WARP_BYTES;
     auto kern = k_shade<F16, DEG, COUNT>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;

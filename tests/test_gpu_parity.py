@@ -433,3 +433,55 @@ def test_census_counters_match_the_oracle(env):
         if t_min is not None:
             hits = sum(int((env.oracle.render_scene(sc, [v], t_min=tm)[0]["ids"] != env.oracle.MISS).sum()) for v in views)
             assert frags < hits, "the early exit must have removed fragments"
+
+
+def test_every_output_is_written_in_bounds(env):
+    """Stand-in for compute-sanitizer memcheck (closed on this pool): every caller-owned output of every entry point is a
+    window inside a larger tensor filled with a sentinel; after the calls the margins must be untouched.  The library's own
+    scratch buffers carry guard bands that vs_query_last_render (Renderer.stats) verifies.  Odd image and texture sizes, so
+    that partial tiles, partial warps and the last texel rows are all exercised."""
+    b, torch = env.binding, env.torch
+    PAD = 4096
+    for cfg, kw in ((1, dict(width=101, height=67, num_cameras=3, tex_size=37)),
+                    (4, dict(mesh_n=14, width=77, height=45, tex_size=33, num_cameras=3))):
+        sc = env.synth.make_config(cfg, **kw)
+        B, W, H, k = len(sc.cameras), sc.width, sc.height, sc.k
+        r = b.Renderer(sc)
+
+        def window(n, dtype, fill):
+            big = torch.full((n + 2 * PAD,), fill, dtype=dtype, device="cuda")
+            return big, big[PAD:PAD + n]
+
+        def intact(big, n, fill):
+            return bool((big[:PAD] == fill).all()) and bool((big[PAD + n:] == fill).all())
+
+        bufs = {"rgba": window(B * H * W * 4, torch.float32, 12345.0), "ids": window(B * k * H * W, torch.int32, 0x5A5A5A5A),
+                "lrgba": window(B * k * H * W * 4, torch.float32, 12345.0), "luv": window(B * k * H * W * 2, torch.float32, 12345.0),
+                "lnrm": window(B * k * H * W * 3, torch.float32, 12345.0)}
+        for flags in (env.path_flags, env.path_flags | b.VS_FLAG_ATTENUATION, env.path_flags | b.VS_FLAG_COUNT_TEXELS):
+            for chunk in (0, 1, 2):
+                p = b.make_params(W, H, sc.near_plane, sc.t_min, sc.background, flags, chunk)
+                b.vs_render(r.handle, sc.cameras, p, bufs["rgba"][1], bufs["ids"][1])
+                b.vs_render_aov(r.handle, sc.cameras, p, bufs["rgba"][1], bufs["ids"][1], bufs["lrgba"][1], bufs["luv"][1], bufs["lnrm"][1])
+                torch.cuda.synchronize()
+                r.stats()           # raises if a scratch guard band was overwritten
+        for name, (big, win) in bufs.items():
+            fill = 0x5A5A5A5A if name == "ids" else 12345.0
+            assert intact(big, win.numel(), fill), "%s: written outside [0, %d)" % (name, win.numel())
+            assert not bool((win == fill).any()) or name != "rgba", "rgba: not every pixel was written"
+        if not env.path_flags:
+            gbig, gwin = [], []
+            for ly in sc.layers:
+                n = int(np.prod(ly.texture.shape))
+                big = torch.full((n + 2 * PAD,), 777.0, dtype=torch.float32, device="cuda")
+                big[PAD:PAD + n] = 0.0
+                gbig.append(big)
+                gwin.append(big[PAD:PAD + n].view(ly.texture.shape))
+            g = torch.ones((B, H, W, 4), dtype=torch.float32, device="cuda")
+            b.vs_render_backward(r.handle, sc.cameras, b.make_params(W, H, sc.near_plane, sc.t_min, sc.background), g, gwin)
+            torch.cuda.synchronize()
+            r.stats()
+            for l, big in enumerate(gbig):
+                assert intact(big, gwin[l].numel(), 777.0), "gradient texture %d: written out of bounds" % l
+                assert float(gwin[l].abs().max()) > 0.0
+        r.close()
