@@ -20,7 +20,7 @@ MISS = 0xFFFFFFFF
 class _Layer(C.Structure):
     _fields_ = [("positions", C.c_void_p), ("uvs", C.c_void_p), ("indices", C.c_void_p),
                 ("texture", C.c_void_p), ("num_vertices", C.c_uint32), ("num_triangles", C.c_uint32),
-                ("tex_w", C.c_uint32), ("tex_h", C.c_uint32)]
+                ("tex_w", C.c_uint32), ("tex_h", C.c_uint32), ("normals", C.c_void_p)]
 
 
 class _Bands(C.Structure):
@@ -56,6 +56,7 @@ def lib():
         L.vso_alpha_attenuation.restype = C.c_double
         L.vso_alpha_attenuation.argtypes = [C.c_void_p, C.c_void_p]
         L.vso_face_normal.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.vso_interp_normal.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.vso_half_to_double.restype = C.c_double
         L.vso_half_to_double.argtypes = [C.c_uint16]
         L.vso_sh_basis.argtypes = [C.c_int, C.c_void_p, C.c_void_p]
@@ -112,6 +113,12 @@ def render_view(layers, sh_degree: int, camera, width: int, height: int, *, near
         assert idx.ndim == 2 and idx.shape[1] == 3
         assert idx.size == 0 or int(idx.max()) < pos.shape[0]
         keep += [pos, uv, idx]
+        nrm = getattr(L, "normals", None)
+        if nrm is not None:
+            nrm = np.ascontiguousarray(nrm, dtype=np.float32)
+            assert nrm.shape == pos.shape
+            keep.append(nrm)
+        nptr = _ptr(nrm) if nrm is not None else None
         if banded:
             assert len(L.band_textures) == sh_degree + 1 and v_range is not None
             for b, t in enumerate(L.band_textures):
@@ -120,7 +127,7 @@ def render_view(layers, sh_degree: int, camera, width: int, height: int, *, near
                 keep.append(t)
                 bands[i].tex[b] = t.ctypes.data
                 bands[i].w[b], bands[i].h[b] = t.shape[1], t.shape[0]
-            arr[i] = _Layer(_ptr(pos), _ptr(uv), _ptr(idx), None, pos.shape[0], idx.shape[0], 0, 0)
+            arr[i] = _Layer(_ptr(pos), _ptr(uv), _ptr(idx), None, pos.shape[0], idx.shape[0], 0, 0, nptr)
             continue
         tex = np.ascontiguousarray(L.texture)
         c = _dtype_code(tex)
@@ -130,7 +137,7 @@ def render_view(layers, sh_degree: int, camera, width: int, height: int, *, near
         assert tex.ndim == 4 and tex.shape[2] == n and tex.shape[3] == 4, tex.shape
         keep.append(tex)
         arr[i] = _Layer(_ptr(pos), _ptr(uv), _ptr(idx), _ptr(tex), pos.shape[0], idx.shape[0],
-                        tex.shape[1], tex.shape[0])
+                        tex.shape[1], tex.shape[0], nptr)
     cam = np.ascontiguousarray(camera, dtype=np.float32)
     assert cam.shape == (16,)
     bg = np.asarray(background, dtype=np.float64)
@@ -179,7 +186,12 @@ def render_backward(layers, sh_degree: int, camera, width: int, height: int, ids
         tex = np.ascontiguousarray(L.texture)
         code = _dtype_code(tex)
         keep += [pos, uv, idx, tex]
-        arr[i] = _Layer(_ptr(pos), _ptr(uv), _ptr(idx), _ptr(tex), pos.shape[0], idx.shape[0], tex.shape[1], tex.shape[0])
+        nrm = getattr(L, "normals", None)
+        if nrm is not None:
+            nrm = np.ascontiguousarray(nrm, dtype=np.float32)
+            keep.append(nrm)
+        arr[i] = _Layer(_ptr(pos), _ptr(uv), _ptr(idx), _ptr(tex), pos.shape[0], idx.shape[0], tex.shape[1], tex.shape[0],
+                        _ptr(nrm) if nrm is not None else None)
     if grad_tex is None:
         grad_tex = [np.zeros(L.texture.shape, dtype=np.float64) for L in layers]
     for gt, L in zip(grad_tex, layers):
@@ -208,7 +220,7 @@ def count_footprints(layers, width: int, height: int, view, *, t_min: float = 2.
     for i, L in enumerate(layers):
         th, tw = (L.band_textures[0].shape[:2] if getattr(L, "band_textures", None) is not None else L.texture.shape[:2])
         sizes.append((th, tw))
-        arr[i] = _Layer(None, None, None, None, 0, 0, tw, th)
+        arr[i] = _Layer(None, None, None, None, 0, 0, tw, th, None)
     if marks is None:
         marks = [np.zeros(s, dtype=np.uint8) for s in sizes]
     for m, s in zip(marks, sizes):
@@ -292,6 +304,14 @@ def alpha_attenuation(v, n) -> float:
     v = np.ascontiguousarray(v, dtype=np.float64)
     n = np.ascontiguousarray(n, dtype=np.float64)
     return float(lib().vso_alpha_attenuation(_ptr(v), _ptr(n)))
+
+
+def interp_normal(b, n0, n1, n2) -> np.ndarray:
+    b = np.ascontiguousarray(b, dtype=np.float64)
+    ns = [np.ascontiguousarray(n, dtype=np.float32) for n in (n0, n1, n2)]
+    out = np.empty(3, dtype=np.float64)
+    lib().vso_interp_normal(_ptr(b), _ptr(ns[0]), _ptr(ns[1]), _ptr(ns[2]), _ptr(out))
+    return out
 
 
 def face_normal(p0, p1, p2) -> np.ndarray:

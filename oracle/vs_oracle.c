@@ -25,7 +25,8 @@
  * Pins (tests/test_oracle_*.py, all -m "not gpu"): closed-form full-screen quad; hand-counted top-left
  * fixtures (tests/golden/); double-precision ray-triangle brute force; scipy sph_harm; torch
  * grid_sample; numpy float16; SPEC.md:L478 blend example; analytic constant-layer compositing;
- * depth-sorted blend equivalence; attenuation: SPEC.md:L468-470 values, tanh(5x), closed-form tilted quads;
+ * depth-sorted blend equivalence; attenuation: SPEC.md:L468-470 values, tanh(5x), closed-form tilted quads; per-vertex
+ * normals: radial normals of a sphere mesh (n = the hit point's direction exactly), flat-quad coincidence with the face normal;
  * banded 8-bit format: SPEC.md:L361-378 values, grid_sample per band, float-twin renders, affine mixed-resolution
  * bands; render buffers: closed-form quad, sphere normals; backward: central finite differences of the forward;
  * footprint census (vso_count_footprints): hand-counted texels of pixel-aligned quads, early-exit and clamp cases.
@@ -51,6 +52,7 @@ typedef struct {
     const uint32_t* indices;  /* [T][3] */
     const void* texture;      /* [tex_h][tex_w][n][4], float or IEEE half */
     uint32_t num_vertices, num_triangles, tex_w, tex_h;
+    const float* normals;     /* [V][3] per-vertex normals (need not be unit) or NULL: the geometric face normal is used */
 } vso_layer;
 
 /* camera = fx fy cx cy R[9] t[3]  (x_cam = R x_world + t; +x right, +y down, +z forward) */
@@ -301,6 +303,18 @@ void vso_face_normal(const float* p0, const float* p1, const float* p2, double* 
     for (int c = 0; c < 3; ++c) n[c] = len > 0.0 ? n[c] / len : 0.0;
 }
 
+/* Surface normal of a fragment when the mesh carries per-vertex normals (SURVEY.md §8(f) NEXT-2 "optional per-vertex normals";
+ * PAPER.md:L279-286 "the angle between the view direction and the surface normal"): the three vertex normals are
+ * interpolated with the fragment's perspective-correct barycentrics b'_i (A.5) and the sum is renormalised; a vanishing sum
+ * gives n = 0 (alpha_w = 0), like a zero-area triangle does for the face normal.  nv = the three vertex normals in the order of
+ * the weights b. */
+void vso_interp_normal(const double* b, const float* n0, const float* n1, const float* n2, double* n)
+{
+    for (int c = 0; c < 3; ++c) n[c] = b[0] * (double)n0[c] + b[1] * (double)n1[c] + b[2] * (double)n2[c];
+    double len = sqrt(n[0] * n[0] + n[1] * n[1] + n[2] * n[2]);
+    for (int c = 0; c < 3; ++c) n[c] = len > 0.0 ? n[c] / len : 0.0;
+}
+
 /* view direction of pixel (i,j): camera -> scene, world frame, unit (reading Q4) */
 static void view_dir(const float* cam, int px, int py, double* v)
 {
@@ -322,9 +336,10 @@ static void view_dir(const float* cam, int px, int py, double* v)
  *   out_layer_rgba [k][H][W][4] double, decoded per-layer RGBA, 0 on miss            (optional)
  *   out_layer_uv   [k][H][W][2] double, interpolated UV, 0 on miss                   (optional)
  *   stats[0] += triangles dropped (near plane / guard band), stats[1] += zero-area triangles
- *   out_layer_normal [k][H][W][3] double, unit face normal of the winning fragment's triangle (world space), signed so that
- *                   it faces the viewer (v . n <= 0), 0 on miss or zero-area triangles                  (optional, last argument)
- *   attenuate != 0: every fragment's opacity is multiplied by alpha_w(v, face normal) before blending
+ *   out_layer_normal [k][H][W][3] double, unit normal of the winning fragment (the face normal of its triangle, or the
+ *                   interpolated vertex normal if the layer has `normals`; world space), signed so that it faces the viewer
+ *                   (v . n <= 0), 0 on miss or when the normal vanishes                                 (optional, last argument)
+ *   attenuate != 0: every fragment's opacity is multiplied by alpha_w(v, that normal) before blending
  *                   (PAPER.md:L279-286); the alpha of out_layer_rgba is the attenuated one
  * Returns 0, or -1 on bad arguments / allocation failure.
  */
@@ -438,9 +453,10 @@ static int render_impl(const vso_layer* layers, const vso_bands* btex, double v_
                 /* A.5 perspective-correct barycentrics: b'_i proportional to E_i q_i */
                 double g[3], gs = 0.0;
                 for (int c = 0; c < 3; ++c) { g[c] = (double)E[c] * (double)tri.q[c]; gs += g[c]; }
-                double uu = 0.0, vv = 0.0;
+                double uu = 0.0, vv = 0.0, bw[3];
                 for (int c = 0; c < 3; ++c) {
                     double b = g[c] / gs;
+                    bw[c] = b;
                     uu += b * (double)L->uvs[2 * (size_t)tri.vi[c] + 0];
                     vv += b * (double)L->uvs[2 * (size_t)tri.vi[c] + 1];
                 }
@@ -450,8 +466,12 @@ static int render_impl(const vso_layer* layers, const vso_bands* btex, double v_
                 if (attenuate || out_layer_normal) {
                     const uint32_t* ix = L->indices + 3 * (size_t)id;
                     double nrm[3];
-                    vso_face_normal(L->positions + 3 * (size_t)ix[0], L->positions + 3 * (size_t)ix[1],
-                                    L->positions + 3 * (size_t)ix[2], nrm);
+                    if (L->normals)
+                        vso_interp_normal(bw, L->normals + 3 * (size_t)tri.vi[0], L->normals + 3 * (size_t)tri.vi[1],
+                                          L->normals + 3 * (size_t)tri.vi[2], nrm);
+                    else
+                        vso_face_normal(L->positions + 3 * (size_t)ix[0], L->positions + 3 * (size_t)ix[1],
+                                        L->positions + 3 * (size_t)ix[2], nrm);
                     if (attenuate) lrgba[4 * l + 3] *= vso_alpha_attenuation(v, nrm);
                     if (out_layer_normal) { /* "Surface normals" buffer: oriented towards the viewer */
                         double sgn = (v[0] * nrm[0] + v[1] * nrm[1] + v[2] * nrm[2]) > 0.0 ? -1.0 : 1.0;
@@ -557,10 +577,11 @@ int vso_render_backward(const vso_layer* layers, uint32_t k, uint32_t sh_degree,
                 int64_t E[3];
                 vso_setup(vtx[l], L->indices + 3 * (size_t)id, &tri);
                 vso_covers(&tri, (int)i, (int)j, E);
-                double g[3], gs = 0.0, uu = 0.0, vv = 0.0;
+                double g[3], gs = 0.0, uu = 0.0, vv = 0.0, bw[3];
                 for (int c = 0; c < 3; ++c) { g[c] = (double)E[c] * (double)tri.q[c]; gs += g[c]; }
                 for (int c = 0; c < 3; ++c) {
                     double b = g[c] / gs;
+                    bw[c] = b;
                     uu += b * (double)L->uvs[2 * (size_t)tri.vi[c] + 0];
                     vv += b * (double)L->uvs[2 * (size_t)tri.vi[c] + 1];
                 }
@@ -586,7 +607,11 @@ int vso_render_backward(const vso_layer* layers, uint32_t k, uint32_t sh_degree,
                 if (attenuate) {
                     const uint32_t* ix = L->indices + 3 * (size_t)id;
                     double nrm[3];
-                    vso_face_normal(L->positions + 3 * (size_t)ix[0], L->positions + 3 * (size_t)ix[1], L->positions + 3 * (size_t)ix[2], nrm);
+                    if (L->normals)
+                        vso_interp_normal(bw, L->normals + 3 * (size_t)tri.vi[0], L->normals + 3 * (size_t)tri.vi[1],
+                                          L->normals + 3 * (size_t)tri.vi[2], nrm);
+                    else
+                        vso_face_normal(L->positions + 3 * (size_t)ix[0], L->positions + 3 * (size_t)ix[1], L->positions + 3 * (size_t)ix[2], nrm);
                     aw[l] = vso_alpha_attenuation(v, nrm);
                 }
                 A[l] = sig3[l] * aw[l];

@@ -275,6 +275,9 @@ static vs_status scene_create_impl(const vs_scene_desc* desc, const vs_scene_des
     d.texel_vecs = 4 * vs_vecs_per_channel(f16, n);
     d.np_pad = vs_vecs_per_channel(f16, n) * (f16 ? 8u : 4u);
     d.frag_layout = (f16 && d.np_pad == 16u && !bd) ? 1u : 0u;   // k_shade's tensor-core path
+#ifdef VS_SHADE_NO_MMA
+    d.frag_layout = 0u;   // experiment switch: channel-major texels and the packed-FFMA k_shade for every format
+#endif
     s->tex_f16 = f16;
     uint64_t vt = 0, tt = 0;
     for (uint32_t l = 0; l < k; ++l) {

@@ -89,7 +89,11 @@ struct VsShadeShape {
     static constexpr int PPV = EPV / 2;                                // fp32 pairs per vector
     // fp16 texels of 16 (padded) coefficients: stored in mma A-fragment order (VsSceneDev::frag_layout) and contracted on
     // the tensor cores, 4 fragments x 4 channels x 16 coefficients per mma.sync.m16n8k16
+#ifdef VS_SHADE_NO_MMA   // experiment switch: the packed-FFMA formulation on channel-major texels for every format (see vs_api.cu)
+    static constexpr bool MMA = false;
+#else
     static constexpr bool MMA = F16 && NCOEF > 8;
+#endif
 };
 
 // D (16x8, fp32) = A (16x16, fp16, row) x B (16x8, fp16, col), C = 0
@@ -111,8 +115,29 @@ __device__ __forceinline__ void vs_mma_16816(float& d0, float& d1, float& d2, fl
 #ifndef VS_SHADE_DEPTH
 #define VS_SHADE_DEPTH 3      // tensor-core path: register buffers of texel vectors per lane (one is being consumed); others: 2
 #endif
+#ifndef VS_SHADE_RING
+#define VS_SHADE_RING 0       // experiment: > 0 = the tensor-core path stages its texel vectors through a shared-memory
+#endif                        // ring of that many fragment columns filled by cp.async (LDGSTS) instead of register buffers
 #define VS_SHADE_PIX (VS_SHADE_WARPS * 32)
-#define VS_SHADE_WARP_BYTES 3072   // shared memory per warp: SH basis 2048 + fragment records 512 + logits 512
+#define VS_SHADE_WARP_BYTES (3072 + VS_SHADE_RING * 2048)   // shared memory per warp: SH basis 2048 + fragment records 512 + logits 512 (+ ring)
+__device__ __forceinline__ void vs_cp_async16(void* smem_dst, const void* gsrc)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
+}
+__device__ __forceinline__ void vs_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+// at most n copy groups of this thread may still be pending (n is a constant after unrolling)
+__device__ __forceinline__ void vs_cp_async_wait(int n)
+{
+    switch (n) {
+        case 0: asm volatile("cp.async.wait_group 0;" ::: "memory"); break;
+        case 1: asm volatile("cp.async.wait_group 1;" ::: "memory"); break;
+        case 2: asm volatile("cp.async.wait_group 2;" ::: "memory"); break;
+        case 3: asm volatile("cp.async.wait_group 3;" ::: "memory"); break;
+        case 4: asm volatile("cp.async.wait_group 4;" ::: "memory"); break;
+        case 5: asm volatile("cp.async.wait_group 5;" ::: "memory"); break;
+        default: asm volatile("cp.async.wait_group 6;" ::: "memory"); break;
+    }
+}
 #define VS_SHADE_SUBTILES (8 / VS_SHADE_WARPS)
 template <int F16, int DEG, bool COUNT>
 __global__ void __launch_bounds__(VS_SHADE_PIX, VS_SHADE_MIN_CTAS)
@@ -330,8 +355,11 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
         // address = per-lane base + 16 * (32-bit texel-vector offset): one IMAD.WIDE.U32 per load
         const char* __restrict__ tb = reinterpret_cast<const char*>(sc.tex[l] + SLOTS * oi);
 
-        constexpr int DEPTH = S::MMA ? VS_SHADE_DEPTH : 2;
-        uint4 tv[DEPTH][SLOTS][4];   // ring of texel vectors: columns j .. j + VS_SHADE_DEPTH - 2 are in flight
+        constexpr bool RING = S::MMA && VS_SHADE_RING > 0;
+        constexpr int DEPTH = RING ? VS_SHADE_RING : (S::MMA ? VS_SHADE_DEPTH : 2);
+        // RING: [stage][texel][lane] 16-byte slots of this warp; a lane reads back only what it copied itself
+        uint4* ring = reinterpret_cast<uint4*>(per_warp + warp * VS_SHADE_WARP_BYTES + 3072);
+        uint4 tv[RING ? 1 : DEPTH][SLOTS][4];   // ring of texel vectors: columns j .. j + VS_SHADE_DEPTH - 2 are in flight
         float fa[DEPTH], fb[DEPTH];  // and the bilinear fractions of their fragments
         auto issue = [&](int j, int b) {
             const uint4 rec = rec_o[8 * oct + ((j + 2 * oct) & 7)];
@@ -339,6 +367,13 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             uint4 o;
             o.x = rec.x & ~3u; o.y = o.x + dxo; o.z = rec.y; o.w = rec.y + dxo;
             fa[b] = __uint_as_float(rec.z); fb[b] = __uint_as_float(rec.w);
+            if (RING) {
+                const uint32_t off4[4] = {o.x, o.y, o.z, o.w};
+#pragma unroll
+                for (int q = 0; q < 4; ++q) vs_cp_async16(ring + (b * 4 + q) * 32 + lane, tb + (unsigned long long)off4[q] * 16ull);
+                vs_cp_async_commit();
+                return;
+            }
 #pragma unroll
             for (int s = 0; s < SLOTS; ++s) {
                 if (lane_on) {
@@ -356,6 +391,12 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
         for (int j = 0; j < 8; ++j) {
             if (j + DEPTH - 1 < 8) issue(j + DEPTH - 1, (j + DEPTH - 1) % DEPTH);
             const int b = j % DEPTH;
+            const int tb_i = RING ? 0 : b;
+            if (RING) {   // the copies of column j have landed (at most the younger groups are still pending)
+                vs_cp_async_wait((7 - j) < (DEPTH - 2) ? (7 - j) : (DEPTH - 2));
+#pragma unroll
+                for (int q = 0; q < 4; ++q) tv[0][0][q] = ring[(b * 4 + q) * 32 + lane];
+            }
             const uint32_t slot = 8 * oct + ((j + 2 * oct) & 7);
             float4 w;
             w.x = (1.0f - fa[b]) * (1.0f - fb[b]); w.y = fa[b] * (1.0f - fb[b]);
@@ -366,13 +407,13 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
                 const uint2 bf = *reinterpret_cast<const uint2*>(reinterpret_cast<const unsigned char*>(ysm) +
                     (oct * 8 + ((uint32_t)j ^ (oct & 1))) * 64 + ((((oi >> 2) * 2 + ((oi & 3) >> 1)) + (oct >> 1) + (j >> 1)) & 3) * 16 + (oi & 1) * 8);
                 float d0, d1, d2, d3, sa, sb;
-                vs_mma_16816(d0, d1, d2, d3, tv[b][0][0], bf.x, bf.y);
+                vs_mma_16816(d0, d1, d2, d3, tv[tb_i][0][0], bf.x, bf.y);
                 sa = w.x * (d0 + d1); sb = w.x * (d2 + d3);
-                vs_mma_16816(d0, d1, d2, d3, tv[b][0][1], bf.x, bf.y);
+                vs_mma_16816(d0, d1, d2, d3, tv[tb_i][0][1], bf.x, bf.y);
                 sa = fmaf(w.y, d0 + d1, sa); sb = fmaf(w.y, d2 + d3, sb);
-                vs_mma_16816(d0, d1, d2, d3, tv[b][0][2], bf.x, bf.y);
+                vs_mma_16816(d0, d1, d2, d3, tv[tb_i][0][2], bf.x, bf.y);
                 sa = fmaf(w.z, d0 + d1, sa); sb = fmaf(w.z, d2 + d3, sb);
-                vs_mma_16816(d0, d1, d2, d3, tv[b][0][3], bf.x, bf.y);
+                vs_mma_16816(d0, d1, d2, d3, tv[tb_i][0][3], bf.x, bf.y);
                 sa = fmaf(w.w, d0 + d1, sa); sb = fmaf(w.w, d2 + d3, sb);
                 // lane (g, t == f) holds channels g & 1 (sa) and (g & 1) + 2 (sb) of its fragment: part = {ch0, ch2, ch1, ch3}
                 if ((lane & 3u) == oct) reinterpret_cast<float2*>(part)[slot * 2 + ((lane >> 2) & 1u)] = make_float2(sa, sb);

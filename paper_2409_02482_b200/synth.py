@@ -29,6 +29,7 @@ class Layer:
     indices: np.ndarray    # [T,3] uint32
     texture: np.ndarray    # [H,W,n,4] float32 or float16 ; ch 0-2 RGB, ch 3 opacity logit (None for banded scenes)
     band_textures: list | None = None   # banded 8-bit format: band b = uint8 [H_b, W_b, 2b+1, 4]
+    normals: np.ndarray | None = None   # optional [V,3] float32 per-vertex normals (transparency attenuation)
 
 
 @dataclasses.dataclass

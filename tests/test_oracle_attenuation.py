@@ -10,6 +10,7 @@ import types
 import numpy as np
 
 import oracle
+from paper_2409_02482_b200 import synth
 
 Y00 = 0.28209479177387814
 
@@ -140,3 +141,106 @@ def test_attenuated_blend_two_layers():
     want_a = 1 - (1 - w0[..., 3]) * (1 - w1[..., 3])
     np.testing.assert_allclose(r["rgba"][both][:, :3], want_rgb[both], atol=1e-7)
     np.testing.assert_allclose(r["rgba"][both][:, 3], want_a[both], atol=1e-7)
+
+
+# ---- optional per-vertex normals ----------------------------------
+
+def test_interp_normal_unit_function():
+    n = oracle.interp_normal([0.2, 0.3, 0.5], [1, 0, 0], [0, 1, 0], [0, 0, 1])
+    want = np.array([0.2, 0.3, 0.5]) / np.linalg.norm([0.2, 0.3, 0.5])
+    np.testing.assert_allclose(n, want, atol=1e-15)
+    np.testing.assert_allclose(oracle.interp_normal([1, 0, 0], [0, 0, 3], [5, 0, 0], [0, 7, 0]), [0, 0, 1], atol=1e-15)   # need not be unit
+    assert np.all(oracle.interp_normal([0.5, 0.5, 0.0], [0, 0, 1], [0, 0, -1], [1, 0, 0]) == 0.0)                        # vanishing sum -> 0
+
+
+def test_radial_vertex_normals_of_a_sphere_mesh_give_the_hit_direction():
+    """Icospheres centred at the origin with vertex normal = vertex position / radius.  The perspective-correct barycentrics
+    interpolate the 3-D hit point p on the facet, so sum b_i n_i = p / r and the renormalised normal is EXACTLY p / |p|:
+    alpha_w = 2 Sigmoid(10 |v . p/|p||) - 1 in closed form from the depth buffer.  The face normal differs from it by up to
+    the facet angle, so the test also tells the two paths apart."""
+    sc = synth.make_config(1, width=96, height=96, num_cameras=2)
+    for ly in sc.layers:
+        ly.texture[...] = 0.0
+        ly.texture[:, :, 0, 3] = 0.9 / Y00                     # constant opacity sigmoid(0.9) everywhere, view independent
+        ly.normals = (ly.positions / np.linalg.norm(ly.positions, axis=1, keepdims=True)).astype(np.float32)
+    a0 = 1.0 / (1.0 + math.exp(-float(np.float32(0.9 / Y00)) * Y00))
+    for vi in (0, 1):
+        cam = sc.cameras[vi]
+        r = oracle.render_scene(sc, [vi], attenuation=True, want_layer_rgba=True, want_qp=True, want_layer_normal=True)[0]
+        rf = None
+        R, t = cam[4:13].reshape(3, 3).astype(np.float64), cam[13:16].astype(np.float64)
+        W, H = sc.width, sc.height
+        pi, pj = np.meshgrid(np.arange(W), np.arange(H), indexing="xy")
+        dcam = np.stack([(pi + 0.5 - cam[2]) / cam[0], (pj + 0.5 - cam[3]) / cam[1], np.ones_like(pi, dtype=np.float64)], -1)
+        vdir = dcam @ R                                         # world = R^T cam
+        vdir /= np.linalg.norm(vdir, axis=-1, keepdims=True)
+        for l in range(sc.k):
+            hit = r["ids"][l] != oracle.MISS
+            z = 1.0 / r["qp"][l][hit].astype(np.float64)
+            pw = (dcam[hit] * z[:, None] - t) @ R
+            nrm = pw / np.linalg.norm(pw, axis=1, keepdims=True)
+            d = np.abs((vdir[hit] * nrm).sum(-1))
+            want = a0 * (2.0 / (1.0 + np.exp(-10.0 * d)) - 1.0)
+            got = r["layer_rgba"][l][hit][:, 3]
+            # the rasteriser's barycentrics belong to the triangle of the SNAPPED vertices (1/256 px): against the exact ray
+            # hit they are off by ~1e-4 relative, which the facet angle (0.1 rad) and the slope of alpha_w (<= 5) turn into
+            # <= ~1e-4 in alpha_w; the face-normal path below is two orders of magnitude away
+            np.testing.assert_allclose(got, want, atol=1.5e-4)
+            # the normal buffer holds the interpolated normal, facing the viewer
+            np.testing.assert_allclose(np.abs((r["layer_normal"][l][hit] * nrm).sum(-1)), 1.0, atol=1e-9)
+            assert np.all((r["layer_normal"][l][hit] * vdir[hit]).sum(-1) <= 1e-12)
+        # negative control: with the FACE normals the opacities differ measurably near the silhouette
+        for ly in sc.layers:
+            ly.normals_saved, ly.normals = ly.normals, None
+        rf = oracle.render_scene(sc, [vi], attenuation=True, want_layer_rgba=True)[0]
+        for ly in sc.layers:
+            ly.normals = ly.normals_saved
+        hit0 = r["ids"][0] != oracle.MISS
+        assert np.abs(rf["layer_rgba"][0][hit0][:, 3] - r["layer_rgba"][0][hit0][:, 3]).max() > 1.5e-2
+
+
+def test_vertex_normals_equal_to_the_face_normal_change_nothing():
+    """A tilted flat quad whose four vertex normals are its face normal: interpolation and renormalisation return that
+    normal, so the render coincides with the face-normal path (and with -n: only |v . n| matters)."""
+    W, H, f = 40, 30, 64.0
+    tilt = 0.6
+    pos = np.array([[-1.2, -0.9, 3.0 - 1.2 * tilt], [1.2, -0.9, 3.0 + 1.2 * tilt], [1.2, 0.9, 3.0 + 1.2 * tilt], [-1.2, 0.9, 3.0 - 1.2 * tilt]], np.float32)
+    uv = [[0, 0], [1, 0], [1, 1], [0, 1]]
+    idx = [[0, 1, 2], [0, 2, 3]]
+    tex = np.zeros((8, 8, 1, 4), np.float32)
+    tex[..., 0, :] = np.array([0.3, -0.2, 0.5, 1.3]) / Y00
+    n = oracle.face_normal(pos[0], pos[1], pos[2])
+    base = L(pos, uv, idx, tex)
+    ref = oracle.render_view([base], 0, ident_cam(f, W, H), W, H, attenuation=True, want_layer_rgba=True)
+    for sign in (1.0, -1.0):
+        lv = L(pos, uv, idx, tex)
+        lv.normals = np.tile((sign * n).astype(np.float32), (4, 1))
+        got = oracle.render_view([lv], 0, ident_cam(f, W, H), W, H, attenuation=True, want_layer_rgba=True)
+        assert np.array_equal(got["ids"], ref["ids"]) and (ref["ids"] != oracle.MISS).sum() > 100
+        np.testing.assert_allclose(got["rgba"], ref["rgba"], atol=1e-7)       # n is stored as fp32: 6e-8 relative
+        np.testing.assert_allclose(got["layer_rgba"], ref["layer_rgba"], atol=1e-7)
+
+
+def test_linearly_varying_vertex_normals_closed_form():
+    """Viewport-filling quad at constant depth facing the camera (perspective-correct == affine in the pixel position) with
+    vertex normals (sx, 0, -1): the interpolated normal at pixel column i is normalize((x(i), 0, -1)), x affine from -s to s;
+    alpha_w = 2 Sigmoid(10 |v . n|) - 1 with the pixel's own view direction -- recomputed here with numpy only."""
+    W, H, f, d, s = 32, 20, 64.0, 2.0, 1.5
+    hx, hy = (W / 2) * d / f, (H / 2) * d / f
+    pos = [[-hx, -hy, d], [hx, -hy, d], [hx, hy, d], [-hx, hy, d]]
+    uv = [[0, 0], [1, 0], [1, 1], [0, 1]]
+    tex = np.zeros((4, 4, 1, 4), np.float32)
+    tex[..., 0, 3] = 0.4 / Y00
+    ly = L(pos, uv, [[0, 1, 2], [0, 2, 3]], tex)
+    ly.normals = np.array([[-s, 0, -1], [s, 0, -1], [s, 0, -1], [-s, 0, -1]], np.float32)
+    r = oracle.render_view([ly], 0, ident_cam(f, W, H), W, H, attenuation=True, want_layer_rgba=True)
+    a0 = 1.0 / (1.0 + math.exp(-float(np.float32(0.4 / Y00)) * Y00))
+    i = np.arange(W) + 0.5
+    x = -s + 2.0 * s * i / W
+    for j in (0, 7, 19):
+        n = np.stack([x, np.zeros(W), -np.ones(W)], -1)
+        n /= np.linalg.norm(n, axis=1, keepdims=True)
+        v = np.stack([(i - W / 2) / f, np.full(W, (j + 0.5 - H / 2) / f), np.ones(W)], -1)
+        v /= np.linalg.norm(v, axis=1, keepdims=True)
+        want = a0 * (2.0 / (1.0 + np.exp(-10.0 * np.abs((v * n).sum(-1)))) - 1.0)
+        np.testing.assert_allclose(r["layer_rgba"][0, j, :, 3], want, atol=1e-6)
