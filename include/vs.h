@@ -101,7 +101,8 @@ enum {
                                          Attenuation"): every fragment's opacity is multiplied by
                                          alpha_w = 2 Sigmoid(10 |v . n|) - 1 before blending, v = the pixel's
                                          unit view direction, n = the unit geometric normal of the fragment's
-                                         triangle in world space (reading Q13); off by default     */
+                                         triangle in world space, or the interpolated per-vertex normal of layers
+                                         given some (vs_scene_set_vertex_normals; reading Q13); off by default */
 };
 
 typedef struct {
@@ -177,6 +178,20 @@ vs_status vs_scene_create_banded(const vs_scene_desc_banded* desc, void* cuda_st
  *   immutable afterwards.  Device memory held: ~ sum over layers of 16 B/vertex... see DESIGN.md §6.
  */
 vs_status vs_scene_create(const vs_scene_desc* desc, void* cuda_stream, vs_scene** out_scene);
+
+/*
+ * vs_scene_set_vertex_normals -- optional per-vertex normals for the transparency attenuation (
+ * PAPER.md:L279-286 "the angle between the view direction and the surface normal").  Part of building the
+ * scene: call it after vs_scene_create* and before rendering (it waits for the device; the scene is immutable while
+ * renders are in flight).
+ *   normals  HOST array of num_layers pointers; entry l is [num_vertices of layer l][3] floats in `memory` (finite, need
+ *            not be unit length), or NULL: that layer keeps the geometric face normal of the hit triangle.
+ * Under VS_FLAG_ATTENUATION a fragment of a layer WITH normals uses n = normalize(sum_i b'_i n_i), the three vertex normals
+ * interpolated with the fragment's perspective-correct barycentrics (n = 0, hence alpha_w = 0, if the sum vanishes); the
+ * layer_normal buffer of vs_render_aov reports the same vector.  Calling it again replaces the normals of the layers given
+ * and drops those of the others.
+ */
+vs_status vs_scene_set_vertex_normals(vs_scene* scene, const float* const* normals, vs_memory memory, void* cuda_stream);
 
 /*
  * vs_render -- the hot path, steps S1-S7 of DESIGN.md §1 for a batch of cameras:

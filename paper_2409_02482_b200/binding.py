@@ -22,7 +22,7 @@ VS_FLAG_ATTENUATION = 16
 VS_FLAG_OVERLAP = 32
 MISS = 0xFFFFFFFF
 
-EXPORTS = ["vs_scene_create", "vs_scene_create_banded", "vs_render", "vs_render_aov", "vs_render_backward", "vs_render_host", "vs_query_last_render", "vs_scene_destroy",
+EXPORTS = ["vs_scene_create", "vs_scene_create_banded", "vs_scene_set_vertex_normals", "vs_render", "vs_render_aov", "vs_render_backward", "vs_render_host", "vs_query_last_render", "vs_scene_destroy",
            "vs_last_error", "vs_version"]
 
 
@@ -119,6 +119,8 @@ def load_library(build_if_missing: bool = True):
     L.vs_render_backward.restype = C.c_int
     L.vs_render_backward.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(vs_render_params), C.c_void_p,
                                      C.POINTER(C.c_void_p), C.c_void_p]
+    L.vs_scene_set_vertex_normals.restype = C.c_int
+    L.vs_scene_set_vertex_normals.argtypes = [C.c_void_p, C.POINTER(C.c_void_p), C.c_int, C.c_void_p]
     L.vs_query_last_render.restype = C.c_int
     L.vs_query_last_render.argtypes = [C.c_void_p, C.POINTER(vs_render_stats)]
     L.vs_scene_destroy.restype = None
@@ -230,6 +232,30 @@ def vs_scene_create_banded(layers, sh_degree: int, v_min: float, v_max: float, s
     _check(L.vs_scene_create_banded(C.byref(desc), _stream_ptr(stream), C.byref(handle)))
     _SCENES[handle.value] = (k, (sh_degree + 1) ** 2, [(int(ly.band_textures[0].shape[0]), int(ly.band_textures[0].shape[1])) for ly in layers], True)
     return handle.value
+
+
+def vs_scene_set_vertex_normals(scene: int, normals, stream=None):
+    """normals: one entry per layer, a [V_l, 3] float32 array (all numpy = host memory, or all CUDA tensors) or None."""
+    k = _scene_info(scene)[0]
+    assert len(normals) == k, "normals: %d entries for a scene of %d layers" % (len(normals), k)
+    given = [n for n in normals if n is not None]
+    on_host = bool(given) and isinstance(given[0], np.ndarray)
+    keep, ptrs = [], (C.c_void_p * k)()
+    for l, n in enumerate(normals):
+        if n is None:
+            continue
+        if on_host:
+            n = np.ascontiguousarray(n, dtype=np.float32)
+            ptrs[l] = n.ctypes.data
+        else:
+            import torch
+            assert n.is_cuda and n.dtype == torch.float32
+            n = n.contiguous()
+            ptrs[l] = n.data_ptr()
+        assert n.ndim == 2 and n.shape[1] == 3, tuple(n.shape)
+        keep.append(n)
+    _check(load_library().vs_scene_set_vertex_normals(scene, ptrs, VS_MEM_HOST if on_host or not given else VS_MEM_DEVICE,
+                                                      _stream_ptr(stream)))
 
 
 def _cams(cameras):
@@ -373,6 +399,9 @@ class Renderer:
                 self.handle = vs_scene_create(layers, scene.sh_degree)
             del layers
             torch.cuda.empty_cache()
+            normals = [getattr(ly, "normals", None) for ly in scene.layers]
+            if any(n is not None for n in normals):
+                vs_scene_set_vertex_normals(self.handle, [None if n is None else np.ascontiguousarray(n, dtype=np.float32) for n in normals])
 
     def render(self, cameras, params, want_ids=False, out_rgba=None, out_ids=None):
         import torch

@@ -444,6 +444,51 @@ extern "C" vs_status vs_scene_create_banded(const vs_scene_desc_banded* bd, void
 }
 
 
+extern "C" vs_status vs_scene_set_vertex_normals(vs_scene* scene, const float* const* normals, vs_memory memory, void* cuda_stream)
+{
+    g_err[0] = 0;
+    if (!scene || !normals) return fail(VS_ERR_INVALID_ARG, "NULL argument");
+    if (memory != VS_MEM_DEVICE && memory != VS_MEM_HOST) return fail(VS_ERR_INVALID_ARG, "bad memory kind");
+    std::lock_guard<std::mutex> lock(scene->mu);
+    DeviceGuard guard(scene->device);
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    CU(cudaDeviceSynchronize());   // renders in flight read the scene: it changes only while nothing runs
+    VsSceneDev& d = scene->dev;
+    float4* vn = const_cast<float4*>(d.vtx_nrm);
+    if (!vn) {
+        vs_status r = dev_alloc(scene, (void**)&vn, (size_t)d.v_total * 16);
+        if (r != VS_OK) return r;
+        CU(cudaMemsetAsync(vn, 0, (size_t)d.v_total * 16, st));
+    }
+    uint32_t* flag = nullptr;
+    CU(cudaMalloc((void**)&flag, 16));
+    CU(cudaMemsetAsync(flag, 0, 16, st));
+    std::vector<void*> temps;
+    uint32_t mask = 0;
+    vs_status r = VS_OK;
+    for (uint32_t l = 0; l < d.k && r == VS_OK; ++l) {
+        if (!normals[l]) continue;
+        const uint32_t nv = d.vtx_off[l + 1] - d.vtx_off[l];
+        const void* src = nullptr;
+        if ((r = stage_in(normals[l], (size_t)nv * 12, memory, st, temps, &src)) != VS_OK) break;
+        cudaError_t e = vs_launch_check_finite((const float*)src, (size_t)nv * 3, flag, st);
+        if (e == cudaSuccess) e = vs_launch_pack_normals((const float*)src, nv, vn + d.vtx_off[l], st);
+        if (e != cudaSuccess) { r = fail(VS_ERR_CUDA, "vs_scene_set_vertex_normals: %s", cudaGetErrorString(e)); break; }
+        mask |= 1u << l;
+    }
+    uint32_t hflag = 0;
+    if (r == VS_OK && cudaMemcpyAsync(&hflag, flag, 4, cudaMemcpyDeviceToHost, st) != cudaSuccess) r = fail(VS_ERR_CUDA, "copy failed");
+    cudaStreamSynchronize(st);
+    for (void* p : temps) cudaFree(p);
+    cudaFree(flag);
+    cudaGetLastError();
+    if (r != VS_OK) return r;
+    if (hflag & 2u) return fail(VS_ERR_INVALID_ARG, "a vertex normal is not finite");
+    d.vtx_nrm = vn;
+    d.vnrm_mask = mask;
+    return VS_OK;
+}
+
 static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, uint32_t n, const vs_render_params* p,
                                  const void* out_rgba)
 {

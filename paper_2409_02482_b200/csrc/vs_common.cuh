@@ -20,6 +20,8 @@ struct VsSceneDev {
     const uint4* tris;        // [t_total] {i0, i1, i2 : global vertex index, w : layer}
     const float4* tri_nrm;    // [t_total] unit geometric normal in world space (fp64 cross product rounded to fp32), w = 0;
                               //           zero vector for zero-area triangles.  Read only under VS_FLAG_ATTENUATION
+    const float4* vtx_nrm;    // [v_total] optional per-vertex normals (vs_scene_set_vertex_normals), w = 0; nullptr if none
+    uint32_t vnrm_mask;       // bit l: layer l has per-vertex normals (the attenuation then uses the interpolated normal)
     uint32_t v_total, t_total;
     uint32_t k, sh_degree, n_coef;
     uint32_t texel_vecs;                  // 16-byte vectors per texel in the internal layout (= 4 * np_pad * elem / 16)
@@ -253,13 +255,34 @@ __device__ __forceinline__ void vs_texel_coord(float u0, float du, float fW, int
 // Perspective-correct barycentrics b'_1, b'_2 of the sample of pixel (px, py) in the triangle of the transformed vertices a, b, c
 // (b'_i ~ E_i q_i).  The oracle orients the triangle first (swap of vertices 1, 2 when A2 < 0); without the swap
 // every E_i changes sign, and so do the g_i and their sum: the quotients are the same bit for bit, so the setup is skipped here.
-__device__ __forceinline__ void vs_barycentrics(const int4& a, const int4& b, const int4& c, int px, int py, float& b1, float& b2)
+__device__ __forceinline__ void vs_barycentrics3(const int4& a, const int4& b, const int4& c, int px, int py, float& b0, float& b1, float& b2)
 {
     const int Sx = 256 * px + 128, Sy = 256 * py + 128;
     const long long E0 = vs_edge(b.x, b.y, c.x, c.y, Sx, Sy), E1 = vs_edge(c.x, c.y, a.x, a.y, Sx, Sy), E2 = vs_edge(a.x, a.y, b.x, b.y, Sx, Sy);
     const float g0 = __ll2float_rn(E0) * __int_as_float(a.z), g1 = __ll2float_rn(E1) * __int_as_float(b.z), g2 = __ll2float_rn(E2) * __int_as_float(c.z);
     const float inv = __fdividef(1.0f, g0 + g1 + g2);
-    b1 = g1 * inv; b2 = g2 * inv;
+    b0 = g0 * inv; b1 = g1 * inv; b2 = g2 * inv;
+}
+__device__ __forceinline__ void vs_barycentrics(const int4& a, const int4& b, const int4& c, int px, int py, float& b1, float& b2)
+{
+    float b0;
+    vs_barycentrics3(a, b, c, px, py, b0, b1, b2);
+}
+
+// Normal of the fragment of triangle `lid` of layer l at pixel (px, py) for the transparency attenuation and the normal buffer
+// (DESIGN.md §3.9): the unit face normal, or -- if the layer was given per-vertex normals (vs_scene_set_vertex_normals) -- the
+// three vertex normals interpolated with the fragment's perspective-correct barycentrics and renormalised (0 if the sum vanishes).
+__device__ __forceinline__ float4 vs_fragment_normal(const VsSceneDev& sc, const int4* __restrict__ vv, uint32_t l, uint32_t lid, int px, int py)
+{
+    if (!((sc.vnrm_mask >> l) & 1u)) return __ldg(&sc.tri_nrm[sc.tri_off[l] + lid]);
+    const uint4 tri = __ldg(&sc.tris[sc.tri_off[l] + lid]);
+    float b0, b1, b2;
+    vs_barycentrics3(__ldg(&vv[tri.x]), __ldg(&vv[tri.y]), __ldg(&vv[tri.z]), px, py, b0, b1, b2);
+    const float4 n0 = __ldg(&sc.vtx_nrm[tri.x]), n1 = __ldg(&sc.vtx_nrm[tri.y]), n2 = __ldg(&sc.vtx_nrm[tri.z]);
+    const float x = b0 * n0.x + b1 * n1.x + b2 * n2.x, y = b0 * n0.y + b1 * n1.y + b2 * n2.y, z = b0 * n0.z + b1 * n1.z + b2 * n2.z;
+    const float len2 = x * x + y * y + z * z;
+    const float inv = len2 > 0.0f ? rsqrtf(len2) : 0.0f;
+    return make_float4(x * inv, y * inv, z * inv, 0.0f);
 }
 
 // `tri` = index record of the winning triangle of layer l
@@ -341,6 +364,7 @@ cudaError_t vs_launch_backward(const VsSceneDev& sc, int f16, const VsFrame& fr,
 cudaError_t vs_launch_layer_aov(const VsSceneDev& sc, int f16, const VsFrame& fr, uint32_t views, const VsCamDev* cams, const int4* vtx,
                                 const uint32_t* ids, float* layer_rgba, float* layer_uv, float* layer_normal, cudaStream_t st);
 cudaError_t vs_launch_check_finite(const float* v, size_t n, uint32_t* error_flag, cudaStream_t st);
+cudaError_t vs_launch_pack_normals(const float* src, uint32_t n, float4* dst, cudaStream_t st);
 cudaError_t vs_launch_pack_texture(const void* src, int f16, uint32_t n_texels, uint32_t n_coef, uint32_t np_pad, uint32_t frag_layout,
                                    uint4* dst, cudaStream_t st);
 

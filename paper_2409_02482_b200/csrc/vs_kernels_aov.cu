@@ -28,7 +28,7 @@ k_layer_aov(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ 
         if (lid != VS_MISS) {
             float s[4];
             vs_plain_logits<F16>(sc, vv, l, lid, px, py, Y, s, uv);
-            n = sc.tri_nrm[sc.tri_off[l] + lid];
+            n = vs_fragment_normal(sc, vv, l, lid, px, py);
             float A = vs_sigmoid(s[3]);
             if (fr.attenuate) A *= vs_alpha_w(vx, vy, vz, n);
             rgba = make_float4(vs_sigmoid(s[0]), vs_sigmoid(s[1]), vs_sigmoid(s[2]), A);

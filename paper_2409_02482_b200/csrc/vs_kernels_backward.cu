@@ -62,7 +62,7 @@ k_backward(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ c
         ids[l] = lid;
         rgb[l][0] = vs_sigmoid(s[0]); rgb[l][1] = vs_sigmoid(s[1]); rgb[l][2] = vs_sigmoid(s[2]);
         sig3[l] = vs_sigmoid(s[3]);
-        aw[l] = fr.attenuate ? vs_alpha_w(vx, vy, vz, sc.tri_nrm[sc.tri_off[l] + lid]) : 1.0f;
+        aw[l] = fr.attenuate ? vs_alpha_w(vx, vy, vz, vs_fragment_normal(sc, vv, l, lid, px, py)) : 1.0f;
         Tl[l] = Tr;
         used |= 1u << l;
         Tr *= (1.0f - sig3[l] * aw[l]);

@@ -79,6 +79,20 @@ cudaError_t vs_launch_pack_tris(const uint32_t* indices, const float* layer_posi
     return cudaGetLastError();
 }
 
+// per-vertex normals [n][3] -> float4 (w = 0)
+__global__ void k_pack_normals(const float* __restrict__ src, uint32_t n, float4* __restrict__ dst)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) dst[i] = make_float4(src[3 * (size_t)i], src[3 * (size_t)i + 1], src[3 * (size_t)i + 2], 0.0f);
+}
+
+cudaError_t vs_launch_pack_normals(const float* src, uint32_t n, float4* dst, cudaStream_t st)
+{
+    if (n == 0) return cudaSuccess;
+    k_pack_normals<<<(n + 255) / 256, 256, 0, st>>>(src, n, dst);
+    return cudaGetLastError();
+}
+
 cudaError_t vs_launch_check_finite(const float* v, size_t n, uint32_t* error_flag, cudaStream_t st)
 {
     if (n == 0) return cudaSuccess;

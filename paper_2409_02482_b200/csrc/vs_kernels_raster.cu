@@ -312,7 +312,7 @@ k_reference(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ 
         float s[4], uv[2];
         vs_plain_logits<F16>(sc, vv, l, lid, px, py, Y, s, uv);
         float A = vs_sigmoid(s[3]);
-        if (fr.attenuate) A *= vs_alpha_w(vx, vy, vz, sc.tri_nrm[sc.tri_off[l] + lid]);
+        if (fr.attenuate) A *= vs_alpha_w(vx, vy, vz, vs_fragment_normal(sc, vv, l, lid, px, py));
         for (int ch = 0; ch < 3; ++ch) C[ch] += Tr * A * vs_sigmoid(s[ch]);
         Tr *= (1.0f - A);
         if (Tr < fr.t_min) alive = false;

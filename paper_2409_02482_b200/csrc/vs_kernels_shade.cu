@@ -212,7 +212,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
 #pragma unroll
             for (int u = 0; u < VS_MAX_LAYERS; ++u)
                 if (u < (int)sc.k && id[u] != VS_MISS)
-                    rec_aw[u * VS_SHADE_PIX + tid] = vs_alpha_w(vx, vy, vz, __ldg(&sc.tri_nrm[sc.tri_off[u] + id[u]]));
+                    rec_aw[u * VS_SHADE_PIX + tid] = vs_alpha_w(vx, vy, vz, vs_fragment_normal(sc, vv, u, id[u], px, py));
         }
 #pragma unroll
         for (int u = 0; u < VS_MAX_LAYERS; ++u) {

@@ -156,7 +156,7 @@ k_shade_banded(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict
 #pragma unroll
             for (int u = 0; u < VS_MAX_LAYERS; ++u)
                 if (u < (int)sc.k && id[u] != VS_MISS)
-                    rec_aw[u * VS_TILE_PIX + tid] = vs_alpha_w(ax, ay, az, __ldg(&sc.tri_nrm[sc.tri_off[u] + id[u]]));
+                    rec_aw[u * VS_TILE_PIX + tid] = vs_alpha_w(ax, ay, az, vs_fragment_normal(sc, vv, u, id[u], px, py));
         }
     }
     // each thread reads back only its own records: no barrier needed

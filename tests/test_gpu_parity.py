@@ -485,3 +485,36 @@ def test_every_output_is_written_in_bounds(env):
                 assert intact(big, gwin[l].numel(), 777.0), "gradient texture %d: written out of bounds" % l
                 assert float(gwin[l].abs().max()) > 0.0
         r.close()
+
+
+def _with_vertex_normals(sc, which):
+    """Smooth (radial, slightly sheared so that they are NOT the facet normals) per-vertex normals on the layers in `which`."""
+    for l, ly in enumerate(sc.layers):
+        if l in which:
+            n = ly.positions.astype(np.float64)
+            n = n / np.linalg.norm(n, axis=1, keepdims=True) + np.array([0.15, -0.1, 0.05]) * n[:, [1]]
+            ly.normals = (1.7 * n).astype(np.float32)          # deliberately not unit length
+    return sc
+
+
+@pytest.mark.parametrize("banded", [False, True])
+def test_per_vertex_normals_attenuation(env, banded):
+    """SURVEY.md §8(f) NEXT-2, the optional per-vertex normals (vs_scene_set_vertex_normals): layers 0 and 2 carry normals,
+    layer 1 keeps its face normals; image, per-layer opacity / normal buffers and the backward pass against the oracle."""
+    sc = _with_vertex_normals(env.synth.make_config(1, width=120, height=90, num_cameras=2, banded=banded), {0, 2})
+    worst, _, _ = check_against_oracle(env, sc, [0, 1], attenuation=True)
+    check_aov(env, sc, [0, 1], attenuation=True)
+    # the normals matter: the same scene without them renders differently
+    plain = env.synth.make_config(1, width=120, height=90, num_cameras=2, banded=banded)
+    a, _, _ = gpu_render(env, sc, [0], flags=env.binding.VS_FLAG_ATTENUATION, want_ids=False)
+    c, _, _ = gpu_render(env, plain, [0], flags=env.binding.VS_FLAG_ATTENUATION, want_ids=False)
+    assert np.abs(a - c).max() > 1e-3
+    if not banded:
+        check_backward(env, sc, [0, 1], attenuation=True)
+    print("per-vertex normals (%s): worst rgba err %.3e" % ("banded" if banded else "float", worst))
+
+
+def test_per_vertex_normals_reduced_config4(env):
+    sc = _with_vertex_normals(env.synth.make_config(4, mesh_n=40, width=320, height=180, tex_size=256, num_cameras=2), set(range(9)))
+    worst, _, _ = check_against_oracle(env, sc, [0, 1], attenuation=True)
+    print("per-vertex normals, reduced C4: worst rgba err %.3e" % worst)
