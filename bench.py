@@ -403,8 +403,22 @@ def main():
                     help="every other camera of the set: on C5 the r=3 orbit cameras resp. the r=1.6 close-ups (SURVEY.md §8(d))")
     ap.add_argument("--strong", action="store_true", help="multi-GPU: split ONE camera batch evenly over the ranks (strong scaling) instead of one batch per rank")
     ap.add_argument("--lib", default=None, help="load this build of the library (an experiment variant made by `python -m paper_2409_02482_b200.build --lib PATH -D...`)")
+    ap.add_argument("--record-traffic", nargs=4, metavar=("KEY", "DRAM_BYTES_PER_VIEW", "COMMIT", "SUMMARY"), default=None,
+                    help="no benchmark: store the dram__bytes_read+write per view of an `ncu --set full` capture of configuration KEY "
+                         "(e.g. 4, 5-close) in profiles/ncu_traffic.json together with the hashes of the kernel sources as they are now")
     ap.add_argument("--cpu-1thread-seconds", type=float, default=30.0, help="budget of the 1-thread oracle sample (one whole view); skipped if a view would take longer")
     args = ap.parse_args()
+    if args.record_traffic:
+        key, nbytes, commit, summary = args.record_traffic
+        try:
+            table = json.load(open(TRAFFIC_FILE))
+        except Exception:
+            table = {}
+        table[key] = {"kernel": "k_shade", "dram_bytes_per_view": float(nbytes), "commit": commit, "summary": summary,
+                      "source_sha256": kernel_source_hashes()}
+        json.dump(table, open(TRAFFIC_FILE, "w"), indent=1, sort_keys=True)
+        print("recorded", key, "in", TRAFFIC_FILE)
+        return 0
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)

@@ -119,7 +119,7 @@ __device__ __forceinline__ void vs_mma_16816(float& d0, float& d1, float& d2, fl
 #define VS_SHADE_RING 0       // experiment: > 0 = the tensor-core path stages its texel vectors through a shared-memory
 #endif                        // ring of that many fragment columns filled by cp.async (LDGSTS) instead of register buffers
 #define VS_SHADE_PIX (VS_SHADE_WARPS * 32)
-#define VS_SHADE_WARP_BYTES (3072 + VS_SHADE_RING * 2048)   // shared memory per warp: SH basis 2048 + fragment records 512 + logits 512 (+ ring)
+#define VS_SHADE_WARP_BYTES (3584 + VS_SHADE_RING * 2048)   // shared memory per warp: SH basis 2048 + fragment records 2 x 512 + logits 512 (+ ring)
 __device__ __forceinline__ void vs_cp_async16(void* smem_dst, const void* gsrc)
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem_dst)), "l"(gsrc) : "memory");
@@ -153,7 +153,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     // [k][pixels] packed texel coordinates, then [k][pixels] float2 fractions (a < 0: no fragment)
     uint32_t* rec_xy = reinterpret_cast<uint32_t*>(smem);
     float2* rec_ab = reinterpret_cast<float2*>(smem + (size_t)sc.k * VS_SHADE_PIX * 4);
-    unsigned char* per_warp = smem + (size_t)sc.k * VS_SHADE_PIX * 12;  // per warp: 2 KB basis + 512 B records + 512 B logits
+    unsigned char* per_warp = smem + (size_t)sc.k * VS_SHADE_PIX * 12;  // per warp: 2 KB basis + 1 KB records + 512 B logits
     float* rec_aw = reinterpret_cast<float*>(per_warp + VS_SHADE_WARPS * VS_SHADE_WARP_BYTES);   // [k][pixels] attenuation weights (only if fr.attenuate)
 
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -277,8 +277,9 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     float4* ysm = reinterpret_cast<float4*>(per_warp + warp * VS_SHADE_WARP_BYTES);
     // record / logit slabs, one 16-byte chunk per pixel, pixel (row o, column j) at chunk 8 o + ((j + 2 o) & 7):
     // the owners' stores (8 columns of one row) and the octets' accesses (4 rows of one column) are both conflict free
-    uint4* rec_o = reinterpret_cast<uint4*>(per_warp + warp * VS_SHADE_WARP_BYTES + 2048);    // fragment records
-    float4* part = reinterpret_cast<float4*>(per_warp + warp * VS_SHADE_WARP_BYTES + 2560);   // 4 channel logits
+    uint4* rec_o = reinterpret_cast<uint4*>(per_warp + warp * VS_SHADE_WARP_BYTES + 2048);    // texel offsets
+    float4* rec_w = reinterpret_cast<float4*>(per_warp + warp * VS_SHADE_WARP_BYTES + 2560);  // bilinear weights
+    float4* part = reinterpret_cast<float4*>(per_warp + warp * VS_SHADE_WARP_BYTES + 3072);   // 4 channel logits
     const uint32_t own_slot = (lane & 24u) + (((lane & 7u) + 2u * (lane >> 3)) & 7u);
     {
         // SH basis of the owner's pixel (layout: see ysm above)
@@ -347,10 +348,11 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             }
         }
         if (COUNT && lane == 0) atomicAdd(&counters[VS_CNT_FRAGS], (unsigned long long)__popc(m));
-        // one 16-byte record per fragment: {offset of texel 00 | "the footprint has a second column", offset of texel 10, a, b}
-        // (offsets are multiples of NVEC >= 4: the low bits are free); the octets rebuild the other two offsets and the four
-        // weights -- half the shared-memory wavefronts of two records
-        rec_o[own_slot] = make_uint4(r.o00 | (r.o01 != r.o00 ? 1u : 0u), r.o10, __float_as_uint(shade ? ab.x : 0.0f), __float_as_uint(shade ? ab.y : 0.0f));
+        // two 16-byte records per fragment (texel offsets, bilinear weights).  One packed record {offset 00 | flag, offset 10, a, b}
+        // from which the octets rebuild the rest was measured: -22 % shared-memory wavefronts but +15 % instructions, 4.455 vs
+        // 4.375 ms per 16-view launch under ncu, no gain under the power cap (profiles/r2_c4_summary.md)
+        rec_o[own_slot] = make_uint4(r.o00, r.o01, r.o10, r.o11);
+        rec_w[own_slot] = make_float4(r.w00, r.w01, r.w10, r.w11);
         __syncwarp();
         // address = per-lane base + 16 * (32-bit texel-vector offset): one IMAD.WIDE.U32 per load
         const char* __restrict__ tb = reinterpret_cast<const char*>(sc.tex[l] + SLOTS * oi);
@@ -358,15 +360,10 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
         constexpr bool RING = S::MMA && VS_SHADE_RING > 0;
         constexpr int DEPTH = RING ? VS_SHADE_RING : (S::MMA ? VS_SHADE_DEPTH : 2);
         // RING: [stage][texel][lane] 16-byte slots of this warp; a lane reads back only what it copied itself
-        uint4* ring = reinterpret_cast<uint4*>(per_warp + warp * VS_SHADE_WARP_BYTES + 3072);
+        uint4* ring = reinterpret_cast<uint4*>(per_warp + warp * VS_SHADE_WARP_BYTES + 3584);
         uint4 tv[RING ? 1 : DEPTH][SLOTS][4];   // ring of texel vectors: columns j .. j + VS_SHADE_DEPTH - 2 are in flight
-        float fa[DEPTH], fb[DEPTH];  // and the bilinear fractions of their fragments
         auto issue = [&](int j, int b) {
-            const uint4 rec = rec_o[8 * oct + ((j + 2 * oct) & 7)];
-            const uint32_t dxo = (rec.x & 1u) * (uint32_t)S::NVEC;
-            uint4 o;
-            o.x = rec.x & ~3u; o.y = o.x + dxo; o.z = rec.y; o.w = rec.y + dxo;
-            fa[b] = __uint_as_float(rec.z); fb[b] = __uint_as_float(rec.w);
+            const uint4 o = rec_o[8 * oct + ((j + 2 * oct) & 7)];
             if (RING) {
                 const uint32_t off4[4] = {o.x, o.y, o.z, o.w};
 #pragma unroll
@@ -398,9 +395,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
                 for (int q = 0; q < 4; ++q) tv[0][0][q] = ring[(b * 4 + q) * 32 + lane];
             }
             const uint32_t slot = 8 * oct + ((j + 2 * oct) & 7);
-            float4 w;
-            w.x = (1.0f - fa[b]) * (1.0f - fb[b]); w.y = fa[b] * (1.0f - fb[b]);
-            w.z = (1.0f - fa[b]) * fb[b];          w.w = fa[b] * fb[b];
+            const float4 w = rec_w[slot];
             if (S::MMA) {
                 // rows of A = (fragment f = octet, channel), columns of B = (fragment, hi | lo): lane (g = lane >> 2, t = lane & 3)
                 // gets D[g][2t .. 2t+1] and D[g+8][..]; the entries of its OWN fragment are those of t == f
