@@ -137,7 +137,8 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
         const uint32_t wl = __reduce_or_sync(0xFFFFFFFFu, valid ? (1u << layer) : 0u);
         const int nx = wx1 - wx0 + 1, nt = nx * (wy1 - wy0 + 1);
         if (wl != 0u && nt <= 32) {
-            if ((int)lane < nt) atomicOr(&tm[(size_t)(wy0 + (int)lane / nx) * fr.tiles_x + (wx0 + (int)lane % nx)], wl);
+            for (int ty = wy0; ty <= wy1; ++ty)   // (warp-uniform trip count; lanes = tile columns: no integer division)
+                if ((int)lane < nx) atomicOr(&tm[(size_t)ty * fr.tiles_x + (wx0 + (int)lane)], wl);
         } else if (wl != 0u) {
 #pragma unroll
             for (int c = 0; c < 4; ++c) {  // the four corner tiles; a box of at most 8x8 samples touches no other
@@ -165,6 +166,10 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
     uint32_t mlo = 0, mhi = 0;  // coverage of the clipped box, sample (r, c) -> bit 8r + c of mhi:mlo
     int E0 = 0, E1 = 0, E2 = 0, sx0 = 0, sx1 = 0, sx2 = 0, sy0 = 0, sy1 = 0, sy2 = 0;
     const bool small = valid && !large;
+    // The coverage loop below runs max-over-lanes(rows) x max-over-lanes(columns) steps for the whole warp.  A lane whose box is
+    // taller than wide transposes it (loop row = image column): every lane then has rows <= columns, and a warp that holds a
+    // 2x7 and a 7x2 box loops 2x7 times instead of 7x7.  `transposed` travels to phase 2 in the sign bit of the stored A2.
+    const bool transposed = small && (j1 - j0) > (i1 - i0);
     if (small) {
         // edge e_i runs (i+1) -> (i+2) and weights vertex i; sample (i0, j0)
         const int dx0 = T.X2 - T.X1, dy0 = T.Y2 - T.Y1, dx1 = T.X0 - T.X2, dy1 = T.Y0 - T.Y2;
@@ -173,18 +178,24 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
         E0 = dx0 * (Sy - T.Y1) - dy0 * (Sx - T.X1);
         E1 = dx1 * (Sy - T.Y2) - dy1 * (Sx - T.X2);
         E2 = dx2 * (Sy - T.Y0) - dy2 * (Sx - T.X0);
-        sx0 = -256 * dy0; sx1 = -256 * dy1; sx2 = -256 * dy2;  // one pixel in +x
-        sy0 = 256 * dx0; sy1 = 256 * dx1; sy2 = 256 * dx2;     // one pixel in +y
-        // three 16-byte vectors per triangle: {E0, E1, sx0, sx1} {sy0, sy1, A2, key offset} {q0, q1, q2, id}
+        sx0 = -256 * dy0; sx1 = -256 * dy1; sx2 = -256 * dy2;  // one step along a loop row: one pixel in +x ...
+        sy0 = 256 * dx0; sy1 = 256 * dx1; sy2 = 256 * dx2;     // one loop row further: one pixel in +y ...
+        if (transposed) {                                       // ... or the other way round
+            int t;
+            t = sx0; sx0 = sy0; sy0 = t; t = sx1; sx1 = sy1; sy1 = t; t = sx2; sx2 = sy2; sy2 = t;
+        }
+        // three 16-byte vectors per triangle: {E0, E1, sx0, sx1} {sy0, sy1, A2 | transposed << 31, key offset} {q0, q1, q2, id}
+        // (A2 < 2^28 on this path: the triangle is narrow)
         rec4[0 * 32 + lane] = make_int4(E0, E1, sx0, sx1);
-        rec4[1 * 32 + lane] = make_int4(sy0, sy1, (int)T.A2, (int)((uint32_t)(layer * plane_px) + (uint32_t)(j0 * W + i0)));  // < 2^32: checked by the launcher
+        rec4[1 * 32 + lane] = make_int4(sy0, sy1, (int)((uint32_t)T.A2 | (transposed ? 0x80000000u : 0u)),
+                                        (int)((uint32_t)(layer * plane_px) + (uint32_t)(j0 * W + i0)));  // < 2^32: checked by the launcher
         rec4[2 * 32 + lane] = make_int4(__float_as_int(T.q0), __float_as_int(T.q1), __float_as_int(T.q2), (int)lid);
         // covered <=> E_e > 0 || (E_e == 0 && topleft_e) <=> F_e := E_e - (topleft_e ? 0 : 1) >= 0
         E0 -= ((dy0 < 0) || (dy0 == 0 && dx0 > 0)) ? 0 : 1;
         E1 -= ((dy1 < 0) || (dy1 == 0 && dx1 > 0)) ? 0 : 1;
         E2 -= ((dy2 < 0) || (dy2 == 0 && dx2 > 0)) ? 0 : 1;
     }
-    const int nr = small ? j1 - j0 + 1 : 0, nc = small ? i1 - i0 + 1 : 0;
+    const int nr = small ? (transposed ? i1 - i0 : j1 - j0) + 1 : 0, nc = small ? (transposed ? j1 - j0 : i1 - i0) + 1 : 0;
     {
         // rows of up to 8 samples, row and column counts uniform over the warp (the lanes' boxes are alike);
         // samples of a row are visited from column cols-1 down to 0 so that each funnel shift pushes the next lower bit
@@ -231,7 +242,7 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
                 if (off < VS_RD_QUEUE) queue[off] = (unsigned short)((lane << 6) | (uint32_t)bit);
                 ++off;
             }
-            m = mhi;
+            m = mhi;   // (rows 4..7: empty for almost every warp now that rows <= columns)
             while (m) {
                 const int bit = __ffs(m) - 1;
                 m &= m - 1;
@@ -245,15 +256,16 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
         for (uint32_t s = lane; s < n; s += 32) {
             const uint32_t code = queue[s];
             const uint32_t src = code >> 6;
-            const int r = (int)((code >> 3) & 7u), c = (int)(code & 7u);
+            const int r = (int)((code >> 3) & 7u), c = (int)(code & 7u);   // loop row / loop column of the sample
             const int4 ra = rec4[0 * 32 + src], rb = rec4[1 * 32 + src], rc = rec4[2 * 32 + src];
             const int e0 = ra.x + r * rb.x + c * ra.z;
             const int e1 = ra.y + r * rb.y + c * ra.w;
-            const int A2 = rb.z;
+            const int A2 = rb.z & 0x7FFFFFFF;
             const int e2 = A2 - e0 - e1;  // E0 + E1 + E2 == A2 at every point
             const float qp = vs_depth_div(__int2float_rn(e0), __int2float_rn(e1), __int2float_rn(e2),
                                           __int_as_float(rc.x), __int_as_float(rc.y), __int_as_float(rc.z), __int2float_rn(A2));
-            vs_key_red(&vkeys[(uint32_t)rb.w + (uint32_t)(r * W + c)], vs_make_key(qp, (uint32_t)rc.w));
+            const int py = rb.z < 0 ? c : r, pxo = rb.z < 0 ? r : c;        // a transposed box: loop row = image column
+            vs_key_red(&vkeys[(uint32_t)rb.w + (uint32_t)(py * W + pxo)], vs_make_key(qp, (uint32_t)rc.w));
         }
         __syncwarp();
     }
