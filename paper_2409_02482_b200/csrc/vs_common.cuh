@@ -258,8 +258,23 @@ __device__ __forceinline__ void vs_texel_coord(float u0, float du, float fW, int
 __device__ __forceinline__ void vs_barycentrics3(const int4& a, const int4& b, const int4& c, int px, int py, float& b0, float& b1, float& b2)
 {
     const int Sx = 256 * px + 128, Sy = 256 * py + 128;
-    const long long E0 = vs_edge(b.x, b.y, c.x, c.y, Sx, Sy), E1 = vs_edge(c.x, c.y, a.x, a.y, Sx, Sy), E2 = vs_edge(a.x, a.y, b.x, b.y, Sx, Sy);
-    const float g0 = __ll2float_rn(E0) * __int_as_float(a.z), g1 = __ll2float_rn(E1) * __int_as_float(b.z), g2 = __ll2float_rn(E2) * __int_as_float(c.z);
+    // The sample lies inside the triangle (it is the fragment's own pixel), so every difference below is bounded by the
+    // triangle's extent: if that is < 2^12 sub-pixel units (16 px) per axis, the products are < 2^25 and the edge functions
+    // are the same integers in int32 arithmetic (2 IMAD + I2F each instead of 64-bit products and I2F.S64).
+    const int ex = max(abs(b.x - a.x), max(abs(c.x - a.x), abs(c.x - b.x))), ey = max(abs(b.y - a.y), max(abs(c.y - a.y), abs(c.y - b.y)));
+    float f0, f1, f2;
+    if ((ex | ey) < 4096) {
+        const int rx = Sx - a.x, ry = Sy - a.y;                        // sample relative to vertex a
+        const int bx = b.x - a.x, by = b.y - a.y, cx = c.x - a.x, cy = c.y - a.y;
+        const int E1 = cy * rx - cx * ry;                              // edge c -> a at S: (a - c) x (S - c) == c x r  (relative to a)
+        const int E2 = bx * ry - by * rx;                              // edge a -> b at S
+        const int A2 = bx * cy - cx * by;                              // E0 + E1 + E2 == A2 at every point
+        f0 = __int2float_rn(A2 - E1 - E2); f1 = __int2float_rn(E1); f2 = __int2float_rn(E2);
+    } else {
+        f0 = __ll2float_rn(vs_edge(b.x, b.y, c.x, c.y, Sx, Sy)); f1 = __ll2float_rn(vs_edge(c.x, c.y, a.x, a.y, Sx, Sy));
+        f2 = __ll2float_rn(vs_edge(a.x, a.y, b.x, b.y, Sx, Sy));
+    }
+    const float g0 = f0 * __int_as_float(a.z), g1 = f1 * __int_as_float(b.z), g2 = f2 * __int_as_float(c.z);
     const float inv = __fdividef(1.0f, g0 + g1 + g2);
     b0 = g0 * inv; b1 = g1 * inv; b2 = g2 * inv;
 }

@@ -155,7 +155,7 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
         }
     }
 #endif
-    {
+    if (__any_sync(0xFFFFFFFFu, status > 0)) {   // rare: dropped (near plane / guard band) or zero-area triangles in this warp
         const unsigned dropped = __popc(__ballot_sync(0xFFFFFFFFu, status == 1));
         const unsigned degen = __popc(__ballot_sync(0xFFFFFFFFu, status == 2));
         if (lane == 0) {
