@@ -492,7 +492,7 @@ extern "C" vs_status vs_scene_set_vertex_normals(vs_scene* scene, const float* c
 static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, uint32_t n, const vs_render_params* p,
                                  const void* out_rgba)
 {
-    if (!scene || !p || !out_rgba || (n && !cams)) return fail(VS_ERR_INVALID_ARG, "NULL argument");
+    if (!scene || !p || (n && (!cams || !out_rgba))) return fail(VS_ERR_INVALID_ARG, "NULL argument");   // zero cameras: a legal no-op
     if (p->width == 0 || p->height == 0) return fail(VS_ERR_INVALID_ARG, "empty image");
     if (p->width > 16384 || p->height > 16384) return fail(VS_ERR_UNSUPPORTED, "image larger than 16384 px");
     if (!(p->near_plane > 0.0f) || !std::isfinite(p->near_plane)) return fail(VS_ERR_INVALID_ARG, "near_plane must be > 0");

@@ -518,3 +518,59 @@ def test_per_vertex_normals_reduced_config4(env):
     sc = _with_vertex_normals(env.synth.make_config(4, mesh_n=40, width=320, height=180, tex_size=256, num_cameras=2), set(range(9)))
     worst, _, _ = check_against_oracle(env, sc, [0, 1], attenuation=True)
     print("per-vertex normals, reduced C4: worst rgba err %.3e" % worst)
+
+
+def test_asynchronous_calls_on_two_streams_and_threads(env):
+    """vs_render is asynchronous and calls on different streams are legal.  Two batches are rendered on two
+    streams without any synchronisation in between (and once more from two host threads): the images must be those of serial
+    calls bit for bit, also under VS_FLAG_OVERLAP (S1-S4 of the next chunk on the internal stream) and with zero cameras."""
+    import threading
+    b, torch = env.binding, env.torch
+    sc = env.synth.make_config(2, mesh_n=30, width=200, height=150, tex_size=128, num_cameras=6)
+    r = b.Renderer(sc)
+    W, H = sc.width, sc.height
+    p = b.make_params(W, H, sc.near_plane, sc.t_min, sc.background, env.path_flags, 2)
+    sets = [sc.cameras[:3], sc.cameras[3:]]
+    serial = []
+    for cams in sets:
+        out, ids = r.render(cams, p, want_ids=True)
+        torch.cuda.synchronize()
+        serial.append((out.clone(), ids.clone()))
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = [(torch.full((3, H, W, 4), -1.0, device="cuda"), torch.full((3, sc.k, H, W), 7, dtype=torch.int32, device="cuda")) for _ in sets]
+    torch.cuda.synchronize()
+    for rep in range(3):                                   # interleaved, nothing waits in between
+        for i, cams in enumerate(sets):
+            b.vs_render(r.handle, cams, p, outs[i][0], outs[i][1], stream=streams[i])
+    torch.cuda.synchronize()
+    for i in range(2):
+        assert torch.equal(outs[i][0], serial[i][0]) and torch.equal(outs[i][1], serial[i][1]), "stream %d differs from the serial call" % i
+
+    def worker(i):
+        with torch.cuda.stream(streams[i]):
+            for _ in range(3):
+                b.vs_render(r.handle, sets[i], p, outs[i][0], outs[i][1], stream=streams[i])
+    for o in outs:
+        o[0].fill_(-1.0)
+    torch.cuda.synchronize()
+    threads = [threading.Thread(target=worker, args=(i,)) for i in range(2)]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    torch.cuda.synchronize()
+    for i in range(2):
+        assert torch.equal(outs[i][0], serial[i][0]) and torch.equal(outs[i][1], serial[i][1]), "thread %d differs from the serial call" % i
+    if not env.path_flags:
+        po = b.make_params(W, H, sc.near_plane, sc.t_min, sc.background, b.VS_FLAG_OVERLAP, 1)
+        for i, cams in enumerate(sets):
+            outs[i][0].fill_(-1.0)
+            b.vs_render(r.handle, cams, po, outs[i][0], outs[i][1], stream=streams[i])
+        torch.cuda.synchronize()
+        for i in range(2):
+            assert torch.equal(outs[i][0], serial[i][0]) and torch.equal(outs[i][1], serial[i][1]), "VS_FLAG_OVERLAP differs"
+    # zero cameras: a legal no-op
+    b.vs_render(r.handle, np.zeros((0, 16), np.float32), p, torch.empty((0, H, W, 4), device="cuda"))
+    torch.cuda.synchronize()
+    assert r.stats()["dropped_triangles"] == 0
+    r.close()
