@@ -206,7 +206,7 @@ def run_ours(args):
     B, W, H = len(sc.cameras), sc.width, sc.height
     renderer = binding.Renderer(sc, dev)
     path_flag = ((binding.VS_FLAG_TILED_PATH if args.tiled else 0) | (binding.VS_FLAG_ATTENUATION if args.attenuation else 0) |
-                 (binding.VS_FLAG_OVERLAP if args.overlap else 0))
+                 (binding.VS_FLAG_OVERLAP if args.overlap else 0) | (binding.VS_FLAG_SCREEN_ORDER if args.screen_order else 0))
     flags = binding.VS_FLAG_KERNEL_TIMING | path_flag
     params = binding.make_params(W, H, sc.near_plane, sc.t_min, sc.background, flags, args.chunk)
     out = torch.empty((B, H, W, 4), dtype=torch.float32, device=dev)
@@ -295,7 +295,7 @@ def run_ours(args):
     step_achieved = alg_bytes_step * world / (secs_max / args.steps) / 1e9
     views_per_launch = B * args.steps / max(shade_launches, 1)
     traffic_key = "%d%s%s" % (args.config, "-" + args.camera_subset if args.camera_subset else "", "-backward" if args.backward else "")
-    plain = not (args.tiled or args.attenuation or args.overlap or args.views or banded or args.lib)
+    plain = not (args.tiled or args.attenuation or args.overlap or args.screen_order or args.views or banded or args.lib)
     traffic_per_view, traffic_src = ncu_traffic_bytes_per_view(traffic_key) if plain else (None, "not the captured launch configuration")
     # the three candidate bounds of SURVEY.md §8(d), per view: HBM (algorithmic bytes), L1 gather (4 texels per fragment through
     # the 128 B/clk/SM data pipe), FP32 issue (algorithmic lane-ops: 4 x 4n bilinear + SH FMAs, 4 x 4n half->float conversions
@@ -365,7 +365,7 @@ def run_ours(args):
                                   "%s %dx%d" % (sc.layers[0].texture.dtype, sc.layers[0].texture.shape[1], sc.layers[0].texture.shape[0]),
                        "raster_path": "tiled (binning + per-tile shared-memory keys)" if args.tiled
                        else "direct (triangle-parallel, 64-bit max keys in HBM/L2)",
-                       "attenuation": bool(args.attenuation), "overlap": bool(args.overlap), "library": args.lib or "libvs_b200.so",
+                       "attenuation": bool(args.attenuation), "overlap": bool(args.overlap), "shading_order": "screen" if (args.screen_order or args.tiled or banded) else "surface", "library": args.lib or "libvs_b200.so",
                        "timed_loop": "K asynchronous vs_render calls, one stream synchronisation at the end; kernel times from CUDA events on the render stream",
                        "pass": "backward to texels (vs_render_backward)" if args.backward else "forward (vs_render)",
                        "parallelism": "views sharded, scene replicated (dp%d)" % world,
@@ -398,6 +398,7 @@ def main():
     ap.add_argument("--banded", action="store_true", help="the paper's 8-bit mixed-resolution textures on the same geometry (PAPER.md:L445-459; not the headline workload)")
     ap.add_argument("--attenuation", action="store_true", help="render with VS_FLAG_ATTENUATION (PAPER.md:L279-286; not the headline workload)")
     ap.add_argument("--tiled", action="store_true", help="time the per-tile raster path (VS_FLAG_TILED_PATH) instead of the default direct one")
+    ap.add_argument("--screen-order", action="store_true", help="VS_FLAG_SCREEN_ORDER: shade view by view instead of in surface order (A/B, DESIGN.md §7)")
     ap.add_argument("--overlap", action="store_true", help="VS_FLAG_OVERLAP: S1-S4 of the next chunk beside S5-S7 of the current one (experiment, DESIGN.md §7)")
     ap.add_argument("--camera-subset", choices=["far", "close"], default=None,
                     help="every other camera of the set: on C5 the r=3 orbit cameras resp. the r=1.6 close-ups (SURVEY.md §8(d))")

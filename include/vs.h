@@ -97,6 +97,10 @@ enum {
                                          high-priority stream, in one resident CTA per SM, beside S5-S7 of the current
                                          chunk instead of back to back on `cuda_stream`; same outputs bit for bit
                                          (measured slower on B200; off by default)                            */
+    VS_FLAG_SCREEN_ORDER   = 1u << 6, /* shade the (view, tile) pairs of a pass in screen order (view by view) instead of the
+                                         default SURFACE order, in which the tiles of all views of a pass that look at the
+                                         same part of the object are shaded together so that their texels are shared
+                                         through L2; same outputs bit for bit; for A/B measurements        */
     VS_FLAG_ATTENUATION    = 1u << 4  /* transparency attenuation (§4.2 "Transparency
                                          Attenuation"): every fragment's opacity is multiplied by
                                          alpha_w = 2 Sigmoid(10 |v . n|) - 1 before blending, v = the pixel's

@@ -20,6 +20,7 @@ VS_MEM_DEVICE, VS_MEM_HOST = 0, 1
 VS_FLAG_REFERENCE_PATH, VS_FLAG_KERNEL_TIMING, VS_FLAG_COUNT_TEXELS, VS_FLAG_TILED_PATH = 1, 2, 4, 8
 VS_FLAG_ATTENUATION = 16
 VS_FLAG_OVERLAP = 32
+VS_FLAG_SCREEN_ORDER = 64
 MISS = 0xFFFFFFFF
 
 EXPORTS = ["vs_scene_create", "vs_scene_create_banded", "vs_scene_set_vertex_normals", "vs_render", "vs_render_aov", "vs_render_backward", "vs_render_host", "vs_query_last_render", "vs_scene_destroy",

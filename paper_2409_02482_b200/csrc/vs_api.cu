@@ -106,6 +106,7 @@ struct DevBuf {
 // Everything one chunk of views writes besides the caller's outputs.
 struct ScratchSet {
     DevBuf vtx, keys, tile_count, big_list, big_count;                 // direct path (tile_count doubles as the tile masks)
+    DevBuf order, order_work;                                          // direct path: surface order of the (view, tile) pairs
     DevBuf tri_tiles, tile_off, tile_cursor, tile_tris, ids;           // per-tile path
     DevBuf texel_bits;                                                 // VS_FLAG_COUNT_TEXELS
     DevBuf aov_ids;                                                    // vs_render_aov without a caller-supplied id buffer
@@ -116,17 +117,17 @@ struct ScratchSet {
     const DevBuf* named(int i, const char** name) const
     {
         static const char* names[] = {"vtx", "keys", "tile_count", "big_list", "big_count", "tri_tiles", "tile_off", "tile_cursor",
-                                      "tile_tris", "ids", "texel_bits", "aov_ids"};
+                                      "tile_tris", "ids", "texel_bits", "aov_ids", "order", "order_work"};
         const DevBuf* bufs[] = {&vtx, &keys, &tile_count, &big_list, &big_count, &tri_tiles, &tile_off, &tile_cursor, &tile_tris, &ids,
-                                &texel_bits, &aov_ids};
-        if (i < 0 || i >= 12) return nullptr;
+                                &texel_bits, &aov_ids, &order, &order_work};
+        if (i < 0 || i >= 14) return nullptr;
         *name = names[i];
         return bufs[i];
     }
     size_t bytes() const
     {
         return vtx.cap + keys.cap + tile_count.cap + big_list.cap + big_count.cap + tri_tiles.cap + tile_off.cap + tile_cursor.cap +
-               tile_tris.cap + ids.cap + texel_bits.cap + aov_ids.cap;
+               tile_tris.cap + ids.cap + texel_bits.cap + aov_ids.cap + order.cap + order_work.cap;
     }
 };
 
@@ -173,7 +174,7 @@ struct vs_scene {
         for (void* p : owned) cudaFree(p);
         for (ScratchSet& ss : sets) {
             DevBuf* bufs[] = {&ss.vtx, &ss.keys, &ss.tile_count, &ss.big_list, &ss.big_count, &ss.tri_tiles, &ss.tile_off, &ss.tile_cursor,
-                              &ss.tile_tris, &ss.ids, &ss.texel_bits, &ss.aov_ids};
+                              &ss.tile_tris, &ss.ids, &ss.texel_bits, &ss.aov_ids, &ss.order, &ss.order_work};
             for (DevBuf* b : bufs) b->release();
             if (ss.ev_raster) cudaEventDestroy(ss.ev_raster);
             if (ss.ev_done) cudaEventDestroy(ss.ev_done);
@@ -354,9 +355,21 @@ static vs_status scene_create_impl(const vs_scene_desc* desc, const vs_scene_des
     }
     CU(vs_launch_check_finite(pos, (size_t)vt * 3, flag, st));
     CU(vs_launch_check_finite((const float*)uvs, (size_t)vt * 2, flag, st));
+    int* bb;
+    if ((r = dev_alloc(s, (void**)&bb, 32)) != VS_OK) return r;
+    CU(vs_launch_bbox(pos, (uint32_t)vt, bb, st));
     uint32_t hflag = 0;
+    int hbb[6];
     CU(cudaMemcpyAsync(&hflag, flag, 4, cudaMemcpyDeviceToHost, st));
+    CU(cudaMemcpyAsync(hbb, bb, sizeof(hbb), cudaMemcpyDeviceToHost, st));
     CU(cudaStreamSynchronize(st));
+    for (int a = 0; a < 3; ++a) {   // (order-preserving ints back to floats; an empty scene gets a unit box)
+        const int lo = hbb[a] ^ ((hbb[a] >> 31) & 0x7FFFFFFF), hi = hbb[3 + a] ^ ((hbb[3 + a] >> 31) & 0x7FFFFFFF);
+        float fmin, fmax;
+        memcpy(&fmin, &lo, 4); memcpy(&fmax, &hi, 4);
+        if (!vt || !(fmax > fmin)) { fmin = vt ? fmin : 0.0f; fmax = fmin + 1.0f; }
+        d.bb_min[a] = fmin; d.bb_scale[a] = 32.0f / (fmax - fmin);
+    }
     if (hflag & 1u) return fail(VS_ERR_INVALID_ARG, "a triangle index is >= num_vertices of its layer");
     if (hflag & 2u) return fail(VS_ERR_INVALID_ARG, "a vertex position or uv is not finite");
     d.positions = pos; d.uvs = uvs; d.tris = tris; d.tri_nrm = nrm;
@@ -498,7 +511,7 @@ static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, u
     if (!(p->near_plane > 0.0f) || !std::isfinite(p->near_plane)) return fail(VS_ERR_INVALID_ARG, "near_plane must be > 0");
     if (!(p->t_min >= 0.0f) || !std::isfinite(p->t_min)) return fail(VS_ERR_INVALID_ARG, "t_min must be >= 0");
     if (p->flags & ~(uint32_t)(VS_FLAG_REFERENCE_PATH | VS_FLAG_KERNEL_TIMING | VS_FLAG_COUNT_TEXELS | VS_FLAG_TILED_PATH |
-                               VS_FLAG_ATTENUATION | VS_FLAG_OVERLAP))
+                               VS_FLAG_ATTENUATION | VS_FLAG_OVERLAP | VS_FLAG_SCREEN_ORDER))
         return fail(VS_ERR_INVALID_ARG, "reserved flag bits set");
     for (int i = 0; i < 3; ++i)
         if (!std::isfinite(p->background[i])) return fail(VS_ERR_INVALID_ARG, "background not finite");
@@ -567,6 +580,7 @@ struct Call {
     cudaStream_t st;      // the caller's stream: consumers (S5-S7) and everything the caller may wait for
     cudaStream_t rs;      // the stream of S1-S4: the scene's aux stream when the call is pipelined, else `st`
     bool timing, reference, tiled;
+    bool ordered;         // direct path: the consumer takes its (view, tile) pairs in surface order (vs_kernels_order.cu)
     CallMode mode;
     const float* grad_rgba;         // MODE_BACKWARD: [num_cameras][H][W][4]
     VsGradTex grad_tex;
@@ -587,6 +601,8 @@ static vs_status begin_call(vs_scene* s, Call& c, const vs_camera* cams, uint32_
     c.timing = (p->flags & VS_FLAG_KERNEL_TIMING) != 0;
     c.reference = (p->flags & VS_FLAG_REFERENCE_PATH) != 0;
     c.tiled = (p->flags & VS_FLAG_TILED_PATH) != 0;
+    // banded scenes keep screen order: their textures are 8x smaller and k_shade_banded leaves the HBM idle
+    c.ordered = !c.reference && !c.tiled && !(p->flags & VS_FLAG_SCREEN_ORDER) && !s->dev.banded;
     // VS_FLAG_OVERLAP (direct path only): S1-S4 go to the internal stream so that they run beside the previous chunk's or
     // the previous call's shading.  Measured slower than back to back on B200 (both kernels are bound by the
     // warps the register file holds), hence opt-in
@@ -656,6 +672,7 @@ static VsChunk make_chunk(const Call& c, ScratchSet& ss, uint32_t views, float* 
         ch.big_count = (uint32_t*)ss.big_count.p;
         ch.big_capacity = 65536;
         ch.tile_mask = ch.tile_count;
+        if (c.ordered) ch.order = (const uint32_t*)ss.order.p;
     }
     if ((c.p->flags & VS_FLAG_COUNT_TEXELS) && c.s->dev.banded) ch.count_fragments = 1;   // banded scenes: fragments only
     else if (c.p->flags & VS_FLAG_COUNT_TEXELS) ch.texel_bits = (uint32_t*)ss.texel_bits.p;
@@ -684,6 +701,10 @@ static vs_status enqueue_geometry(Call& c, ScratchSet& ss, uint32_t views, uint3
         CU(ss.tile_count.reserve(ntile * 4, s->pool, c.rs));   // per-tile layer masks
         CU(ss.big_list.reserve((size_t)65536 * 8, s->pool, c.rs));
         CU(ss.big_count.reserve(16, s->pool, c.rs));
+        if (c.ordered) {
+            CU(ss.order.reserve(ntile * 4 + 16, s->pool, c.rs));
+            CU(ss.order_work.reserve((2 * ntile + VS_ORDER_BINS) * 4 + 16, s->pool, c.rs));
+        }
     }
     if (!c.reference && c.tiled) {
         CU(ss.tri_tiles.reserve((size_t)s->dev.t_total * views * 4 + 16, s->pool, c.rs));
@@ -724,6 +745,10 @@ static vs_status enqueue_geometry(Call& c, ScratchSet& ss, uint32_t views, uint3
 #endif
         if ((r = span_begin(s, c.timing, 2, c.rs)) != VS_OK) return r;
         CU(vs_launch_raster_direct(s->dev, fr, ch, c.rs, resident ? s->resident_ctas : 0u));
+        if (c.ordered) {   // counted with the raster stage: it is part of what S4 hands to the consumer
+            CU(vs_launch_order(s->dev, fr, ch, (uint32_t*)ss.order.p, (uint32_t*)ss.order_work.p, c.rs));
+            s->launches += 3;
+        }
         if ((r = span_end(s, c.timing, c.rs)) != VS_OK) return r;
         s->launches += s->dev.t_total ? 2 : 0;
         s->raster_launches += 1;

@@ -12,6 +12,7 @@
 #define VS_TILE_H 16
 #define VS_TILE_PIX (VS_TILE_W * VS_TILE_H)
 #define VS_MISS 0xFFFFFFFFu
+#define VS_ORDER_BINS 32769u   // surface-order sort keys: 15-bit Morton code of a 32^3 cell + one bin for "nothing at the probes"
 
 // Device-side description of an immutable scene (passed by value to kernels).
 struct VsSceneDev {
@@ -27,6 +28,7 @@ struct VsSceneDev {
     uint32_t texel_vecs;                  // 16-byte vectors per texel in the internal layout (= 4 * np_pad * elem / 16)
     uint32_t np_pad;                      // coefficients per channel row of the internal layout [texel][ch][np_pad]
     uint32_t frag_layout;                 // 1: fp16 texels of 16 (padded) coefficients stored in mma A-fragment order (see below)
+    float bb_min[3], bb_scale[3];         // object-space bounding box of all vertices: cell = (p - bb_min) * bb_scale in [0, 32) (vs_kernels_order.cu)
     uint32_t tri_off[VS_MAX_LAYERS + 1];  // global triangle id of each layer's triangle 0
     uint32_t vtx_off[VS_MAX_LAYERS + 1];  // global vertex index of each layer's vertex 0
     const uint4* tex[VS_MAX_LAYERS];      // [tex_h][tex_w][texel_vecs] 16-byte vectors
@@ -358,6 +360,7 @@ struct VsChunk {                 // one pass over `views` cameras
     uint32_t* big_count;         // DEVICE entries appended this chunk (may exceed big_capacity: the rest was done in place)
     uint32_t big_capacity;
     uint32_t* tile_mask;         // DEVICE [views][tiles] layers whose triangles' boxes touch the 16x16 tile (zero on entry)
+    const uint32_t* order;       // DEVICE [views * tiles] (view * tiles + tile) in shading order, or nullptr = screen order
 };
 
 cudaError_t vs_launch_transform(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
@@ -367,6 +370,8 @@ cudaError_t vs_launch_bin_scatter(const VsSceneDev& sc, const VsFrame& fr, const
 cudaError_t vs_launch_raster_direct(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st, uint32_t resident_ctas);
 cudaError_t vs_launch_raster(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_shade(const VsSceneDev& sc, int tex_f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_order(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, uint32_t* order, uint32_t* work, cudaStream_t st);
+cudaError_t vs_launch_bbox(const float* pos, uint32_t n_vertices, int* bb6, cudaStream_t st);
 cudaError_t vs_launch_popcount(const uint32_t* words, size_t n, unsigned long long* counter, cudaStream_t st);
 cudaError_t vs_launch_reference(const VsSceneDev& sc, int tex_f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 

@@ -23,11 +23,15 @@ template <int F16>
 __global__ void __launch_bounds__(256, 3)
 k_backward(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams, const int4* __restrict__ vtx,
            const uint32_t* __restrict__ tile_mask, unsigned long long* __restrict__ keys, const float* __restrict__ grad_out,
-           VsGradTex gt)
+           VsGradTex gt, const uint32_t* __restrict__ order)
 {
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t tile = blockIdx.x, view = blockIdx.y;
     const uint32_t tiles = fr.tiles_x * fr.tiles_y;
+    uint32_t tile = blockIdx.x, view = blockIdx.y;
+    if (order) {   // surface order (vs_kernels_order.cu): the views' updates of a gradient texel meet in L2
+        const uint32_t e = __ldg(&order[view * tiles + tile]);
+        view = e / tiles; tile = e - view * tiles;
+    }
     const int W = (int)fr.width, H = (int)fr.height;
     const int lx = (int)(warp & 1) * 8 + (int)(lane & 7), ly = (int)(warp >> 1) * 4 + (int)(lane >> 3);
     const int px = (int)(tile % fr.tiles_x) * VS_TILE_W + lx, py = (int)(tile / fr.tiles_x) * VS_TILE_H + ly;
@@ -140,7 +144,7 @@ cudaError_t vs_launch_backward(const VsSceneDev& sc, int f16, const VsFrame& fr,
 {
     dim3 grid(fr.tiles_x * fr.tiles_y, ch.views);
     const size_t smem = 8 * 3584;
-    if (f16) k_backward<1><<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_mask, ch.keys, ch.grad_out, ch.grad_tex);
-    else k_backward<0><<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_mask, ch.keys, ch.grad_out, ch.grad_tex);
+    if (f16) k_backward<1><<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_mask, ch.keys, ch.grad_out, ch.grad_tex, ch.order);
+    else k_backward<0><<<grid, 256, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_mask, ch.keys, ch.grad_out, ch.grad_tex, ch.order);
     return cudaGetLastError();
 }

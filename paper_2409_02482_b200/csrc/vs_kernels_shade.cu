@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(VS_SHADE_PIX, VS_SHADE_MIN_CTAS)
 k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams, const int4* __restrict__ vtx,
         const uint32_t* __restrict__ tile_off, const uint32_t* __restrict__ ids, unsigned long long* __restrict__ keys,
         uint32_t* __restrict__ out_ids, float* __restrict__ out_rgba,
-        uint32_t* __restrict__ texel_bits, unsigned long long* __restrict__ counters)
+        uint32_t* __restrict__ texel_bits, unsigned long long* __restrict__ counters, const uint32_t* __restrict__ order)
 {
     typedef VsShadeShape<F16, DEG> S;
     constexpr int SLOTS = S::SLOTS, LPC = S::LPC, NACT = S::NACT, NE = S::NE, PPV = S::PPV;
@@ -157,8 +157,13 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     float* rec_aw = reinterpret_cast<float*>(per_warp + VS_SHADE_WARPS * VS_SHADE_WARP_BYTES);   // [k][pixels] attenuation weights (only if fr.attenuate)
 
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const uint32_t tile = blockIdx.x / VS_SHADE_SUBTILES, sub = blockIdx.x % VS_SHADE_SUBTILES, view = blockIdx.y;
     const uint32_t tiles = fr.tiles_x * fr.tiles_y;
+    uint32_t tile = blockIdx.x / VS_SHADE_SUBTILES, view = blockIdx.y;
+    const uint32_t sub = blockIdx.x % VS_SHADE_SUBTILES;
+    if (order) {   // surface order (vs_kernels_order.cu): CTAs are dispatched in launch order, entry = linear CTA index
+        const uint32_t e = __ldg(&order[view * tiles + tile]);
+        view = e / tiles; tile = e - view * tiles;
+    }
     const int W = (int)fr.width, H = (int)fr.height;
     // lane -> pixel of the warp's 8x4 block: column = lane & 7, row = lane >> 3
     const int lx = (int)(warp & 1) * 8 + (int)(lane & 7), ly = (int)(sub * (VS_SHADE_WARPS / 2) + (warp >> 1)) * 4 + (int)(lane >> 3);
@@ -482,10 +487,10 @@ static cudaError_t launch_sh2(const VsSceneDev& sc, const VsFrame& fr, const VsC
     dim3 grid(fr.tiles_x * fr.tiles_y * VS_SHADE_SUBTILES, ch.views);
     if (ch.keys)
         kern<<<grid, VS_SHADE_PIX, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_mask, nullptr, ch.keys, ch.ids_is_output ? ch.ids : nullptr,
-                                      ch.out_rgba, ch.texel_bits, ch.counters);
+                                      ch.out_rgba, ch.texel_bits, ch.counters, ch.order);
     else
         kern<<<grid, VS_SHADE_PIX, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_off, ch.ids, nullptr, nullptr, ch.out_rgba, ch.texel_bits,
-                                      ch.counters);
+                                      ch.counters, nullptr);
     return cudaGetLastError();
 }
 

@@ -311,6 +311,25 @@ def test_determinism_and_chunking(env):
         assert np.array_equal(a[0], x[0]) and np.array_equal(a[1], x[1])
 
 
+def test_surface_order_is_a_permutation_of_screen_order(env):
+    """The default shading order (the (view, tile) pairs of a pass sorted by where on the object they look,
+    vs_kernels_order.cu) changes scheduling only: images and ids are bit-identical to VS_FLAG_SCREEN_ORDER, for forward,
+    AOV-less backward and every chunking (a lost or doubled entry of the sorted list would leave a tile unshaded)."""
+    b = env.binding
+    sc = env.synth.make_config(4, mesh_n=40, width=333, height=217, tex_size=128, num_cameras=7)
+    ref = gpu_render(env, sc, range(7), flags=b.VS_FLAG_SCREEN_ORDER)
+    for chunk in (0, 1, 3, 7):
+        got = gpu_render(env, sc, range(7), views_per_chunk=chunk)
+        assert np.array_equal(ref[0], got[0]) and np.array_equal(ref[1], got[1])
+    # a scene whose box is degenerate in one axis (a single quad), and an empty view (camera looking away)
+    quad = env.synth.make_config(1, width=90, height=70, num_cameras=3, tex_size=32)
+    for ly in quad.layers:
+        ly.positions[:, 2] = 0.25
+    a = gpu_render(env, quad, range(3), flags=b.VS_FLAG_SCREEN_ORDER)
+    c = gpu_render(env, quad, range(3))
+    assert np.array_equal(a[0], c[0]) and np.array_equal(a[1], c[1])
+
+
 @pytest.mark.parametrize("dtype,deg", [(np.float32, 0), (np.float16, 0), (np.float16, 1), (np.float32, 2), (np.float32, 3)])
 def test_all_texture_formats(env, dtype, deg):
     rng = np.random.default_rng(5)
