@@ -12,7 +12,10 @@
 #define VS_TILE_H 16
 #define VS_TILE_PIX (VS_TILE_W * VS_TILE_H)
 #define VS_MISS 0xFFFFFFFFu
-#define VS_ORDER_BINS 32769u   // surface-order sort keys: 15-bit Morton code of a 32^3 cell + one bin for "nothing at the probes"
+#ifndef VS_ORDER_BITS
+#define VS_ORDER_BITS 7        // surface-order sort keys: cells per axis of the octahedral map = 2^VS_ORDER_BITS
+#endif
+#define VS_ORDER_BINS ((VS_ORDER_BITS > 7 ? (1u << (2 * VS_ORDER_BITS)) : 32768u) + 1u)   // + one bin for "nothing at the probes"
 
 // Device-side description of an immutable scene (passed by value to kernels).
 struct VsSceneDev {

@@ -23,6 +23,9 @@ __device__ __forceinline__ uint32_t vs_spread3(uint32_t v)   // 5 bits -> every 
     return v;
 }
 
+#ifndef VS_ORDER_LAYER_NUM
+#define VS_ORDER_LAYER_NUM 3   // the probe starts at layer k * VS_ORDER_LAYER_NUM / 8
+#endif
 #ifndef VS_ORDER_MODE
 #define VS_ORDER_MODE 1   // 0: Morton code of a 32^3 object-space cell; 1: Hilbert index of the octahedral map of the direction from the box centre
 #endif
@@ -61,7 +64,11 @@ k_order_key(const VsSceneDev sc, const VsFrame fr, const unsigned long long* __r
         bool found = false;
         for (int p = 0; p < 5 && !found; ++p) {
             const int px = min(x0 + probe_x[p], W - 1), py = min(y0 + probe_y[p], H - 1);
-            for (uint32_t l = 0; l < sc.k && !found; ++l) {
+            for (uint32_t li = 0; li < sc.k && !found; ++li) {
+                // start at a layer a third of the way in (VS_ORDER_LAYER_NUM / 8 of k): seen from different directions, the
+                // fragments of a pixel's deeper layers lie on different parts of the inner shells (parallax), and a
+                // reference layer in the middle of the shaded ones halves the largest offset
+                const uint32_t l = (li + (sc.k * VS_ORDER_LAYER_NUM) / 8u) % sc.k;
                 if (!((lmask >> l) & 1u)) continue;
                 const unsigned long long kk = keys[((size_t)view * sc.k + l) * plane + (size_t)py * W + px];
                 if (!kk) continue;
@@ -75,7 +82,7 @@ k_order_key(const VsSceneDev sc, const VsFrame fr, const unsigned long long* __r
                     const uint32_t iz = (uint32_t)min(max((int)cz, 0), 31);
                     key = vs_spread3(ix) | (vs_spread3(iy) << 1) | (vs_spread3(iz) << 2);
                 } else {
-                    // direction from the box centre in box units -> octahedral map -> 128 x 128 cells along a Hilbert curve: a
+                    // direction from the box centre in box units -> octahedral map -> 2^VS_ORDER_BITS squared cells along a Hilbert curve: a
                     // range of consecutive keys is a compact patch of the object's surface
                     float dx = cx - 16.0f, dy = cy - 16.0f, dz = cz - 16.0f;
                     const float n1 = fabsf(dx) + fabsf(dy) + fabsf(dz);
@@ -83,9 +90,10 @@ k_order_key(const VsSceneDev sc, const VsFrame fr, const unsigned long long* __r
                     dx *= inv; dy *= inv; dz *= inv;
                     float ox = dx, oy = dy;
                     if (dz < 0.0f) { ox = (1.0f - fabsf(dy)) * (dx < 0.0f ? -1.0f : 1.0f); oy = (1.0f - fabsf(dx)) * (dy < 0.0f ? -1.0f : 1.0f); }
-                    const uint32_t ux = (uint32_t)min(max((int)((ox * 0.5f + 0.5f) * 128.0f), 0), 127);
-                    const uint32_t uy = (uint32_t)min(max((int)((oy * 0.5f + 0.5f) * 128.0f), 0), 127);
-                    key = vs_hilbert2(ux, uy, 7);
+                    constexpr int NC = 1 << VS_ORDER_BITS;
+                    const uint32_t ux = (uint32_t)min(max((int)((ox * 0.5f + 0.5f) * (float)NC), 0), NC - 1);
+                    const uint32_t uy = (uint32_t)min(max((int)((oy * 0.5f + 0.5f) * (float)NC), 0), NC - 1);
+                    key = vs_hilbert2(ux, uy, VS_ORDER_BITS);
                 }
                 found = true;
             }
