@@ -13,9 +13,12 @@
 #define VS_TILE_PIX (VS_TILE_W * VS_TILE_H)
 #define VS_MISS 0xFFFFFFFFu
 #ifndef VS_ORDER_BITS
-#define VS_ORDER_BITS 7        // surface-order sort keys: cells per axis of the octahedral map = 2^VS_ORDER_BITS
+#define VS_ORDER_BITS 6        // surface-order sort keys: cells per axis of the octahedral map = 2^VS_ORDER_BITS (5..8 measure the same)
 #endif
-#define VS_ORDER_BINS ((VS_ORDER_BITS > 7 ? (1u << (2 * VS_ORDER_BITS)) : 32768u) + 1u)   // + one bin for "nothing at the probes"
+#ifndef VS_ORDER_MODE
+#define VS_ORDER_MODE 1        // 1: Hilbert index of the octahedral map of the direction from the box centre; 0: Morton code of a 32^3 cell
+#endif
+#define VS_ORDER_BINS ((VS_ORDER_MODE == 0 ? 32768u : (1u << (2 * VS_ORDER_BITS))) + 1u)   // + one bin for "nothing at the probes"
 
 // Device-side description of an immutable scene (passed by value to kernels).
 struct VsSceneDev {

@@ -26,9 +26,6 @@ __device__ __forceinline__ uint32_t vs_spread3(uint32_t v)   // 5 bits -> every 
 #ifndef VS_ORDER_LAYER_NUM
 #define VS_ORDER_LAYER_NUM 3   // the probe starts at layer k * VS_ORDER_LAYER_NUM / 8
 #endif
-#ifndef VS_ORDER_MODE
-#define VS_ORDER_MODE 1   // 0: Morton code of a 32^3 object-space cell; 1: Hilbert index of the octahedral map of the direction from the box centre
-#endif
 
 // Hilbert curve index of cell (x, y) of a 2^bits x 2^bits grid
 __device__ __forceinline__ uint32_t vs_hilbert2(uint32_t x, uint32_t y, int bits)
@@ -59,48 +56,62 @@ k_order_key(const VsSceneDev sc, const VsFrame fr, const unsigned long long* __r
     const uint32_t lmask = tile_mask[vt];
     uint32_t key = VS_ORDER_BINS - 1u;   // nothing found: background and silhouette-corner tiles go last
     if (lmask) {
-        // centre of the tile first, then the centres of its quadrants; front-most layer first
+        // centre of the tile first, then the centres of its quadrants; per probe the keys of all layers are requested at once
         const int probe_x[5] = {8, 4, 12, 12, 4}, probe_y[5] = {8, 4, 12, 4, 12};
-        bool found = false;
-        for (int p = 0; p < 5 && !found; ++p) {
+        // the reference layer: start a third of the way in (VS_ORDER_LAYER_NUM / 8 of k).  Seen from different directions, the
+        // fragments of a pixel's deeper layers lie on different parts of the inner shells (parallax); a reference layer in
+        // the middle of the shaded ones halves the largest offset (k_shade DRAM reads 11.7 -> 8.5 GB per 16-view C4 launch)
+        const uint32_t l0 = (sc.k * VS_ORDER_LAYER_NUM) / 8u;
+        for (int p = 0; p < 5; ++p) {
             const int px = min(x0 + probe_x[p], W - 1), py = min(y0 + probe_y[p], H - 1);
-            for (uint32_t li = 0; li < sc.k && !found; ++li) {
-                // start at a layer a third of the way in (VS_ORDER_LAYER_NUM / 8 of k): seen from different directions, the
-                // fragments of a pixel's deeper layers lie on different parts of the inner shells (parallax), and a
-                // reference layer in the middle of the shaded ones halves the largest offset
-                const uint32_t l = (li + (sc.k * VS_ORDER_LAYER_NUM) / 8u) % sc.k;
-                if (!((lmask >> l) & 1u)) continue;
-                const unsigned long long kk = keys[((size_t)view * sc.k + l) * plane + (size_t)py * W + px];
-                if (!kk) continue;
-                const uint32_t lid = 0xFFFFFFFFu - (uint32_t)kk;
-                const uint4 tri = __ldg(&sc.tris[sc.tri_off[l] + lid]);
-                const float* P = sc.positions + (size_t)tri.x * 3;
-                const float cx = (__ldg(P) - sc.bb_min[0]) * sc.bb_scale[0], cy = (__ldg(P + 1) - sc.bb_min[1]) * sc.bb_scale[1];
-                const float cz = (__ldg(P + 2) - sc.bb_min[2]) * sc.bb_scale[2];
-                if (VS_ORDER_MODE == 0) {
-                    const uint32_t ix = (uint32_t)min(max((int)cx, 0), 31), iy = (uint32_t)min(max((int)cy, 0), 31);
-                    const uint32_t iz = (uint32_t)min(max((int)cz, 0), 31);
-                    key = vs_spread3(ix) | (vs_spread3(iy) << 1) | (vs_spread3(iz) << 2);
-                } else {
-                    // direction from the box centre in box units -> octahedral map -> 2^VS_ORDER_BITS squared cells along a Hilbert curve: a
-                    // range of consecutive keys is a compact patch of the object's surface
-                    float dx = cx - 16.0f, dy = cy - 16.0f, dz = cz - 16.0f;
-                    const float n1 = fabsf(dx) + fabsf(dy) + fabsf(dz);
-                    const float inv = n1 > 0.0f ? 1.0f / n1 : 0.0f;
-                    dx *= inv; dy *= inv; dz *= inv;
-                    float ox = dx, oy = dy;
-                    if (dz < 0.0f) { ox = (1.0f - fabsf(dy)) * (dx < 0.0f ? -1.0f : 1.0f); oy = (1.0f - fabsf(dx)) * (dy < 0.0f ? -1.0f : 1.0f); }
-                    constexpr int NC = 1 << VS_ORDER_BITS;
-                    const uint32_t ux = (uint32_t)min(max((int)((ox * 0.5f + 0.5f) * (float)NC), 0), NC - 1);
-                    const uint32_t uy = (uint32_t)min(max((int)((oy * 0.5f + 0.5f) * (float)NC), 0), NC - 1);
-                    key = vs_hilbert2(ux, uy, VS_ORDER_BITS);
-                }
-                found = true;
+            const unsigned long long* kp = keys + (size_t)view * sc.k * plane + (size_t)py * W + px;
+            unsigned long long kk[VS_MAX_LAYERS];
+#pragma unroll
+            for (int l = 0; l < VS_MAX_LAYERS; ++l) kk[l] = ((uint32_t)l < sc.k && ((lmask >> l) & 1u)) ? kp[(size_t)l * plane] : 0ull;
+            unsigned long long hit = 0ull;
+            uint32_t hl = 0, best = 0xFFFFFFFFu;   // the hit layer that comes first in the order l0, l0 + 1, ..., k - 1, 0, ..., l0 - 1
+#pragma unroll
+            for (int l = 0; l < VS_MAX_LAYERS; ++l) {
+                const uint32_t rank = ((uint32_t)l + sc.k - l0) % sc.k;
+                if (kk[l] && rank < best) { best = rank; hit = kk[l]; hl = (uint32_t)l; }
             }
+            if (!hit) continue;
+            const uint32_t lid = 0xFFFFFFFFu - (uint32_t)hit;
+            const uint4 tri = __ldg(&sc.tris[sc.tri_off[hl] + lid]);
+            const float* P = sc.positions + (size_t)tri.x * 3;
+            const float cx = (__ldg(P) - sc.bb_min[0]) * sc.bb_scale[0], cy = (__ldg(P + 1) - sc.bb_min[1]) * sc.bb_scale[1];
+            const float cz = (__ldg(P + 2) - sc.bb_min[2]) * sc.bb_scale[2];
+            if (VS_ORDER_MODE == 0) {
+                const uint32_t ix = (uint32_t)min(max((int)cx, 0), 31), iy = (uint32_t)min(max((int)cy, 0), 31);
+                const uint32_t iz = (uint32_t)min(max((int)cz, 0), 31);
+                key = vs_spread3(ix) | (vs_spread3(iy) << 1) | (vs_spread3(iz) << 2);
+            } else {
+                // direction from the box centre in box units -> octahedral map -> 2^VS_ORDER_BITS squared cells along a Hilbert
+                // curve: a range of consecutive keys is a compact patch of the object's surface
+                float dx = cx - 16.0f, dy = cy - 16.0f, dz = cz - 16.0f;
+                const float n1 = fabsf(dx) + fabsf(dy) + fabsf(dz);
+                const float inv = n1 > 0.0f ? 1.0f / n1 : 0.0f;
+                dx *= inv; dy *= inv; dz *= inv;
+                float ox = dx, oy = dy;
+                if (dz < 0.0f) { ox = (1.0f - fabsf(dy)) * (dx < 0.0f ? -1.0f : 1.0f); oy = (1.0f - fabsf(dx)) * (dy < 0.0f ? -1.0f : 1.0f); }
+                constexpr int NC = 1 << VS_ORDER_BITS;
+                const uint32_t ux = (uint32_t)min(max((int)((ox * 0.5f + 0.5f) * (float)NC), 0), NC - 1);
+                const uint32_t uy = (uint32_t)min(max((int)((oy * 0.5f + 0.5f) * (float)NC), 0), NC - 1);
+                key = vs_hilbert2(ux, uy, VS_ORDER_BITS);
+            }
+            break;
         }
     }
     okey[vt] = key;
-    orank[vt] = atomicAdd(&hist[key], 1u);
+    // rank inside the bin: one atomic per distinct key of the warp (most background tiles share ONE bin: per-thread atomics on
+    // it serialise in L2 and took 55 of the kernel's 60 us)
+    const uint32_t active = __activemask();
+    const uint32_t peers = __match_any_sync(active, key);
+    const uint32_t leader = (uint32_t)__ffs(peers) - 1u, lane = threadIdx.x & 31u;
+    uint32_t base = 0;
+    if (lane == leader) base = atomicAdd(&hist[key], (uint32_t)__popc(peers));
+    base = __shfl_sync(peers, base, (int)leader);
+    orank[vt] = base + (uint32_t)__popc(peers & ((1u << lane) - 1u));
 }
 
 // one CTA of 1024 threads: hist[VS_ORDER_BINS] -> exclusive prefix sums, in place

@@ -24,7 +24,7 @@ struct __align__(16) VsFragRec {
 };
 
 #ifndef VS_SHADE_PREFETCH
-#define VS_SHADE_PREFETCH 2   // 0: off, 1: left column of the footprint, 2: all four texels
+#define VS_SHADE_PREFETCH 2   // 0: off, 1: left column of the footprint, 2: all four texels (screen order only), 3: all four, in surface order too
 #endif
 #ifndef VS_SHADE_PF_DIST
 #define VS_SHADE_PF_DIST 1    // layers between the prefetch of a footprint and its use
@@ -139,7 +139,7 @@ __device__ __forceinline__ void vs_cp_async_wait(int n)
     }
 }
 #define VS_SHADE_SUBTILES (8 / VS_SHADE_WARPS)
-template <int F16, int DEG, bool COUNT>
+template <int F16, int DEG, bool COUNT, bool PF>
 __global__ void __launch_bounds__(VS_SHADE_PIX, VS_SHADE_MIN_CTAS)
 k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams, const int4* __restrict__ vtx,
         const uint32_t* __restrict__ tile_off, const uint32_t* __restrict__ ids, unsigned long long* __restrict__ keys,
@@ -251,7 +251,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             const uint32_t dx = ((xy >> 15) & 1u) * S::NVEC;
             if (VS_SHADE_PFMODE == 0) {
                 vs_prefetch_l2(p0); vs_prefetch_l2(p1);
-                if (VS_SHADE_PREFETCH > 1) { vs_prefetch_l2(p0 + dx); vs_prefetch_l2(p1 + dx); }
+                if (VS_SHADE_PREFETCH != 1) { vs_prefetch_l2(p0 + dx); vs_prefetch_l2(p1 + dx); }
             } else if (VS_SHADE_PFMODE == 1) {
                 const uint32_t bytes = (S::NVEC + dx) * 16u;
                 vs_prefetch_l2_bulk(p0, bytes);
@@ -266,7 +266,11 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             }
         }
     };
-    if (VS_SHADE_PREFETCH)
+    // In surface order most texels are already in L2 (another view's tile has just used them) and the prefetches are pure issue
+    // overhead: C4 step 23.55 ms without against 24.67 ms with them.  In screen order they pay (27.1 against 27.7 ms).
+    // (PF is a template parameter: the prefetch code left in the kernel behind a run-time flag still costs 0.1 ms per launch)
+    constexpr bool pf_on = PF;
+    if (pf_on)
         for (uint32_t ln = 0; ln < VS_SHADE_PF_DIST && ln < sc.k; ++ln) prefetch_layer(ln);
 
     if (!__any_sync(0xFFFFFFFFu, any_hit)) {
@@ -388,7 +392,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
         };
 #pragma unroll
         for (int j = 0; j < DEPTH - 1; ++j) issue(j, j);
-        if (VS_SHADE_PREFETCH && l + VS_SHADE_PF_DIST < sc.k && alive) prefetch_layer(l + VS_SHADE_PF_DIST);
+        if (pf_on && l + VS_SHADE_PF_DIST < sc.k && alive) prefetch_layer(l + VS_SHADE_PF_DIST);
 #pragma unroll
         for (int j = 0; j < 8; ++j) {
             if (j + DEPTH - 1 < 8) issue(j + DEPTH - 1, (j + DEPTH - 1) % DEPTH);
@@ -477,7 +481,8 @@ static cudaError_t launch_sh2(const VsSceneDev& sc, const VsFrame& fr, const VsC
 {
     if (sc.texel_vecs != (uint32_t)VsShadeShape<F16, DEG>::NVEC) return cudaErrorInvalidValue;
     const size_t smem = (size_t)sc.k * VS_SHADE_PIX * (fr.attenuate ? 16 : 12) + VS_SHADE_WARPS * VS_SHADE_WARP_BYTES;
-    auto kern = k_shade<F16, DEG, COUNT>;
+    const bool pf = VS_SHADE_PREFETCH && (VS_SHADE_PREFETCH >= 3 || ch.order == nullptr);
+    auto kern = pf ? k_shade<F16, DEG, COUNT, true> : k_shade<F16, DEG, COUNT, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
 #ifdef VS_SHADE_CARVEOUT
