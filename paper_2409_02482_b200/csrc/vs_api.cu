@@ -294,6 +294,7 @@ static vs_status scene_create_impl(const vs_scene_desc* desc, const vs_scene_des
         d.vtx_off[l] = (uint32_t)vt;
         vt += L.num_vertices; tt += L.num_triangles;
         if (vt >= (1ull << 31) || tt >= (1ull << 31)) return fail(VS_ERR_UNSUPPORTED, "scene too large");
+        if (L.num_triangles >= (1u << 28)) return fail(VS_ERR_UNSUPPORTED, "layer %u: more than 2^28 - 1 triangles", l);
     }
     for (uint32_t l = k; l <= VS_MAX_LAYERS; ++l) { d.tri_off[l] = (uint32_t)tt; d.vtx_off[l] = (uint32_t)vt; }
     uint64_t bits = 0;

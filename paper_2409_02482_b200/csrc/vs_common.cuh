@@ -24,7 +24,7 @@
 struct VsSceneDev {
     const float* positions;   // [v_total][3], all layers concatenated
     const float2* uvs;        // [v_total]
-    const uint4* tris;        // [t_total] {i0, i1, i2 : global vertex index, w : layer}
+    const uint4* tris;        // [t_total] {i0, i1, i2 : global vertex index, w : layer << 28 | index of the triangle in its layer}
     const float4* tri_nrm;    // [t_total] unit geometric normal in world space (fp64 cross product rounded to fp32), w = 0;
                               //           zero vector for zero-area triangles.  Read only under VS_FLAG_ATTENUATION
     const float4* vtx_nrm;    // [v_total] optional per-vertex normals (vs_scene_set_vertex_normals), w = 0; nullptr if none
@@ -65,6 +65,9 @@ struct VsFrame {
 // counters[0] dropped, [1] degenerate, [2] tile refs, [3] shaded fragments, [4] unique texels,
 // [5] max over chunks of the references a chunk needed when that exceeded ref_capacity (0 = no overflow)
 enum { VS_CNT_DROPPED = 0, VS_CNT_DEGENERATE = 1, VS_CNT_REFS = 2, VS_CNT_FRAGS = 3, VS_CNT_TEXELS = 4, VS_CNT_OVERFLOW = 5, VS_CNT_N = 8 };
+
+__host__ __device__ inline uint32_t vs_tri_layer(uint32_t w) { return w >> 28; }
+__host__ __device__ inline uint32_t vs_tri_lid(uint32_t w) { return w & 0x0FFFFFFFu; }
 
 // ---- packed fp32 pairs (sm_100: FADD2 / FMUL2 / FFMA2 issue one instruction for two lanes' worth of fp32 work) ----
 typedef unsigned long long f32x2;

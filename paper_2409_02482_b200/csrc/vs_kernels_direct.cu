@@ -83,9 +83,7 @@ __device__ __forceinline__ void vs_direct_large(int X0, int Y0, int X1, int Y1, 
 #ifndef VS_RD_MIN_CTAS
 #define VS_RD_MIN_CTAS (1024 / VS_RD_THREADS)
 #endif
-#ifndef VS_RD_PIPELINE
-#define VS_RD_PIPELINE 0      // experiment: > 0 = resident grid of that many CTAs per SM slot with next-item prefetch (see the kernel)
-#endif
+template <bool RESIDENT>
 __global__ void __launch_bounds__(VS_RD_THREADS, VS_RD_MIN_CTAS)
 k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, unsigned long long* __restrict__ keys,
                 uint32_t* __restrict__ tile_mask, uint2* __restrict__ big_list, uint32_t* __restrict__ big_count, uint32_t big_capacity,
@@ -97,21 +95,12 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
     const size_t plane_px = (size_t)W * H;
     int4* rec4 = reinterpret_cast<int4*>(slab + warp * VS_RD_WARP_WORDS);                 // [vector][lane]
     unsigned short* queue = reinterpret_cast<unsigned short*>(slab + warp * VS_RD_WARP_WORDS + VS_RD_FIELDS * 32);   // [512]
-    // work item = (view, block of VS_RD_THREADS consecutive triangles).  The grid either has one CTA per item or, when the
-    // kernel runs beside the previous chunk's k_shade, a few resident CTAs per SM that stride over the items
-#if VS_RD_PIPELINE
-    // experiment: a resident grid strides over the items; the index record of a lane's NEXT triangle is loaded one
-    // item ahead and its three vertex records are prefetched into L1 while the current item is being rasterised
-    uint4 tri_next = make_uint4(0, 0, 0, 0);
-    {
-        const uint32_t v0 = blockIdx.x / blocks_per_view, g0 = (blockIdx.x - v0 * blocks_per_view) * (uint32_t)VS_RD_THREADS + tid;
-        if (blockIdx.x < total_blocks && g0 < sc.t_total) tri_next = __ldg(&sc.tris[g0]);
-    }
-#endif
-    for (uint32_t item = blockIdx.x; item < total_blocks; item += gridDim.x) {
-    __syncwarp();   // the previous item's phase 2 has finished reading this warp's slab
-    const uint32_t view = item / blocks_per_view;
-    const uint32_t gt = (item - view * blocks_per_view) * (uint32_t)VS_RD_THREADS + tid;
+    // work item = (view, block of VS_RD_THREADS consecutive triangles).  The grid has one CTA per item (x = block, y = view)
+    // or, RESIDENT (the kernel runs beside the previous chunk's k_shade), a few CTAs per SM that stride over the items
+    for (uint32_t item = RESIDENT ? blockIdx.x : 0u; item < (RESIDENT ? total_blocks : 1u); item += gridDim.x) {
+    if (RESIDENT) __syncwarp();   // the previous item's phase 2 has finished reading this warp's slab
+    const uint32_t view = RESIDENT ? item / blocks_per_view : blockIdx.y;
+    const uint32_t gt = (RESIDENT ? item - view * blocks_per_view : blockIdx.x) * (uint32_t)VS_RD_THREADS + tid;
     const int4* __restrict__ vv = vtx + (size_t)view * sc.v_total;
     unsigned long long* __restrict__ vkeys = keys + (size_t)view * sc.k * plane_px;
 
@@ -120,19 +109,8 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
     int i0 = 0, i1 = -1, j0 = 0, j1 = -1, status = -1;
     uint32_t layer = 0, lid = 0;
     bool narrow = false, valid = false, large = false;
-#if VS_RD_PIPELINE
-    const uint4 tri_cur = tri_next;
-    const uint32_t item2 = item + gridDim.x, view2 = item2 / blocks_per_view;
-    const uint32_t gt2 = (item2 - view2 * blocks_per_view) * (uint32_t)VS_RD_THREADS + tid;
-    const bool next_ok = item2 < total_blocks && gt2 < sc.t_total;
-    if (next_ok) tri_next = __ldg(&sc.tris[gt2]);
-#endif
     if (gt < sc.t_total) {
-#if VS_RD_PIPELINE
-        const uint4 tri = tri_cur;
-#else
         const uint4 tri = __ldg(&sc.tris[gt]);
-#endif
         const int4 a = __ldg(&vv[tri.x]), b = __ldg(&vv[tri.y]), c = __ldg(&vv[tri.z]);
         status = vs_setup_tri(a, b, c, T);
         if (status == 0) {
@@ -140,7 +118,7 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
             const int minY = min(T.Y0, min(T.Y1, T.Y2)), maxY = max(T.Y0, max(T.Y1, T.Y2));
             i0 = max((minX + 127) >> 8, 0); i1 = min((maxX - 128) >> 8, W - 1);
             j0 = max((minY + 127) >> 8, 0); j1 = min((maxY - 128) >> 8, H - 1);
-            layer = tri.w; lid = gt - sc.tri_off[layer];
+            layer = vs_tri_layer(tri.w); lid = vs_tri_lid(tri.w);
             narrow = maxX - minX < 8192 && maxY - minY < 8192;  // every int32 intermediate < 2^28
             valid = i0 <= i1 && j0 <= j1;
             large = valid && !(narrow && i1 - i0 < 8 && j1 - j0 < 8);
@@ -246,14 +224,6 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
         mlo &= colm & (nr >= 4 ? 0xFFFFFFFFu : ((1u << (8 * nr)) - 1u));
         mhi &= colm & (nr >= 8 ? 0xFFFFFFFFu : (nr > 4 ? ((1u << (8 * (nr - 4))) - 1u) : 0u));
     }
-#if VS_RD_PIPELINE
-    if (next_ok) {
-        const int4* __restrict__ vv2 = vtx + (size_t)view2 * sc.v_total;
-        asm volatile("prefetch.global.L1 [%0];" ::"l"(vv2 + tri_next.x));
-        asm volatile("prefetch.global.L1 [%0];" ::"l"(vv2 + tri_next.y));
-        asm volatile("prefetch.global.L1 [%0];" ::"l"(vv2 + tri_next.z));
-    }
-#endif
     // ---------------- compaction: (lane, bit) codes of the covered samples ----------------
     const uint32_t cnt = (uint32_t)(__popc(mlo) + __popc(mhi));
     uint32_t incl = cnt;
@@ -356,8 +326,8 @@ k_raster_big(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx
         const int minX = min(T.X0, min(T.X1, T.X2)), maxX = max(T.X0, max(T.X1, T.X2));
         const int minY = min(T.Y0, min(T.Y1, T.Y2)), maxY = max(T.Y0, max(T.Y1, T.Y2));
         const bool narrow = maxX - minX < 8192 && maxY - minY < 8192;
-        unsigned long long* plane = keys + ((size_t)ent.x * sc.k + tri.w) * plane_px;
-        const uint32_t lid = ent.y - sc.tri_off[tri.w];
+        unsigned long long* plane = keys + ((size_t)ent.x * sc.k + vs_tri_layer(tri.w)) * plane_px;
+        const uint32_t lid = vs_tri_lid(tri.w);
         if (narrow) vs_direct_large<int, false>(T.X0, T.Y0, T.X1, T.Y1, T.X2, T.Y2, T.q0, T.q1, T.q2, __ll2float_rn(T.A2), i0, i1, j0, j1, W, plane, lid, lane, gw, warps);
         else vs_direct_large<long long, false>(T.X0, T.Y0, T.X1, T.Y1, T.X2, T.Y2, T.q0, T.q1, T.q2, __ll2float_rn(T.A2), i0, i1, j0, j1, W, plane, lid, lane, gw, warps);
     }
@@ -372,12 +342,12 @@ cudaError_t vs_launch_raster_direct(const VsSceneDev& sc, const VsFrame& fr, con
     const unsigned long long total = (unsigned long long)bpv * ch.views;
     if (total >= (1ull << 31)) return cudaErrorInvalidValue;
     // resident_ctas != 0: that many CTAs stride over the work items (the kernel shares the SMs with another one)
-    uint32_t grid = resident_ctas && resident_ctas < total ? resident_ctas : (uint32_t)total;
-#if VS_RD_PIPELINE
-    if (!resident_ctas && total > 148u * VS_RD_MIN_CTAS * VS_RD_PIPELINE) grid = 148u * VS_RD_MIN_CTAS * VS_RD_PIPELINE;
-#endif
-    k_raster_direct<<<grid, VS_RD_THREADS, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.tile_mask, ch.big_list, ch.big_count, ch.big_capacity,
-                                                   ch.counters, bpv, (uint32_t)total);
+    if (resident_ctas && resident_ctas < total)
+        k_raster_direct<true><<<resident_ctas, VS_RD_THREADS, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.tile_mask, ch.big_list, ch.big_count,
+                                                                       ch.big_capacity, ch.counters, bpv, (uint32_t)total);
+    else
+        k_raster_direct<false><<<dim3(bpv, ch.views), VS_RD_THREADS, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.tile_mask, ch.big_list,
+                                                                              ch.big_count, ch.big_capacity, ch.counters, bpv, (uint32_t)total);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     k_raster_big<<<resident_ctas ? 148 : 148 * 4, 256, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.big_list, ch.big_count, ch.big_capacity);

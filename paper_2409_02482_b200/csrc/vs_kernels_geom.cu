@@ -12,7 +12,7 @@ __global__ void k_pack_tris(const uint32_t* __restrict__ idx, const float* __res
     if (t >= nt) return;
     uint32_t a = idx[3 * (size_t)t], b = idx[3 * (size_t)t + 1], c = idx[3 * (size_t)t + 2];
     if (a >= nv || b >= nv || c >= nv) { atomicOr(err, 1u); a = b = c = 0; }
-    out[t] = make_uint4(a + voff, b + voff, c + voff, layer);
+    out[t] = make_uint4(a + voff, b + voff, c + voff, (layer << 28) | t);
     // unit geometric normal (for the transparency attenuation): fp64 cross product of the fp32 positions, once per scene
     const double ax = (double)pos[3 * (size_t)b] - (double)pos[3 * (size_t)a], ay = (double)pos[3 * (size_t)b + 1] - (double)pos[3 * (size_t)a + 1],
                  az = (double)pos[3 * (size_t)b + 2] - (double)pos[3 * (size_t)a + 2];

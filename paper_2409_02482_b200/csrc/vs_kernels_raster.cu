@@ -125,7 +125,7 @@ k_raster(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, co
                 const int minY = min(T.Y0, min(T.Y1, T.Y2)), maxY = max(T.Y0, max(T.Y1, T.Y2));
                 i0 = max((minX + 127) >> 8, px0); i1 = min((maxX - 128) >> 8, tx1);
                 j0 = max((minY + 127) >> 8, py0); j1 = min((maxY - 128) >> 8, ty1);
-                layer = tri.w; lid = gt - sc.tri_off[layer];
+                layer = vs_tri_layer(tri.w); lid = vs_tri_lid(tri.w);
                 narrow = maxX - minX < 8192 && maxY - minY < 8192;  // every int32 intermediate < 2^28
                 valid = i0 <= i1 && j0 <= j1;
                 large = valid && !(narrow && i1 - i0 < 8 && j1 - j0 < 8);
