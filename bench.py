@@ -36,7 +36,7 @@ UNIT = "MP/s"
 # and the SHA-256 of the kernel sources the capture was taken from.  `roofline.traffic` is reported only while those
 # sources are unchanged (else null: a capture of other code is not evidence about this run).
 TRAFFIC_FILE = os.path.join(os.path.dirname(os.path.abspath(__file__)), "profiles", "ncu_traffic.json")
-TRAFFIC_SOURCES = ("vs_kernels_shade.cu", "vs_common.cuh")
+TRAFFIC_SOURCES = ("vs_kernels_shade.cu", "vs_kernels_order.cu", "vs_common.cuh")
 
 
 def kernel_source_hashes():
@@ -45,8 +45,9 @@ def kernel_source_hashes():
     return {f: hashlib.sha256(open(os.path.join(d, f), "rb").read()).hexdigest() for f in TRAFFIC_SOURCES}
 
 
-def ncu_traffic_bytes_per_view(config_key):
-    """(bytes per view, provenance) of the committed capture of this configuration, or (None, why not)."""
+def ncu_traffic_bytes_per_view(config_key, views_per_launch=None):
+    """(bytes per view, provenance) of the committed capture of this configuration, or (None, why not).  In surface order the
+    views of a launch share texels through L2, so a capture only speaks for launches of the same number of views."""
     try:
         table = json.load(open(TRAFFIC_FILE))
     except Exception:
@@ -56,6 +57,9 @@ def ncu_traffic_bytes_per_view(config_key):
         return None, "no committed ncu capture of this configuration"
     if ent.get("source_sha256") != kernel_source_hashes():
         return None, "kernel sources changed since the capture of commit %s" % ent.get("commit")
+    if views_per_launch is not None and ent.get("views_per_launch") not in (None, int(round(views_per_launch))):
+        return None, "the committed capture is of a %s-view launch, this run launched %g views at a time" % (
+            ent.get("views_per_launch"), views_per_launch)
     return float(ent["dram_bytes_per_view"]), "ncu --set full capture of commit %s (%s)" % (ent.get("commit"), ent.get("summary"))
 
 
@@ -296,7 +300,7 @@ def run_ours(args):
     views_per_launch = B * args.steps / max(shade_launches, 1)
     traffic_key = "%d%s%s" % (args.config, "-" + args.camera_subset if args.camera_subset else "", "-backward" if args.backward else "")
     plain = not (args.tiled or args.attenuation or args.overlap or args.screen_order or args.views or banded or args.lib)
-    traffic_per_view, traffic_src = ncu_traffic_bytes_per_view(traffic_key) if plain else (None, "not the captured launch configuration")
+    traffic_per_view, traffic_src = ncu_traffic_bytes_per_view(traffic_key, views_per_launch) if plain else (None, "not the captured launch configuration")
     # the three candidate bounds of SURVEY.md §8(d), per view: HBM (algorithmic bytes), L1 gather (4 texels per fragment through
     # the 128 B/clk/SM data pipe), FP32 issue (algorithmic lane-ops: 4 x 4n bilinear + SH FMAs, 4 x 4n half->float conversions
     # for fp16 texels, ~40 for sigmoids and blend; 128 lanes per SM) -- the largest one binds
@@ -404,19 +408,19 @@ def main():
                     help="every other camera of the set: on C5 the r=3 orbit cameras resp. the r=1.6 close-ups (SURVEY.md §8(d))")
     ap.add_argument("--strong", action="store_true", help="multi-GPU: split ONE camera batch evenly over the ranks (strong scaling) instead of one batch per rank")
     ap.add_argument("--lib", default=None, help="load this build of the library (an experiment variant made by `python -m paper_2409_02482_b200.build --lib PATH -D...`)")
-    ap.add_argument("--record-traffic", nargs=4, metavar=("KEY", "DRAM_BYTES_PER_VIEW", "COMMIT", "SUMMARY"), default=None,
+    ap.add_argument("--record-traffic", nargs=5, metavar=("KEY", "DRAM_BYTES_PER_VIEW", "VIEWS_PER_LAUNCH", "COMMIT", "SUMMARY"), default=None,
                     help="no benchmark: store the dram__bytes_read+write per view of an `ncu --set full` capture of configuration KEY "
                          "(e.g. 4, 5-close) in profiles/ncu_traffic.json together with the hashes of the kernel sources as they are now")
     ap.add_argument("--cpu-1thread-seconds", type=float, default=30.0, help="budget of the 1-thread oracle sample (one whole view); skipped if a view would take longer")
     args = ap.parse_args()
     if args.record_traffic:
-        key, nbytes, commit, summary = args.record_traffic
+        key, nbytes, vpl, commit, summary = args.record_traffic
         try:
             table = json.load(open(TRAFFIC_FILE))
         except Exception:
             table = {}
-        table[key] = {"kernel": "k_shade", "dram_bytes_per_view": float(nbytes), "commit": commit, "summary": summary,
-                      "source_sha256": kernel_source_hashes()}
+        table[key] = {"kernel": "k_shade", "dram_bytes_per_view": float(nbytes), "views_per_launch": int(vpl), "commit": commit,
+                      "summary": summary, "source_sha256": kernel_source_hashes()}
         json.dump(table, open(TRAFFIC_FILE, "w"), indent=1, sort_keys=True)
         print("recorded", key, "in", TRAFFIC_FILE)
         return 0
