@@ -282,6 +282,32 @@ vs_status vs_render_backward(vs_scene* scene, const vs_camera* cameras, uint32_t
 /* Waits for the most recent render call on this scene and returns its counters (see vs_render_stats). */
 vs_status vs_query_last_render(vs_scene* scene, vs_render_stats* out_stats);
 
+/*
+ * vs_render_static -- vs_render for callers that must not allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same steps S1-S7 on the default (direct) path, with EVERYTHING the call writes
+ * besides the caller's outputs -- staged cameras, transformed vertices, key image, tile masks, the surface-order list and its
+ * sort work space -- placed in one file-scope `static __device__` array of VS_STATIC_SCRATCH_BYTES inside the library
+ * (csrc/vs_noalloc.cu).  The call makes no cudaMalloc / cudaFree / pool allocation of any kind; its outputs are bit-identical
+ * to vs_render's.
+ *
+ *   Arguments, layouts and asynchrony as vs_render (cameras HOST, outputs DEVICE, work enqueued on `cuda_stream`).
+ *   flags: only VS_FLAG_ATTENUATION and VS_FLAG_SCREEN_ORDER (else VS_ERR_UNSUPPORTED); views_per_chunk is ignored: the call
+ *   is ONE pass.  No statistics: vs_query_last_render does not see these calls.
+ *   LIMIT: the call needs about  num_cameras * (num_layers * width * height * 8 + total_vertices * 16 + tiles * 16 + 64) +
+ *   0.6 MB  bytes of scratch (tiles = ceil(width / 16) * ceil(height / 16)); if that exceeds VS_STATIC_SCRATCH_BYTES the call
+ *   fails with VS_ERR_UNSUPPORTED and a message that states both numbers -- render fewer cameras per call, or use vs_render.
+ *   (k = 9 layers and 100 000 vertices: one 1024 x 768 view needs 58.8 MB, four 480 x 360 views 56.8 MB, of the 67.1 MB.)
+ *   The array exists once per GPU that loads the library (64 MiB of device memory held until the process exits) and is
+ *   SHARED by every call, every scene and every stream: what has to start at zero (key image, tile masks, counters) is
+ *   cleared by each call on its stream, so stale contents never matter, but two calls whose device work OVERLAPS (different
+ *   streams, or several host threads without ordering between their streams) RACE on it.  Order them on one stream or with
+ *   events.  Host-side the call is serialised by a library-wide mutex.
+ */
+#define VS_STATIC_SCRATCH_BYTES (64u << 20)
+vs_status vs_render_static(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
+                           const vs_render_params* params, float* out_rgba, uint32_t* out_tri_ids,
+                           void* cuda_stream);
+
 /* Frees all device memory of the scene after synchronising the device.  NULL is a no-op. */
 void vs_scene_destroy(vs_scene* scene);
 

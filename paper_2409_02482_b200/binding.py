@@ -21,9 +21,10 @@ VS_FLAG_REFERENCE_PATH, VS_FLAG_KERNEL_TIMING, VS_FLAG_COUNT_TEXELS, VS_FLAG_TIL
 VS_FLAG_ATTENUATION = 16
 VS_FLAG_OVERLAP = 32
 VS_FLAG_SCREEN_ORDER = 64
+VS_STATIC_SCRATCH_BYTES = 64 << 20   # vs_render_static: size of the library's static device scratch
 MISS = 0xFFFFFFFF
 
-EXPORTS = ["vs_scene_create", "vs_scene_create_banded", "vs_scene_set_vertex_normals", "vs_render", "vs_render_aov", "vs_render_backward", "vs_render_host", "vs_query_last_render", "vs_scene_destroy",
+EXPORTS = ["vs_scene_create", "vs_scene_create_banded", "vs_scene_set_vertex_normals", "vs_render", "vs_render_aov", "vs_render_backward", "vs_render_host", "vs_render_static", "vs_query_last_render", "vs_scene_destroy",
            "vs_last_error", "vs_version"]
 
 
@@ -109,7 +110,7 @@ def load_library(build_if_missing: bool = True):
     L.vs_scene_create.argtypes = [C.POINTER(vs_scene_desc), C.c_void_p, C.POINTER(C.c_void_p)]
     L.vs_scene_create_banded.restype = C.c_int
     L.vs_scene_create_banded.argtypes = [C.POINTER(vs_scene_desc_banded), C.c_void_p, C.POINTER(C.c_void_p)]
-    for name in ("vs_render", "vs_render_host"):
+    for name in ("vs_render", "vs_render_host", "vs_render_static"):
         f = getattr(L, name)
         f.restype = C.c_int
         f.argtypes = [C.c_void_p, C.c_void_p, C.c_uint32, C.POINTER(vs_render_params), C.c_void_p,
@@ -280,6 +281,22 @@ def vs_render(scene: int, cameras, params: vs_render_params, out_rgba, out_tri_i
         ids_ptr = out_tri_ids.data_ptr()
     _check(load_library().vs_render(scene, cams.ctypes.data, cams.shape[0], C.byref(params),
                                     out_rgba.data_ptr(), ids_ptr, _stream_ptr(stream)))
+
+
+def vs_render_static(scene: int, cameras, params: vs_render_params, out_rgba, out_tri_ids=None, stream=None):
+    """vs_render without any allocation: all scratch in the library's static 64 MiB device array (include/vs.h).  Same
+    arguments as vs_render; raises VsError(VS_ERR_UNSUPPORTED) when the call does not fit.  Calls that overlap on the GPU race."""
+    import torch
+    cams = _cams(cameras)
+    k = _scene_info(scene)[0]
+    px = cams.shape[0] * params.width * params.height
+    assert out_rgba.is_cuda and out_rgba.is_contiguous() and out_rgba.dtype == torch.float32 and out_rgba.numel() == px * 4
+    ids_ptr = None
+    if out_tri_ids is not None:
+        assert out_tri_ids.is_cuda and out_tri_ids.is_contiguous() and out_tri_ids.element_size() == 4 and out_tri_ids.numel() == px * k
+        ids_ptr = out_tri_ids.data_ptr()
+    _check(load_library().vs_render_static(scene, cams.ctypes.data, cams.shape[0], C.byref(params),
+                                           out_rgba.data_ptr(), ids_ptr, _stream_ptr(stream)))
 
 
 def vs_render_aov(scene: int, cameras, params: vs_render_params, out_rgba, tri_ids=None, layer_rgba=None, layer_uv=None,

@@ -21,6 +21,7 @@
 
 #include "../../include/vs.h"
 #include "vs_common.cuh"
+#include "vs_internal.cuh"
 
 static thread_local char g_err[512] = "";
 
@@ -1091,3 +1092,18 @@ extern "C" vs_status vs_query_last_render(vs_scene* scene, vs_render_stats* out)
     scene->launches = scene->raster_launches = scene->shade_launches = 0;
     return VS_OK;
 }
+
+// ---- hooks for vs_noalloc.cu (vs_render_static); declared in vs_internal.cuh ----
+vs_status vs_internal_validate_render(const vs_scene* scene, const vs_camera* cams, uint32_t n, const vs_render_params* p,
+                                      const void* out_rgba)
+{
+    g_err[0] = 0;
+    return validate_render(scene, cams, n, p, out_rgba);
+}
+
+void vs_internal_scene_view(const vs_scene* scene, const VsSceneDev** dev, int* tex_f16, int* device)
+{
+    *dev = &scene->dev; *tex_f16 = scene->tex_f16; *device = scene->device;
+}
+
+vs_status vs_internal_fail(vs_status s, const char* message) { return fail(s, "%s", message); }
