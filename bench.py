@@ -325,6 +325,15 @@ def run_ours(args):
                 "stage_ms_per_step": {"transform": xf_ms / args.steps, "binning": bin_ms / args.steps,
                                       "raster": raster_ms / args.steps, "shade": shade_ms / args.steps}}
 
+    if roofline["traffic"]:
+        # < 1 in surface order: the views of a launch share texels through L2, while the algorithmic bytes
+        # charge every view its unique texels once.  `frac` then measures speed against a view-by-view renderer running at the
+        # HBM peak, not DRAM utilisation
+        roofline["traffic_over_algorithmic"] = roofline["traffic"] / bytes_per_launch
+        if roofline["traffic_over_algorithmic"] < 1.0:
+            roofline["note"] = ("DRAM traffic is below the per-view algorithmic bytes: the views of a launch share texels through L2 "
+                                "(surface-ordered shading); frac is against a view-by-view renderer at the HBM peak, the kernel "
+                                "itself is bound by SM-side work (L1 data pipe), see DESIGN.md 7-8")
     if banded:
         # The banded 8-bit path is bound by the plain FP32/ALU pipes: algorithmic lane-ops per shaded
         # fragment at degree d = 4 texels x 4(d+1)^2 byte->float conversions + as many bilinear FMAs + 4(d+1)^2 SH FMAs
