@@ -210,7 +210,8 @@ def run_ours(args):
     B, W, H = len(sc.cameras), sc.width, sc.height
     renderer = binding.Renderer(sc, dev)
     path_flag = ((binding.VS_FLAG_TILED_PATH if args.tiled else 0) | (binding.VS_FLAG_ATTENUATION if args.attenuation else 0) |
-                 (binding.VS_FLAG_OVERLAP if args.overlap else 0) | (binding.VS_FLAG_SCREEN_ORDER if args.screen_order else 0))
+                 (binding.VS_FLAG_OVERLAP if args.overlap else 0) | (binding.VS_FLAG_SCREEN_ORDER if args.screen_order else 0) |
+                 (binding.VS_FLAG_PLAIN_BACKWARD if args.plain_backward else 0))
     flags = binding.VS_FLAG_KERNEL_TIMING | path_flag
     params = binding.make_params(W, H, sc.near_plane, sc.t_min, sc.background, flags, args.chunk)
     out = torch.empty((B, H, W, 4), dtype=torch.float32, device=dev)
@@ -228,7 +229,7 @@ def run_ours(args):
     alg_bytes_step = b_tex + b_geom + b_fb
 
     if args.backward:
-        # step = one vs_render_backward call (S1-S4 + k_backward) over the batch; the fp32 gradient textures are
+        # step = one vs_render_backward call (S1-S4 + k_shade<BWD>, or k_backward with --plain-backward) over the batch; the fp32 gradient textures are
         # accumulated into across steps (zeroed once, outside the timed region)
         gen = torch.Generator(device=dev).manual_seed(1234)
         gout = torch.randn((B, H, W, 4), dtype=torch.float32, device=dev, generator=gen)
@@ -299,7 +300,7 @@ def run_ours(args):
     step_achieved = alg_bytes_step * world / (secs_max / args.steps) / 1e9
     views_per_launch = B * args.steps / max(shade_launches, 1)
     traffic_key = "%d%s%s" % (args.config, "-" + args.camera_subset if args.camera_subset else "", "-backward" if args.backward else "")
-    plain = not (args.tiled or args.attenuation or args.overlap or args.screen_order or args.views or banded or args.lib)
+    plain = not (args.tiled or args.attenuation or args.overlap or args.screen_order or args.views or banded or args.lib or args.plain_backward)
     traffic_per_view, traffic_src = ncu_traffic_bytes_per_view(traffic_key, views_per_launch) if plain else (None, "not the captured launch configuration")
     # the three candidate bounds of SURVEY.md §8(d), per view: HBM (algorithmic bytes), L1 gather (4 texels per fragment through
     # the 128 B/clk/SM data pipe), FP32 issue (algorithmic lane-ops: 4 x 4n bilinear + SH FMAs, 4 x 4n half->float conversions
@@ -313,7 +314,7 @@ def run_ours(args):
     cand = {"hbm": t_hbm, "l1_gather": t_l1, "fp32_issue": t_fp32}
     bounds = {"ms_per_view": cand, "binding": max(cand, key=cand.get), "measured_ms_per_view": 1e3 * secs_max / args.steps / B,
               "lane_ops_per_fragment": lane_ops, "note": "148 SMs x 128 B/clk resp. 128 lanes at 1965 MHz; HBM at the measured copy peak"}
-    roofline = {"bound": "hbm", "kernel": "k_backward" if args.backward else "k_shade", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    roofline = {"bound": "hbm", "kernel": ("k_backward" if args.plain_backward else "k_shade<BWD>") if args.backward else "k_shade", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": traffic_per_view * views_per_launch if traffic_per_view else None,
                 "traffic_source": traffic_src, "bounds": bounds,
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": bytes_per_launch,
@@ -411,6 +412,7 @@ def main():
     ap.add_argument("--banded", action="store_true", help="the paper's 8-bit mixed-resolution textures on the same geometry (PAPER.md:L445-459; not the headline workload)")
     ap.add_argument("--attenuation", action="store_true", help="render with VS_FLAG_ATTENUATION (PAPER.md:L279-286; not the headline workload)")
     ap.add_argument("--tiled", action="store_true", help="time the per-tile raster path (VS_FLAG_TILED_PATH) instead of the default direct one")
+    ap.add_argument("--plain-backward", action="store_true", help="with --backward: VS_FLAG_PLAIN_BACKWARD, the plain per-lane k_backward instead of k_shade<BWD> (A/B)")
     ap.add_argument("--screen-order", action="store_true", help="VS_FLAG_SCREEN_ORDER: shade view by view instead of in surface order (A/B, DESIGN.md §7)")
     ap.add_argument("--overlap", action="store_true", help="VS_FLAG_OVERLAP: S1-S4 of the next chunk beside S5-S7 of the current one (experiment, DESIGN.md §7)")
     ap.add_argument("--camera-subset", choices=["far", "close"], default=None,

@@ -101,6 +101,10 @@ enum {
                                          default SURFACE order, in which the tiles of all views of a pass that look at the
                                          same part of the object are shaded together so that their texels are shared
                                          through L2; same outputs bit for bit; for A/B measurements        */
+    VS_FLAG_PLAIN_BACKWARD = 1u << 7, /* vs_render_backward only: the first backward kernel (k_backward: one lane per pixel
+                                         re-shades its fragments with the plain per-lane routine) instead of the default
+                                         k_shade<BWD>, which shares k_shade's octet / tensor-core forward pass; same
+                                         gradients up to the fp32 summation order; for A/B measurements and cross-checks  */
     VS_FLAG_ATTENUATION    = 1u << 4  /* transparency attenuation (§4.2 "Transparency
                                          Attenuation"): every fragment's opacity is multiplied by
                                          alpha_w = 2 Sigmoid(10 |v . n|) - 1 before blending, v = the pixel's
@@ -272,8 +276,9 @@ vs_status vs_render_aov(vs_scene* scene, const vs_camera* cameras, uint32_t num_
  *   grad_textures  HOST array of num_layers DEVICE pointers, layer l: [tex_h][tex_w][(deg+1)^2][4] float (the API layout
  *                  of vs_layer_desc.texture, always fp32); the caller zeroes them; sums are fp32 atomics in no fixed order
  *   Float-texture scenes only (VS_ERR_UNSUPPORTED on banded scenes and with VS_FLAG_REFERENCE_PATH / TILED / COUNT).
- *   Runs S1-S4 again (nothing of the forward call is kept) and k_backward in place of k_shade; asynchronous on
- *   `cuda_stream` like vs_render.
+ *   Runs S1-S4 again (nothing of the forward call is kept) and k_shade<BWD> in place of k_shade (forward pass of the tile,
+ *   then the recurrence and the scatter; VS_FLAG_PLAIN_BACKWARD: the plain k_backward); asynchronous on `cuda_stream` like
+ *   vs_render.
  */
 vs_status vs_render_backward(vs_scene* scene, const vs_camera* cameras, uint32_t num_cameras,
                              const vs_render_params* params, const float* grad_rgba, float* const* grad_textures,

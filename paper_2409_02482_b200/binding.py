@@ -21,6 +21,7 @@ VS_FLAG_REFERENCE_PATH, VS_FLAG_KERNEL_TIMING, VS_FLAG_COUNT_TEXELS, VS_FLAG_TIL
 VS_FLAG_ATTENUATION = 16
 VS_FLAG_OVERLAP = 32
 VS_FLAG_SCREEN_ORDER = 64
+VS_FLAG_PLAIN_BACKWARD = 128
 VS_STATIC_SCRATCH_BYTES = 64 << 20   # vs_render_static: size of the library's static device scratch
 MISS = 0xFFFFFFFF
 

@@ -514,7 +514,7 @@ static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, u
     if (!(p->near_plane > 0.0f) || !std::isfinite(p->near_plane)) return fail(VS_ERR_INVALID_ARG, "near_plane must be > 0");
     if (!(p->t_min >= 0.0f) || !std::isfinite(p->t_min)) return fail(VS_ERR_INVALID_ARG, "t_min must be >= 0");
     if (p->flags & ~(uint32_t)(VS_FLAG_REFERENCE_PATH | VS_FLAG_KERNEL_TIMING | VS_FLAG_COUNT_TEXELS | VS_FLAG_TILED_PATH |
-                               VS_FLAG_ATTENUATION | VS_FLAG_OVERLAP | VS_FLAG_SCREEN_ORDER))
+                               VS_FLAG_ATTENUATION | VS_FLAG_OVERLAP | VS_FLAG_SCREEN_ORDER | VS_FLAG_PLAIN_BACKWARD))
         return fail(VS_ERR_INVALID_ARG, "reserved flag bits set");
     for (int i = 0; i < 3; ++i)
         if (!std::isfinite(p->background[i])) return fail(VS_ERR_INVALID_ARG, "background not finite");
@@ -804,7 +804,9 @@ static vs_status enqueue_consumer(Call& c, ScratchSet& ss, uint32_t views, float
         s->launches += 1;
     } else {
         if ((r = span_begin(s, c.timing, 3, c.st)) != VS_OK) return r;
-        if (c.mode == MODE_BACKWARD) CU(vs_launch_backward(s->dev, s->tex_f16, fr, ch, c.st));
+        if (c.mode == MODE_BACKWARD)
+            CU((c.p->flags & VS_FLAG_PLAIN_BACKWARD) ? vs_launch_backward(s->dev, s->tex_f16, fr, ch, c.st)
+                                                     : vs_launch_shade_backward(s->dev, s->tex_f16, fr, ch, c.st));
         else CU(s->dev.banded ? vs_launch_shade_banded(s->dev, fr, ch, c.st) : vs_launch_shade(s->dev, s->tex_f16, fr, ch, c.st));
         if ((r = span_end(s, c.timing, c.st)) != VS_OK) return r;
         if (!c.tiled) ss.keys_dirty = false;   // the consumer clears what it reads

@@ -188,6 +188,28 @@ __device__ __forceinline__ unsigned long long vs_make_key(float qp, uint32_t loc
     return ((unsigned long long)__float_as_uint(qp) << 32) | (unsigned long long)(0xFFFFFFFFu - local_tri);
 }
 
+// The last stage's read-and-clear of the key image (k_shade, k_backward).  VS_KEYS_STREAM: 1 = evict-first cache hints on both
+// (a key line is touched once per pass and only competes with the texels for L2), 0 = plain accesses.
+#ifndef VS_KEYS_STREAM
+#define VS_KEYS_STREAM 0
+#endif
+__device__ __forceinline__ unsigned long long vs_key_load(const unsigned long long* p)
+{
+#if VS_KEYS_STREAM
+    return __ldcs(p);
+#else
+    return *p;
+#endif
+}
+__device__ __forceinline__ void vs_key_clear(unsigned long long* p)
+{
+#if VS_KEYS_STREAM
+    __stcs(p, 0ull);
+#else
+    *p = 0ull;
+#endif
+}
+
 // Real SH basis, fp32, tolerance domain.
 template <int DEG>
 __device__ __forceinline__ void vs_sh_basis(float x, float y, float z, float* Y)
@@ -390,6 +412,7 @@ cudaError_t vs_launch_pack_tris(const uint32_t* indices, const float* layer_posi
 cudaError_t vs_launch_pack_band(const unsigned char* src, uint32_t n_texels, uint32_t band, unsigned char* dst, cudaStream_t st);
 cudaError_t vs_launch_shade_banded(const VsSceneDev& sc, const VsFrame& fr, const struct VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_backward(const VsSceneDev& sc, int f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
+cudaError_t vs_launch_shade_backward(const VsSceneDev& sc, int f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st);
 cudaError_t vs_launch_layer_aov(const VsSceneDev& sc, int f16, const VsFrame& fr, uint32_t views, const VsCamDev* cams, const int4* vtx,
                                 const uint32_t* ids, float* layer_rgba, float* layer_uv, float* layer_normal, cudaStream_t st);
 cudaError_t vs_launch_check_finite(const float* v, size_t n, uint32_t* error_flag, cudaStream_t st);

@@ -16,6 +16,9 @@
 
 __device__ __forceinline__ void vs_red_add4(float* p, float a, float b, float c, float d)
 {
+#ifdef VS_BW_EXP_NORED     // timing experiment only (wrong gradients): everything but the reductions
+    if (a != 12345.678f) return;
+#endif
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
 
@@ -56,9 +59,9 @@ k_backward(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ c
     for (uint32_t l = 0; l < sc.k; ++l) {
         ids[l] = VS_MISS;
         if (!inimg || !((lmask >> l) & 1u)) continue;
-        const unsigned long long key = keys[pix0 + (size_t)l * plane];
+        const unsigned long long key = vs_key_load(&keys[pix0 + (size_t)l * plane]);
         if (!key) continue;
-        keys[pix0 + (size_t)l * plane] = 0ull;   // cleared for the next pass over this buffer, as k_shade does
+        vs_key_clear(&keys[pix0 + (size_t)l * plane]);   // cleared for the next pass over this buffer, as k_shade does
         if (!alive) continue;
         const uint32_t lid = 0xFFFFFFFFu - (uint32_t)key;
         float s[4], uv[2];
@@ -123,7 +126,10 @@ k_backward(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ c
             const uint32_t p = oct * 8 + j;       // owner lane of the fragment (pixel row oct, column j)
             const float4 w = rec_w[p];
             if (w.x == 0.0f && w.y == 0.0f && w.z == 0.0f && w.w == 0.0f) continue;
-            const uint4 o = rec_o[p];
+            uint4 o = rec_o[p];
+#ifdef VS_BW_EXP_REDMASK   // timing experiment only (wrong gradients): the reductions stay inside a cache-resident window of float4s
+            o.x &= (uint32_t)VS_BW_EXP_REDMASK; o.y &= (uint32_t)VS_BW_EXP_REDMASK; o.z &= (uint32_t)VS_BW_EXP_REDMASK; o.w &= (uint32_t)VS_BW_EXP_REDMASK;
+#endif
             const float4 d = rec_d[p];
 #pragma unroll
             for (int h = 0; h < 2; ++h) {

@@ -139,12 +139,27 @@ __device__ __forceinline__ void vs_cp_async_wait(int n)
     }
 }
 #define VS_SHADE_SUBTILES (8 / VS_SHADE_WARPS)
-template <int F16, int DEG, bool COUNT, bool PF>
-__global__ void __launch_bounds__(VS_SHADE_PIX, VS_SHADE_MIN_CTAS)
+// BWD (vs_render_backward): the same forward pass, but instead of writing the image every owner keeps
+// (rgb, sigma, T) of the layers it composited in shared memory, then walks them back to front with the recurrence
+//   R_end = bg . g_rgb - g_a ;  dL/dA_l = T_l (rgb_l . g_rgb - R_l) ;  R_{l-1} = A_l (rgb_l . g_rgb) + (1 - A_l) R_l
+// and the octets scatter w_q Y_c dL/ds_ch into the fp32 gradient textures ([texel][c][ch], the API layout): lane i of an
+// octet adds the coefficients c = i and c = 8 + i (a float4 of the 4 channels each) of the four texels of its fragment with
+// red.global.add.v4.f32, so that every reduction instruction covers whole 128-byte lines.
+__device__ __forceinline__ void vs_red_add4(float4* p, float a, float b, float c, float d)
+{
+#ifdef VS_BW_EXP_NORED     // timing experiment only (wrong gradients): everything but the reductions
+    if (a != 12345.678f) return;
+#endif
+    asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+
+template <int F16, int DEG, bool COUNT, bool PF, bool BWD>
+__global__ void __launch_bounds__(VS_SHADE_PIX, BWD ? 4 : VS_SHADE_MIN_CTAS)
 k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams, const int4* __restrict__ vtx,
         const uint32_t* __restrict__ tile_off, const uint32_t* __restrict__ ids, unsigned long long* __restrict__ keys,
         uint32_t* __restrict__ out_ids, float* __restrict__ out_rgba,
-        uint32_t* __restrict__ texel_bits, unsigned long long* __restrict__ counters, const uint32_t* __restrict__ order)
+        uint32_t* __restrict__ texel_bits, unsigned long long* __restrict__ counters, const uint32_t* __restrict__ order,
+        const float* __restrict__ grad_out, const __grid_constant__ VsGradTex gt)
 {
     typedef VsShadeShape<F16, DEG> S;
     constexpr int SLOTS = S::SLOTS, LPC = S::LPC, NACT = S::NACT, NE = S::NE, PPV = S::PPV;
@@ -154,7 +169,9 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     uint32_t* rec_xy = reinterpret_cast<uint32_t*>(smem);
     float2* rec_ab = reinterpret_cast<float2*>(smem + (size_t)sc.k * VS_SHADE_PIX * 4);
     unsigned char* per_warp = smem + (size_t)sc.k * VS_SHADE_PIX * 12;  // per warp: 2 KB basis + 1 KB records + 512 B logits
-    float* rec_aw = reinterpret_cast<float*>(per_warp + VS_SHADE_WARPS * VS_SHADE_WARP_BYTES);   // [k][pixels] attenuation weights (only if fr.attenuate)
+    float* rec_aw = reinterpret_cast<float*>(per_warp + VS_SHADE_WARPS * VS_SHADE_WARP_BYTES);   // [k][pixels] attenuation weights (only if fr.attenuate; always reserved under BWD)
+    float4* act = reinterpret_cast<float4*>(rec_aw + (size_t)sc.k * VS_SHADE_PIX);                // BWD: [k][pixels] {sigmoid rgb, sigmoid of the opacity logit}
+    float* trans = reinterpret_cast<float*>(act + (size_t)sc.k * VS_SHADE_PIX);                   // BWD: [k][pixels] transmittance in front of the layer
 
     const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const uint32_t tiles = fr.tiles_x * fr.tiles_y;
@@ -174,6 +191,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     // tiled path: tile_off = reference list offsets; direct path: tile_off = per-tile masks of the layers drawn into
     const uint32_t lmask = keys ? tile_off[view * tiles + tile] : 0xFFFFFFFFu;
     if (keys ? lmask == 0u : tile_off[view * tiles + tile] == tile_off[view * tiles + tile + 1]) {  // nothing drawn here: background
+        if (BWD) return;   // no fragment, no gradient
         if (out_ids && inimg)
             for (uint32_t l = 0; l < sc.k; ++l) out_ids[((size_t)view * sc.k + l) * ((size_t)W * H) + (size_t)py * W + px] = VS_MISS;
         if (inimg) reinterpret_cast<float4*>(out_rgba)[pix] = make_float4(fr.bg[0], fr.bg[1], fr.bg[2], 0.0f);
@@ -196,11 +214,11 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             unsigned long long key[VS_MAX_LAYERS];
 #pragma unroll
             for (int u = 0; u < VS_MAX_LAYERS; ++u)
-                key[u] = (inimg && u < (int)sc.k && ((lmask >> u) & 1u)) ? keys[pix0 + (size_t)u * plane] : 0ull;
+                key[u] = (inimg && u < (int)sc.k && ((lmask >> u) & 1u)) ? vs_key_load(&keys[pix0 + (size_t)u * plane]) : 0ull;
 #pragma unroll
             for (int u = 0; u < VS_MAX_LAYERS; ++u) {
                 id[u] = key[u] ? 0xFFFFFFFFu - (uint32_t)key[u] : VS_MISS;
-                if (key[u]) keys[pix0 + (size_t)u * plane] = 0ull;
+                if (key[u]) vs_key_clear(&keys[pix0 + (size_t)u * plane]);
                 if (out_ids && inimg && u < (int)sc.k) out_ids[pix0 + (size_t)u * plane] = id[u];
             }
         } else {
@@ -274,7 +292,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
         for (uint32_t ln = 0; ln < VS_SHADE_PF_DIST && ln < sc.k; ++ln) prefetch_layer(ln);
 
     if (!__any_sync(0xFFFFFFFFu, any_hit)) {
-        if (inimg) reinterpret_cast<float4*>(out_rgba)[pix] = make_float4(fr.bg[0], fr.bg[1], fr.bg[2], 0.0f);
+        if (!BWD && inimg) reinterpret_cast<float4*>(out_rgba)[pix] = make_float4(fr.bg[0], fr.bg[1], fr.bg[2], 0.0f);
         return;
     }
 
@@ -330,6 +348,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
 
     float Tr = 1.0f, Cr = 0.0f, Cg = 0.0f, Cb = 0.0f;
     bool alive = true;
+    uint32_t used = 0;   // BWD: layers this pixel composited (bit l)
     for (uint32_t l = 0; l < sc.k; ++l) {
         const float2 ab = rec_ab[l * VS_SHADE_PIX + tid];
         const bool shade = ab.x >= 0.0f && alive;
@@ -465,15 +484,102 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             float4 s4 = part[own_slot];
             if (S::MMA) { const float t = s4.y; s4.y = s4.z; s4.z = t; }   // stored as {ch0, ch2, ch1, ch3}
             float A = vs_sigmoid(s4.w);
+            if (BWD) {
+                act[l * VS_SHADE_PIX + tid] = make_float4(vs_sigmoid(s4.x), vs_sigmoid(s4.y), vs_sigmoid(s4.z), A);
+                trans[l * VS_SHADE_PIX + tid] = Tr;
+                used |= 1u << l;
+            }
             if (fr.attenuate) A *= rec_aw[l * VS_SHADE_PIX + tid];
             const float TA = Tr * A;
-            Cr += TA * vs_sigmoid(s4.x); Cg += TA * vs_sigmoid(s4.y); Cb += TA * vs_sigmoid(s4.z);
+            if (!BWD) { Cr += TA * vs_sigmoid(s4.x); Cg += TA * vs_sigmoid(s4.y); Cb += TA * vs_sigmoid(s4.z); }
             Tr *= (1.0f - A);
             if (Tr < fr.t_min) alive = false;
         }
     }
-    if (inimg)
-        reinterpret_cast<float4*>(out_rgba)[pix] = make_float4(Cr + Tr * fr.bg[0], Cg + Tr * fr.bg[1], Cb + Tr * fr.bg[2], 1.0f - Tr);
+    if (BWD) {
+        // ---------------- backward: recurrence in the owner, octet scatter (every slab below belongs to this warp) ----------------
+        // fp32 SH basis over the fp16 B operand: pixel (row r, column c) at slot c * 4 + r, coefficient i at (i + 8 (r >> 1)) & 15,
+        // so that the four octets' reads of one column (8 consecutive coefficients each) touch every bank once
+        float* y32 = reinterpret_cast<float*>(ysm);
+        float4* rec_d = part;   // dL/ds of the four channels, slot mapping of rec_o / rec_w
+        __syncwarp();
+        {
+            float Y[16];
+#pragma unroll
+            for (int c = 0; c < 16; ++c) Y[c] = 0.0f;
+            float vx, vy, vz;
+            vs_view_dir(cams[view], px, py, vx, vy, vz);
+            vs_sh_basis<DEG>(vx, vy, vz, Y);
+            const uint32_t yr = lane >> 3, yc = lane & 7;
+            float4* row = reinterpret_cast<float4*>(y32 + (yc * 4 + yr) * 16);
+#pragma unroll
+            for (int q = 0; q < 4; ++q) row[(q + 2 * (yr >> 1)) & 3] = make_float4(Y[4 * q], Y[4 * q + 1], Y[4 * q + 2], Y[4 * q + 3]);
+        }
+        float4 g = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        if (inimg) g = __ldg(reinterpret_cast<const float4*>(grad_out) + pix);
+        float R = fr.bg[0] * g.x + fr.bg[1] * g.y + fr.bg[2] * g.z - g.w;
+        constexpr uint32_t NC = (uint32_t)S::NCOEF;   // float4s per gradient texel
+        for (int l = (int)sc.k - 1; l >= 0; --l) {
+            const bool on = (used >> l) & 1u;
+            if (__ballot_sync(0xFFFFFFFFu, on) == 0u) continue;   // warp-uniform
+            uint4 ro = make_uint4(0, 0, 0, 0);
+            float4 rw = make_float4(0.0f, 0.0f, 0.0f, 0.0f), rd = rw;
+            if (on) {
+                const float4 a4 = act[l * VS_SHADE_PIX + tid];
+                const float Tl = trans[l * VS_SHADE_PIX + tid];
+                const float aw = fr.attenuate ? rec_aw[l * VS_SHADE_PIX + tid] : 1.0f;
+                const float A = a4.w * aw;
+                const float cg = a4.x * g.x + a4.y * g.y + a4.z * g.z;
+                const float TA = Tl * A;
+                rd.x = TA * g.x * a4.x * (1.0f - a4.x);
+                rd.y = TA * g.y * a4.y * (1.0f - a4.y);
+                rd.z = TA * g.z * a4.z * (1.0f - a4.z);
+                rd.w = Tl * (cg - R) * aw * a4.w * (1.0f - a4.w);
+                R = A * cg + (1.0f - A) * R;
+                const float2 ab = rec_ab[l * VS_SHADE_PIX + tid];
+                const uint32_t xy = rec_xy[l * VS_SHADE_PIX + tid];
+                const uint32_t cx0 = xy & 0x7FFFu, cy0 = (xy >> 16) & 0x7FFFu, Wt = sc.tex_w[l];
+                const uint32_t row0 = cy0 * Wt, row1 = row0 + ((xy >> 31) ? Wt : 0u), cx1 = cx0 + ((xy >> 15) & 1u);
+                ro = make_uint4((row0 + cx0) * NC, (row0 + cx1) * NC, (row1 + cx0) * NC, (row1 + cx1) * NC);   // < 2^32: checked at scene creation
+                rw = make_float4((1.0f - ab.x) * (1.0f - ab.y), ab.x * (1.0f - ab.y), (1.0f - ab.x) * ab.y, ab.x * ab.y);
+            }
+            rec_o[own_slot] = ro; rec_w[own_slot] = rw; rec_d[own_slot] = rd;
+            __syncwarp();
+            float4* __restrict__ gl = reinterpret_cast<float4*>(gt.p[l]);
+#pragma unroll 2
+            for (int j = 0; j < 8; ++j) {
+                const uint32_t slot = 8 * oct + ((j + 2 * oct) & 7);   // fragment of pixel row oct, column j
+                const float4 w = rec_w[slot];
+                if (w.x == 0.0f && w.y == 0.0f && w.z == 0.0f && w.w == 0.0f) continue;
+                const uint4 o = rec_o[slot];
+                const float4 d = rec_d[slot];
+#pragma unroll
+#ifdef VS_BW_EXP_HALF   // timing experiment only (wrong gradients): half of the reductions
+                for (int h = 0; h < 1; ++h) {
+#else
+                for (int h = 0; h < 2; ++h) {
+#endif
+                    const uint32_t c = oi + 8 * h;
+                    if (c >= NC) continue;
+                    const float y = y32[(j * 4 + oct) * 16 + ((c + 8 * (oct >> 1)) & 15)];
+                    float wy = w.x * y; vs_red_add4(gl + o.x + c, wy * d.x, wy * d.y, wy * d.z, wy * d.w);
+                    wy = w.y * y;       vs_red_add4(gl + o.y + c, wy * d.x, wy * d.y, wy * d.z, wy * d.w);
+                    wy = w.z * y;       vs_red_add4(gl + o.z + c, wy * d.x, wy * d.y, wy * d.z, wy * d.w);
+                    wy = w.w * y;       vs_red_add4(gl + o.w + c, wy * d.x, wy * d.y, wy * d.z, wy * d.w);
+                }
+            }
+            __syncwarp();
+        }
+        return;
+    }
+    if (inimg) {
+        const float4 o4 = make_float4(Cr + Tr * fr.bg[0], Cg + Tr * fr.bg[1], Cb + Tr * fr.bg[2], 1.0f - Tr);
+#if VS_KEYS_STREAM >= 2
+        __stcs(reinterpret_cast<float4*>(out_rgba) + pix, o4);
+#else
+        reinterpret_cast<float4*>(out_rgba)[pix] = o4;
+#endif
+    }
 }
 
 template <int F16, int DEG, bool COUNT>
@@ -482,7 +588,7 @@ static cudaError_t launch_sh2(const VsSceneDev& sc, const VsFrame& fr, const VsC
     if (sc.texel_vecs != (uint32_t)VsShadeShape<F16, DEG>::NVEC) return cudaErrorInvalidValue;
     const size_t smem = (size_t)sc.k * VS_SHADE_PIX * (fr.attenuate ? 16 : 12) + VS_SHADE_WARPS * VS_SHADE_WARP_BYTES;
     const bool pf = VS_SHADE_PREFETCH && (VS_SHADE_PREFETCH >= 3 || ch.order == nullptr);
-    auto kern = pf ? k_shade<F16, DEG, COUNT, true> : k_shade<F16, DEG, COUNT, false>;
+    auto kern = pf ? k_shade<F16, DEG, COUNT, true, false> : k_shade<F16, DEG, COUNT, false, false>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
 #ifdef VS_SHADE_CARVEOUT
@@ -492,11 +598,42 @@ static cudaError_t launch_sh2(const VsSceneDev& sc, const VsFrame& fr, const VsC
     dim3 grid(fr.tiles_x * fr.tiles_y * VS_SHADE_SUBTILES, ch.views);
     if (ch.keys)
         kern<<<grid, VS_SHADE_PIX, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_mask, nullptr, ch.keys, ch.ids_is_output ? ch.ids : nullptr,
-                                      ch.out_rgba, ch.texel_bits, ch.counters, ch.order);
+                                      ch.out_rgba, ch.texel_bits, ch.counters, ch.order, nullptr, VsGradTex{});
     else
         kern<<<grid, VS_SHADE_PIX, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_off, ch.ids, nullptr, nullptr, ch.out_rgba, ch.texel_bits,
-                                      ch.counters, nullptr);
+                                      ch.counters, nullptr, nullptr, VsGradTex{});
     return cudaGetLastError();
+}
+
+// vs_render_backward on the direct path: k_shade<BWD> in place of k_shade (consumes and clears the same key image)
+template <int F16, int DEG>
+static cudaError_t launch_bwd(const VsSceneDev& sc, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
+{
+    if (sc.texel_vecs != (uint32_t)VsShadeShape<F16, DEG>::NVEC || !ch.keys) return cudaErrorInvalidValue;
+    // fragment records 12 B + attenuation weights 4 B + kept activations 20 B per pixel and layer, and the per-warp slabs
+    const size_t smem = (size_t)sc.k * VS_SHADE_PIX * 36 + VS_SHADE_WARPS * VS_SHADE_WARP_BYTES;
+    auto kern = k_shade<F16, DEG, false, false, true>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    dim3 grid(fr.tiles_x * fr.tiles_y * VS_SHADE_SUBTILES, ch.views);
+    kern<<<grid, VS_SHADE_PIX, smem, st>>>(sc, fr, ch.cams, ch.vtx, ch.tile_mask, nullptr, ch.keys, nullptr, nullptr, nullptr, ch.counters,
+                                           ch.order, ch.grad_out, ch.grad_tex);
+    return cudaGetLastError();
+}
+
+cudaError_t vs_launch_shade_backward(const VsSceneDev& sc, int f16, const VsFrame& fr, const VsChunk& ch, cudaStream_t st)
+{
+    switch ((f16 ? 4 : 0) + (int)sc.sh_degree) {
+        case 0: return launch_bwd<0, 0>(sc, fr, ch, st);
+        case 1: return launch_bwd<0, 1>(sc, fr, ch, st);
+        case 2: return launch_bwd<0, 2>(sc, fr, ch, st);
+        case 3: return launch_bwd<0, 3>(sc, fr, ch, st);
+        case 4: return launch_bwd<1, 0>(sc, fr, ch, st);
+        case 5: return launch_bwd<1, 1>(sc, fr, ch, st);
+        case 6: return launch_bwd<1, 2>(sc, fr, ch, st);
+        case 7: return launch_bwd<1, 3>(sc, fr, ch, st);
+    }
+    return cudaErrorInvalidValue;
 }
 
 template <int F16, int DEG>

@@ -235,7 +235,9 @@ def test_aov_reduced_config4(env, banded):
 # ---- backward pass to the texels through vs_render_backward ----
 def check_backward(env, sc, views, attenuation=False, t_min=None, background=None, views_per_chunk=0):
     """GPU gradient textures (fp32 atomics, any order) against the oracle's fp64 ones: max abs error <= 1e-4 of the
-    largest gradient magnitude of the layer + exact zeros where the oracle has exact zeros."""
+    largest gradient magnitude of the layer + exact zeros where the oracle has exact zeros.  Both backward kernels are
+    checked: the default k_shade<BWD> (k_shade's octet / tensor-core forward pass + recurrence + scatter) and the plain
+    k_backward (VS_FLAG_PLAIN_BACKWARD)."""
     if env.path_flags:
         pytest.skip("vs_render_backward runs on the direct raster path only")
     b, torch = env.binding, env.torch
@@ -244,30 +246,34 @@ def check_backward(env, sc, views, attenuation=False, t_min=None, background=Non
     g = rng.normal(size=(B, H, W, 4)).astype(np.float32)
     t_min = sc.t_min if t_min is None else t_min
     background = sc.background if background is None else background
-    p = b.make_params(W, H, sc.near_plane, t_min, background, b.VS_FLAG_ATTENUATION if attenuation else 0, views_per_chunk)
-    r = b.Renderer(sc)
-    grads = [torch.zeros(ly.texture.shape, dtype=torch.float32, device="cuda") for ly in sc.layers]
-    b.vs_render_backward(r.handle, sc.cameras[list(views)], p, torch.from_numpy(g).cuda(), grads)
-    torch.cuda.synchronize()
-    # the scene is untouched by the backward call: a forward render afterwards still matches the oracle
-    rgba, ids = r.render(sc.cameras[list(views)], p, want_ids=True)
-    torch.cuda.synchronize()
-    r.close()
     want = None
-    for n, v in enumerate(views):
-        ref = env.oracle.render_scene(sc, [v], t_min=t_min, background=background, attenuation=attenuation)[0]
-        assert np.array_equal(ids[n].cpu().numpy().view(np.uint32), ref["ids"])
-        want = env.oracle.render_backward(sc.layers, sc.sh_degree, sc.cameras[v], W, H, ref["ids"], g[n].astype(np.float64),
-                                          want, near_plane=sc.near_plane, t_min=t_min, background=background,
-                                          attenuation=attenuation)
     worst = 0.0
-    for l in range(sc.k):
-        got = grads[l].cpu().numpy().astype(np.float64)
-        scale = max(np.abs(want[l]).max(), 1e-30)
-        err = np.abs(got - want[l]).max() / scale
-        worst = max(worst, err)
-        assert err <= 1e-4, "layer %d: relative gradient error %.3e" % (l, err)
-        assert np.all(got[want[l] == 0.0] == 0.0)
+    for kernel_flag in (0, b.VS_FLAG_PLAIN_BACKWARD):
+        p = b.make_params(W, H, sc.near_plane, t_min, background, (b.VS_FLAG_ATTENUATION if attenuation else 0) | kernel_flag,
+                          views_per_chunk)
+        r = b.Renderer(sc)
+        grads = [torch.zeros(ly.texture.shape, dtype=torch.float32, device="cuda") for ly in sc.layers]
+        b.vs_render_backward(r.handle, sc.cameras[list(views)], p, torch.from_numpy(g).cuda(), grads)
+        torch.cuda.synchronize()
+        # the scene is untouched by the backward call: a forward render afterwards still matches the oracle
+        p_fwd = b.make_params(W, H, sc.near_plane, t_min, background, b.VS_FLAG_ATTENUATION if attenuation else 0, views_per_chunk)
+        rgba, ids = r.render(sc.cameras[list(views)], p_fwd, want_ids=True)
+        torch.cuda.synchronize()
+        r.close()
+        if want is None:
+            for n, v in enumerate(views):
+                ref = env.oracle.render_scene(sc, [v], t_min=t_min, background=background, attenuation=attenuation)[0]
+                assert np.array_equal(ids[n].cpu().numpy().view(np.uint32), ref["ids"])
+                want = env.oracle.render_backward(sc.layers, sc.sh_degree, sc.cameras[v], W, H, ref["ids"], g[n].astype(np.float64),
+                                                  want, near_plane=sc.near_plane, t_min=t_min, background=background,
+                                                  attenuation=attenuation)
+        for l in range(sc.k):
+            got = grads[l].cpu().numpy().astype(np.float64)
+            scale = max(np.abs(want[l]).max(), 1e-30)
+            err = np.abs(got - want[l]).max() / scale
+            worst = max(worst, err)
+            assert err <= 1e-4, "layer %d: relative gradient error %.3e (kernel flag %d)" % (l, err, kernel_flag)
+            assert np.all(got[want[l] == 0.0] == 0.0)
     return worst, want
 
 
@@ -330,7 +336,7 @@ def test_surface_order_is_a_permutation_of_screen_order(env):
     assert np.array_equal(a[0], c[0]) and np.array_equal(a[1], c[1])
 
 
-@pytest.mark.parametrize("dtype,deg", [(np.float32, 0), (np.float16, 0), (np.float16, 1), (np.float32, 2), (np.float32, 3)])
+@pytest.mark.parametrize("dtype,deg", [(np.float32, 0), (np.float16, 0), (np.float16, 1), (np.float16, 2), (np.float32, 2), (np.float32, 3)])
 def test_all_texture_formats(env, dtype, deg):
     rng = np.random.default_rng(5)
     sc = env.synth.make_config(1, width=96, height=80, num_cameras=2, tex_size=64)
@@ -339,6 +345,8 @@ def test_all_texture_formats(env, dtype, deg):
         ly.texture = rng.normal(0, 0.5, size=(48, 64, n, 4)).astype(dtype)     # non-square texture too
     sc.sh_degree = deg
     check_against_oracle(env, sc, [0, 1])
+    if not env.path_flags:   # every (format, degree) instantiation of the backward kernels too
+        check_backward(env, sc, [1])
 
 
 def test_edge_cases(env):
