@@ -141,6 +141,8 @@ def build_scene(cfg, rank, world, args):
         kw["num_cameras"] = args.views
     if getattr(args, "banded", False):
         kw["banded"] = True
+    if getattr(args, "tex_size", 0):
+        kw["tex_size"] = args.tex_size
     if getattr(args, "camera_subset", None):
         kw["camera_subset"] = args.camera_subset
     if getattr(args, "strong", False):
@@ -300,7 +302,7 @@ def run_ours(args):
     step_achieved = alg_bytes_step * world / (secs_max / args.steps) / 1e9
     views_per_launch = B * args.steps / max(shade_launches, 1)
     traffic_key = "%d%s%s" % (args.config, "-" + args.camera_subset if args.camera_subset else "", "-backward" if args.backward else "")
-    plain = not (args.tiled or args.attenuation or args.overlap or args.screen_order or args.views or banded or args.lib or args.plain_backward)
+    plain = not (args.tiled or args.attenuation or args.overlap or args.screen_order or args.views or banded or args.lib or args.plain_backward or args.tex_size)
     traffic_per_view, traffic_src = ncu_traffic_bytes_per_view(traffic_key, views_per_launch) if plain else (None, "not the captured launch configuration")
     # the three candidate bounds of SURVEY.md §8(d), per view: HBM (algorithmic bytes), L1 gather (4 texels per fragment through
     # the 128 B/clk/SM data pipe), FP32 issue (algorithmic lane-ops: 4 x 4n bilinear + SH FMAs, 4 x 4n half->float conversions
@@ -412,6 +414,7 @@ def main():
     ap.add_argument("--banded", action="store_true", help="the paper's 8-bit mixed-resolution textures on the same geometry (PAPER.md:L445-459; not the headline workload)")
     ap.add_argument("--attenuation", action="store_true", help="render with VS_FLAG_ATTENUATION (PAPER.md:L279-286; not the headline workload)")
     ap.add_argument("--tiled", action="store_true", help="time the per-tile raster path (VS_FLAG_TILED_PATH) instead of the default direct one")
+    ap.add_argument("--tex-size", type=int, default=0, help="override the texture side (e.g. 512 on C4: magnified texels, the fitting regime of PAPER.md:L441-443; not the headline workload)")
     ap.add_argument("--plain-backward", action="store_true", help="with --backward: VS_FLAG_PLAIN_BACKWARD, the plain per-lane k_backward instead of k_shade<BWD> (A/B)")
     ap.add_argument("--screen-order", action="store_true", help="VS_FLAG_SCREEN_ORDER: shade view by view instead of in surface order (A/B, DESIGN.md §7)")
     ap.add_argument("--overlap", action="store_true", help="VS_FLAG_OVERLAP: S1-S4 of the next chunk beside S5-S7 of the current one (experiment, DESIGN.md §7)")

@@ -530,8 +530,8 @@ static vs_status validate_render(const vs_scene* scene, const vs_camera* cams, u
 // Views per internal pass (chunk).  A pass keeps the transformed vertices and the key image (or packed tile ranges + id
 // planes) of its views in one of the scene's two scratch sets.  Larger passes let more views share texels through L2 in
 // surface order and launch fewer kernels (C4, 64 views: 23.5 ms in passes of 16, 23.0 of 32, 22.9 of 64), so device outputs
-// take up to VS_CHUNK_DEVICE views as long as a set stays under a sixteenth of the device memory that is free at the
-// scene's first call (and under 8 GB); the views are then spread evenly over the passes.  Host outputs: at most 4 views, so
+// take up to VS_CHUNK_DEVICE views as long as a set stays under a twelfth of the device memory that is free at the
+// scene's first call (and under 12 GB); the views are then spread evenly over the passes.  Host outputs: at most 4 views, so
 // that the download of one chunk overlaps the rendering of the next.
 #ifndef VS_CHUNK_DEVICE
 #define VS_CHUNK_DEVICE 64u
@@ -543,8 +543,8 @@ static uint32_t pick_chunk(vs_scene* s, const vs_render_params* p, uint32_t n, b
     if (s->scratch_budget == 0) {
         size_t free_b = 0, total_b = 0;
         if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); free_b = (size_t)48 << 30; }
-        s->scratch_budget = free_b / 16;
-        if (s->scratch_budget > ((size_t)8 << 30)) s->scratch_budget = (size_t)8 << 30;
+        s->scratch_budget = free_b / 12;   // per scratch set (there are two)
+        if (s->scratch_budget > ((size_t)12 << 30)) s->scratch_budget = (size_t)12 << 30;
         if (s->scratch_budget < ((size_t)1 << 30)) s->scratch_budget = (size_t)1 << 30;
     }
     const bool tiled = (p->flags & VS_FLAG_TILED_PATH) != 0;

@@ -544,8 +544,68 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
                 rw = make_float4((1.0f - ab.x) * (1.0f - ab.y), ab.x * (1.0f - ab.y), (1.0f - ab.x) * ab.y, ab.x * ab.y);
             }
             rec_o[own_slot] = ro; rec_w[own_slot] = rw; rec_d[own_slot] = rd;
+            // Magnified textures (close-ups; the fitting regime of PAPER.md:L441-443, where many pixels fall into one texel
+            // cell): neighbouring pixels of a row then have the SAME 2x2 footprint, and the octet, which walks its row from
+            // left to right, sums such a run in registers and issues the reductions once per run instead of once per pixel.
+            // Taken only by warps in which some pixel shares its footprint with its left neighbour (warp-uniform).
+            bool merge;
+            {
+                const uint32_t lx0 = __shfl_up_sync(0xFFFFFFFFu, ro.x, 1), ly0 = __shfl_up_sync(0xFFFFFFFFu, ro.y, 1);
+                const uint32_t lz0 = __shfl_up_sync(0xFFFFFFFFu, ro.z, 1), lw0 = __shfl_up_sync(0xFFFFFFFFu, ro.w, 1);
+                const int lon = __shfl_up_sync(0xFFFFFFFFu, (int)on, 1);
+                merge = __any_sync(0xFFFFFFFFu, on && lon && (lane & 7u) != 0u && lx0 == ro.x && ly0 == ro.y && lz0 == ro.z && lw0 == ro.w);
+            }
             __syncwarp();
             float4* __restrict__ gl = reinterpret_cast<float4*>(gt.p[l]);
+#ifdef VS_BW_NO_MERGE   // experiment switch: always one set of reductions per pixel
+            merge = false;
+#endif
+            if (merge) {
+                float4 acc[2][4];
+                uint4 cur = make_uint4(0, 0, 0, 0);
+                bool have = false;
+                auto flush = [&]() {
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const uint32_t c = oi + 8 * h;
+                        if (c >= NC) continue;
+                        vs_red_add4(gl + cur.x + c, acc[h][0].x, acc[h][0].y, acc[h][0].z, acc[h][0].w);
+                        vs_red_add4(gl + cur.y + c, acc[h][1].x, acc[h][1].y, acc[h][1].z, acc[h][1].w);
+                        vs_red_add4(gl + cur.z + c, acc[h][2].x, acc[h][2].y, acc[h][2].z, acc[h][2].w);
+                        vs_red_add4(gl + cur.w + c, acc[h][3].x, acc[h][3].y, acc[h][3].z, acc[h][3].w);
+                    }
+                };
+#pragma unroll 1
+                for (int j = 0; j < 8; ++j) {
+                    const uint32_t slot = 8 * oct + ((j + 2 * oct) & 7);
+                    const float4 w = rec_w[slot];
+                    if (w.x == 0.0f && w.y == 0.0f && w.z == 0.0f && w.w == 0.0f) continue;   // (does not end a run)
+                    const uint4 o = rec_o[slot];
+                    const float4 d = rec_d[slot];
+                    if (!(have && o.x == cur.x && o.y == cur.y && o.z == cur.z && o.w == cur.w)) {   // octet-uniform
+                        if (have) flush();
+                        cur = o; have = true;
+#pragma unroll
+                        for (int h = 0; h < 2; ++h)
+#pragma unroll
+                            for (int q = 0; q < 4; ++q) acc[h][q] = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+                    }
+                    const float wq[4] = {w.x, w.y, w.z, w.w};
+#pragma unroll
+                    for (int h = 0; h < 2; ++h) {
+                        const uint32_t c = oi + 8 * h;
+                        if (c >= NC) continue;
+                        const float y = y32[(j * 4 + oct) * 16 + ((c + 8 * (oct >> 1)) & 15)];
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) {
+                            const float wy = wq[q] * y;
+                            acc[h][q].x = fmaf(wy, d.x, acc[h][q].x); acc[h][q].y = fmaf(wy, d.y, acc[h][q].y);
+                            acc[h][q].z = fmaf(wy, d.z, acc[h][q].z); acc[h][q].w = fmaf(wy, d.w, acc[h][q].w);
+                        }
+                    }
+                }
+                if (have) flush();
+            } else {
 #pragma unroll 2
             for (int j = 0; j < 8; ++j) {
                 const uint32_t slot = 8 * oct + ((j + 2 * oct) & 7);   // fragment of pixel row oct, column j
@@ -567,6 +627,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
                     wy = w.z * y;       vs_red_add4(gl + o.z + c, wy * d.x, wy * d.y, wy * d.z, wy * d.w);
                     wy = w.w * y;       vs_red_add4(gl + o.w + c, wy * d.x, wy * d.y, wy * d.z, wy * d.w);
                 }
+            }
             }
             __syncwarp();
         }
