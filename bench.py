@@ -433,7 +433,7 @@ def main():
             table = json.load(open(TRAFFIC_FILE))
         except Exception:
             table = {}
-        table[key] = {"kernel": "k_shade", "dram_bytes_per_view": float(nbytes), "views_per_launch": int(vpl), "commit": commit,
+        table[key] = {"kernel": "k_shade<BWD>" if key.endswith("-backward") else "k_shade", "dram_bytes_per_view": float(nbytes), "views_per_launch": int(vpl), "commit": commit,
                       "summary": summary, "source_sha256": kernel_source_hashes()}
         json.dump(table, open(TRAFFIC_FILE, "w"), indent=1, sort_keys=True)
         print("recorded", key, "in", TRAFFIC_FILE)
