@@ -6,22 +6,22 @@
 // rasterisation itself, so this path visits every triangle exactly once:
 //   phase 1, lane = triangle: coalesced index record, three vertex gathers, integer setup, sample
 //     bounding box clipped to the screen.  A triangle whose box fits 8x8 samples gets its coverage mask
-//     from three biased int32 edge functions stepped with exact adds (same arithmetic as k_raster) and
-//     leaves a 12-word record in the warp's shared-memory slab.
-//   phase 2, lane = covered sample: the warp's masks are compacted into a queue of (lane, sample) codes so
-//     that all 32 lanes evaluate one covered sample each: fp32-exact depth key (IEEE division) and one
-//     fire-and-forget 64-bit max (RED.MAX.U64) on keys[view][layer][y][x].  The maximum is order
-//     independent, so the key image is the same whatever the scheduling (reading Q18).
+//     from three biased int32 edge functions stepped with exact adds (same arithmetic as k_raster).
+//   phase 2, lane = triangle: every lane walks the set bits of its own mask: fp32-exact depth key (IEEE
+//     division, the reciprocal of the triangle's area hoisted out of the loop) and one fire-and-forget
+//     64-bit max (RED.MAX.U64) on keys[view][layer][y][x] per covered sample.  The maximum is order
+//     independent, so the key image is the same whatever the scheduling (reading Q18).  (Until round 2's
+//     last session the covered samples of a warp were compacted into a shared-memory queue so that all 32
+//     lanes had one sample each; measured: 5.6 iterations of 48 instructions + 141 for the compaction
+//     against 7.4 iterations of ~27 -- the warp's largest mask is only 1.7x its mean.)
 //   larger triangles are broadcast one at a time and the warp maps its lanes to 8x4 pixel chunks of the
 //     box; triangles whose box exceeds VS_BIG_SAMPLES samples are appended to a list that k_raster_big
 //     spreads over the whole grid.
 // The key image must be zero on entry; k_shade reads it (id = ~low word) and clears what it read.
 // tile_mask[view][tile] (zero on entry) receives the layers whose triangles' boxes touch the tile.
 #include "vs_common.cuh"
+#include "vs_div.cuh"
 
-#define VS_RD_FIELDS 12
-#define VS_RD_QUEUE 512u
-#define VS_RD_WARP_WORDS (VS_RD_FIELDS * 32 + 256)
 #define VS_BIG_SAMPLES 4096   // clipped-box samples above which a triangle goes to the big list
 
 __device__ __forceinline__ void vs_key_red(unsigned long long* slot, unsigned long long key)
@@ -89,16 +89,12 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
                 uint32_t* __restrict__ tile_mask, uint2* __restrict__ big_list, uint32_t* __restrict__ big_count, uint32_t big_capacity,
                 unsigned long long* __restrict__ counters, uint32_t blocks_per_view, uint32_t total_blocks)
 {
-    __shared__ __align__(16) int slab[(VS_RD_THREADS / 32) * VS_RD_WARP_WORDS];
-    const uint32_t tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const uint32_t tid = threadIdx.x, lane = tid & 31;
     const int W = (int)fr.width, H = (int)fr.height;
     const size_t plane_px = (size_t)W * H;
-    int4* rec4 = reinterpret_cast<int4*>(slab + warp * VS_RD_WARP_WORDS);                 // [vector][lane]
-    unsigned short* queue = reinterpret_cast<unsigned short*>(slab + warp * VS_RD_WARP_WORDS + VS_RD_FIELDS * 32);   // [512]
     // work item = (view, block of VS_RD_THREADS consecutive triangles).  The grid has one CTA per item (x = block, y = view)
     // or, RESIDENT (the kernel runs beside the previous chunk's k_shade), a few CTAs per SM that stride over the items
     for (uint32_t item = RESIDENT ? blockIdx.x : 0u; item < (RESIDENT ? total_blocks : 1u); item += gridDim.x) {
-    if (RESIDENT) __syncwarp();   // the previous item's phase 2 has finished reading this warp's slab
     const uint32_t view = RESIDENT ? item / blocks_per_view : blockIdx.y;
     const uint32_t gt = (RESIDENT ? item - view * blocks_per_view : blockIdx.x) * (uint32_t)VS_RD_THREADS + tid;
     const int4* __restrict__ vv = vtx + (size_t)view * sc.v_total;
@@ -165,11 +161,11 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
         }
     }
     uint32_t mlo = 0, mhi = 0;  // coverage of the clipped box, sample (r, c) -> bit 8r + c of mhi:mlo
-    int E0 = 0, E1 = 0, E2 = 0, sx0 = 0, sx1 = 0, sx2 = 0, sy0 = 0, sy1 = 0, sy2 = 0;
+    int E0 = 0, E1 = 0, E2 = 0, sx0 = 0, sx1 = 0, sx2 = 0, sy0 = 0, sy1 = 0, sy2 = 0, E0u = 0, E1u = 0;
     const bool small = valid && !large;
     // The coverage loop below runs max-over-lanes(rows) x max-over-lanes(columns) steps for the whole warp.  A lane whose box is
     // taller than wide transposes it (loop row = image column): every lane then has rows <= columns, and a warp that holds a
-    // 2x7 and a 7x2 box loops 2x7 times instead of 7x7.  `transposed` travels to phase 2 in the sign bit of the stored A2.
+    // 2x7 and a 7x2 box loops 2x7 times instead of 7x7.  
     const bool transposed = small && (j1 - j0) > (i1 - i0);
     if (small) {
         // edge e_i runs (i+1) -> (i+2) and weights vertex i; sample (i0, j0)
@@ -185,12 +181,7 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
             int t;
             t = sx0; sx0 = sy0; sy0 = t; t = sx1; sx1 = sy1; sy1 = t; t = sx2; sx2 = sy2; sy2 = t;
         }
-        // three 16-byte vectors per triangle: {E0, E1, sx0, sx1} {sy0, sy1, A2 | transposed << 31, key offset} {q0, q1, q2, id}
-        // (A2 < 2^28 on this path: the triangle is narrow)
-        rec4[0 * 32 + lane] = make_int4(E0, E1, sx0, sx1);
-        rec4[1 * 32 + lane] = make_int4(sy0, sy1, (int)((uint32_t)T.A2 | (transposed ? 0x80000000u : 0u)),
-                                        (int)((uint32_t)(layer * plane_px) + (uint32_t)(j0 * W + i0)));  // < 2^32: checked by the launcher
-        rec4[2 * 32 + lane] = make_int4(__float_as_int(T.q0), __float_as_int(T.q1), __float_as_int(T.q2), (int)lid);
+        E0u = E0; E1u = E1;   // the unbiased values at sample (i0, j0): the depth key interpolates with these
         // covered <=> E_e > 0 || (E_e == 0 && topleft_e) <=> F_e := E_e - (topleft_e ? 0 : 1) >= 0
         E0 -= ((dy0 < 0) || (dy0 == 0 && dx0 > 0)) ? 0 : 1;
         E1 -= ((dy1 < 0) || (dy1 == 0 && dx1 > 0)) ? 0 : 1;
@@ -224,51 +215,46 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
         mlo &= colm & (nr >= 4 ? 0xFFFFFFFFu : ((1u << (8 * nr)) - 1u));
         mhi &= colm & (nr >= 8 ? 0xFFFFFFFFu : (nr > 4 ? ((1u << (8 * (nr - 4))) - 1u) : 0u));
     }
-    // ---------------- compaction: (lane, bit) codes of the covered samples ----------------
-    const uint32_t cnt = (uint32_t)(__popc(mlo) + __popc(mhi));
-    uint32_t incl = cnt;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t u = __shfl_up_sync(0xFFFFFFFFu, incl, o);
-        if (lane >= (uint32_t)o) incl += u;
+#ifndef VS_RD_NO_DEMOTE
+    {
+        // phase 2 runs as many rounds as the warp's LARGEST mask has bits.  A lane whose mask is far above the warp's mean (a few
+        // big triangles among small ones: close-ups, silhouettes) would keep the other 31 waiting: it hands its triangle to the
+        // warp-cooperative path below instead (every lane one sample of the box per round).
+        const uint32_t cnt = (uint32_t)(__popc(mlo) + __popc(mhi));
+        const uint32_t tot = __reduce_add_sync(0xFFFFFFFFu, cnt);
+        if (cnt > max(12u, (3u * tot) >> 5)) { large = true; mlo = 0u; mhi = 0u; }
     }
-    const uint32_t total = __shfl_sync(0xFFFFFFFFu, incl, 31);
-    for (uint32_t win = 0; win < total; win += VS_RD_QUEUE) {  // one round unless the warp covers > 512 samples
-        {
-            uint32_t off = incl - cnt - win;  // wraps for codes in front of the window: fails the bound test
-            uint32_t m = mlo;
-            while (m) {
-                const int bit = __ffs(m) - 1;
-                m &= m - 1;
-                if (off < VS_RD_QUEUE) queue[off] = (unsigned short)((lane << 6) | (uint32_t)bit);
-                ++off;
-            }
-            m = mhi;   // (rows 4..7: empty for almost every warp now that rows <= columns)
-            while (m) {
-                const int bit = __ffs(m) - 1;
-                m &= m - 1;
-                if (off < VS_RD_QUEUE) queue[off] = (unsigned short)((lane << 6) | 32u | (uint32_t)bit);
-                ++off;
-            }
-        }
-        __syncwarp();
-        // ---------------- phase 2: lane = covered sample ----------------
-        const uint32_t n = min(total - win, (uint32_t)VS_RD_QUEUE);
-        for (uint32_t s = lane; s < n; s += 32) {
-            const uint32_t code = queue[s];
-            const uint32_t src = code >> 6;
-            const int r = (int)((code >> 3) & 7u), c = (int)(code & 7u);   // loop row / loop column of the sample
-            const int4 ra = rec4[0 * 32 + src], rb = rec4[1 * 32 + src], rc = rec4[2 * 32 + src];
-            const int e0 = ra.x + r * rb.x + c * ra.z;
-            const int e1 = ra.y + r * rb.y + c * ra.w;
-            const int A2 = rb.z & 0x7FFFFFFF;
+#endif
+    // ---------------- phase 2: lane = triangle, one covered sample of every lane's own mask per round ----------------
+    if (__any_sync(0xFFFFFFFFu, (mlo | mhi) != 0u)) {
+        // (a small triangle's A2 < 2^24: its box has at most 8x8 samples, so A2 and the edge values are exact in fp32)
+        const int A2 = (int)T.A2;
+        const float fA = __int2float_rn(A2);
+        const float rA = vs_rcp_seed(fA);
+        // the seeded division is __fdiv_rn's own in-range path; operands near the ends of the exponent range (a scene at
+        // w ~ 1e20 or 1e-20) take the library division instead
+        const float qlo = fminf(T.q0, fminf(T.q1, T.q2)), qhi = fmaxf(T.q0, fmaxf(T.q1, T.q2));
+        const bool seeded = qlo > 1e-20f && qhi < 1e20f;
+        const int str_r = transposed ? 1 : W, str_c = transposed ? W : 1;   // a transposed box: loop row = image column
+        const uint32_t koff = (uint32_t)(layer * plane_px) + (uint32_t)(j0 * W + i0);   // < 2^32: checked by the launcher
+        const uint32_t klo = 0xFFFFFFFFu - lid;
+        auto resolve = [&](int r, int c) {
+            const int e0 = E0u + r * sy0 + c * sx0;
+            const int e1 = E1u + r * sy1 + c * sx1;
             const int e2 = A2 - e0 - e1;  // E0 + E1 + E2 == A2 at every point
-            const float qp = vs_depth_div(__int2float_rn(e0), __int2float_rn(e1), __int2float_rn(e2),
-                                          __int_as_float(rc.x), __int_as_float(rc.y), __int_as_float(rc.z), __int2float_rn(A2));
-            const int py = rb.z < 0 ? c : r, pxo = rb.z < 0 ? r : c;        // a transposed box: loop row = image column
-            vs_key_red(&vkeys[(uint32_t)rb.w + (uint32_t)(py * W + pxo)], vs_make_key(qp, (uint32_t)rc.w));
+            const float num = __fmaf_rn(__int2float_rn(e2), T.q2, __fmaf_rn(__int2float_rn(e1), T.q1, __fmul_rn(__int2float_rn(e0), T.q0)));
+            const float qp = seeded ? vs_div_seeded(num, fA, rA) : __fdiv_rn(num, fA);
+            const uint32_t idx = koff + (uint32_t)(r * str_r + c * str_c);
+            vs_key_red(&vkeys[idx], ((unsigned long long)__float_as_uint(qp) << 32) | klo);
+        };
+        for (uint32_t m = mlo; m; m &= m - 1) {
+            const int bit = __ffs(m) - 1;
+            resolve(bit >> 3, bit & 7);
         }
-        __syncwarp();
+        for (uint32_t m = mhi; m; m &= m - 1) {   // (rows 4..7: empty for most warps now that rows <= columns)
+            const int bit = __ffs(m) - 1;
+            resolve(4 + (bit >> 3), bit & 7);
+        }
     }
     // ---------------- large triangles ----------------
     bool big = false;
