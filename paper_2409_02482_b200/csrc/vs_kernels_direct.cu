@@ -21,6 +21,7 @@
 // tile_mask[view][tile] (zero on entry) receives the layers whose triangles' boxes touch the tile.
 #include "vs_common.cuh"
 #include "vs_div.cuh"
+#include <type_traits>
 
 #define VS_BIG_SAMPLES 4096   // clipped-box samples above which a triangle goes to the big list
 
@@ -78,7 +79,7 @@ __device__ __forceinline__ void vs_direct_large(int X0, int Y0, int X1, int Y1, 
 }
 
 #ifndef VS_RD_THREADS
-#define VS_RD_THREADS 256
+#define VS_RD_THREADS 128
 #endif
 #ifndef VS_RD_MIN_CTAS
 #define VS_RD_MIN_CTAS (1024 / VS_RD_THREADS)
@@ -87,7 +88,7 @@ template <bool RESIDENT>
 __global__ void __launch_bounds__(VS_RD_THREADS, VS_RD_MIN_CTAS)
 k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ vtx, unsigned long long* __restrict__ keys,
                 uint32_t* __restrict__ tile_mask, uint2* __restrict__ big_list, uint32_t* __restrict__ big_count, uint32_t big_capacity,
-                unsigned long long* __restrict__ counters, uint32_t blocks_per_view, uint32_t total_blocks)
+                unsigned long long* __restrict__ counters, uint32_t blocks_per_view, uint32_t total_blocks, uint32_t view_major)
 {
     const uint32_t tid = threadIdx.x, lane = tid & 31;
     const int W = (int)fr.width, H = (int)fr.height;
@@ -95,8 +96,11 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
     // work item = (view, block of VS_RD_THREADS consecutive triangles).  The grid has one CTA per item (x = block, y = view)
     // or, RESIDENT (the kernel runs beside the previous chunk's k_shade), a few CTAs per SM that stride over the items
     for (uint32_t item = RESIDENT ? blockIdx.x : 0u; item < (RESIDENT ? total_blocks : 1u); item += gridDim.x) {
-    const uint32_t view = RESIDENT ? item / blocks_per_view : blockIdx.y;
-    const uint32_t gt = (RESIDENT ? item - view * blocks_per_view : blockIdx.x) * (uint32_t)VS_RD_THREADS + tid;
+    // 2-D grid: x = view, y = block of triangles when the block count fits gridDim.y (view_major), else x = block, y = view.
+    // View-major, CTAs that are dispatched together read the SAME index records for different views: the 16 bytes per
+    // triangle come from L2 instead of HBM for all views but one, and a warp's first load returns sooner.
+    const uint32_t view = RESIDENT ? item / blocks_per_view : (view_major ? blockIdx.x : blockIdx.y);
+    const uint32_t gt = (RESIDENT ? item - view * blocks_per_view : (view_major ? blockIdx.y : blockIdx.x)) * (uint32_t)VS_RD_THREADS + tid;
     const int4* __restrict__ vv = vtx + (size_t)view * sc.v_total;
     unsigned long long* __restrict__ vkeys = keys + (size_t)view * sc.k * plane_px;
 
@@ -199,13 +203,21 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
             if (r < rows) {
                 uint32_t bits = 0;
                 int c0 = a0, c1 = a1, c2 = a2;
-#pragma unroll
-                for (int c = 7; c >= 0; --c) {
-                    if (c < cols) {  // warp-uniform
-                        bits = __funnelshift_l((uint32_t)(c0 | c1 | c2), bits, 1);
-                        c0 -= sx0; c1 -= sx1; c2 -= sx2;
-                    }
+                // exactly `cols` steps (warp-uniform): enter the unrolled sequence at the right step instead of predicating
+                // all eight (the predicated-off steps of a 4-column warp still cost their issue slots)
+#define VS_RD_STEP bits = __funnelshift_l((uint32_t)(c0 | c1 | c2), bits, 1); c0 -= sx0; c1 -= sx1; c2 -= sx2;
+                switch (cols) {
+                    case 8: VS_RD_STEP  // fall through
+                    case 7: VS_RD_STEP  // fall through
+                    case 6: VS_RD_STEP  // fall through
+                    case 5: VS_RD_STEP  // fall through
+                    case 4: VS_RD_STEP  // fall through
+                    case 3: VS_RD_STEP  // fall through
+                    case 2: VS_RD_STEP  // fall through
+                    case 1: bits = __funnelshift_l((uint32_t)(c0 | c1 | c2), bits, 1);
+                    default: break;
                 }
+#undef VS_RD_STEP
                 bits = ~bits & 0xFFu;
                 if (r < 4) mlo |= bits << (8 * r); else mhi |= bits << (8 * (r - 4));
                 a0 += sy0; a1 += sy1; a2 += sy2;
@@ -234,27 +246,32 @@ k_raster_direct(const VsSceneDev sc, const VsFrame fr, const int4* __restrict__ 
         // the seeded division is __fdiv_rn's own in-range path; operands near the ends of the exponent range (a scene at
         // w ~ 1e20 or 1e-20) take the library division instead
         const float qlo = fminf(T.q0, fminf(T.q1, T.q2)), qhi = fmaxf(T.q0, fmaxf(T.q1, T.q2));
-        const bool seeded = qlo > 1e-20f && qhi < 1e20f;
+        const bool seeded = __all_sync(0xFFFFFFFFu, (mlo | mhi) == 0u || (qlo > 1e-20f && qhi < 1e20f));   // warp-uniform
         const int str_r = transposed ? 1 : W, str_c = transposed ? W : 1;   // a transposed box: loop row = image column
         const uint32_t koff = (uint32_t)(layer * plane_px) + (uint32_t)(j0 * W + i0);   // < 2^32: checked by the launcher
         const uint32_t klo = 0xFFFFFFFFu - lid;
-        auto resolve = [&](int r, int c) {
+        auto resolve = [&](int r, int c, auto seeded_tag) {
             const int e0 = E0u + r * sy0 + c * sx0;
             const int e1 = E1u + r * sy1 + c * sx1;
             const int e2 = A2 - e0 - e1;  // E0 + E1 + E2 == A2 at every point
             const float num = __fmaf_rn(__int2float_rn(e2), T.q2, __fmaf_rn(__int2float_rn(e1), T.q1, __fmul_rn(__int2float_rn(e0), T.q0)));
-            const float qp = seeded ? vs_div_seeded(num, fA, rA) : __fdiv_rn(num, fA);
+            const float qp = decltype(seeded_tag)::value ? vs_div_seeded(num, fA, rA) : __fdiv_rn(num, fA);
             const uint32_t idx = koff + (uint32_t)(r * str_r + c * str_c);
-            vs_key_red(&vkeys[idx], ((unsigned long long)__float_as_uint(qp) << 32) | klo);
+            unsigned long long* slot;   // one IMAD.WIDE.U32: 64-bit base + 8 * 32-bit index
+            asm("mad.wide.u32 %0, %1, 8, %2;" : "=l"(slot) : "r"(idx), "l"(vkeys));
+            vs_key_red(slot, ((unsigned long long)__float_as_uint(qp) << 32) | klo);
         };
-        for (uint32_t m = mlo; m; m &= m - 1) {
-            const int bit = __ffs(m) - 1;
-            resolve(bit >> 3, bit & 7);
-        }
-        for (uint32_t m = mhi; m; m &= m - 1) {   // (rows 4..7: empty for most warps now that rows <= columns)
-            const int bit = __ffs(m) - 1;
-            resolve(4 + (bit >> 3), bit & 7);
-        }
+        auto walk = [&](auto seeded_tag) {
+            for (uint32_t m = mlo; m; m &= m - 1) {
+                const int bit = __ffs(m) - 1;
+                resolve(bit >> 3, bit & 7, seeded_tag);
+            }
+            for (uint32_t m = mhi; m; m &= m - 1) {   // (rows 4..7: empty for most warps now that rows <= columns)
+                const int bit = __ffs(m) - 1;
+                resolve(4 + (bit >> 3), bit & 7, seeded_tag);
+            }
+        };
+        if (seeded) walk(std::true_type{}); else walk(std::false_type{});
     }
     // ---------------- large triangles ----------------
     bool big = false;
@@ -330,10 +347,16 @@ cudaError_t vs_launch_raster_direct(const VsSceneDev& sc, const VsFrame& fr, con
     // resident_ctas != 0: that many CTAs stride over the work items (the kernel shares the SMs with another one)
     if (resident_ctas && resident_ctas < total)
         k_raster_direct<true><<<resident_ctas, VS_RD_THREADS, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.tile_mask, ch.big_list, ch.big_count,
-                                                                       ch.big_capacity, ch.counters, bpv, (uint32_t)total);
-    else
-        k_raster_direct<false><<<dim3(bpv, ch.views), VS_RD_THREADS, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.tile_mask, ch.big_list,
-                                                                              ch.big_count, ch.big_capacity, ch.counters, bpv, (uint32_t)total);
+                                                                       ch.big_capacity, ch.counters, bpv, (uint32_t)total, 0u);
+    else {
+#ifdef VS_RD_BLOCK_MAJOR   // experiment switch: the grid order of the earlier versions
+        const bool view_major = false;
+#else
+        const bool view_major = bpv <= 65535u;
+#endif
+        k_raster_direct<false><<<view_major ? dim3(ch.views, bpv) : dim3(bpv, ch.views), VS_RD_THREADS, 0, st>>>(
+            sc, fr, ch.vtx, ch.keys, ch.tile_mask, ch.big_list, ch.big_count, ch.big_capacity, ch.counters, bpv, (uint32_t)total, view_major ? 1u : 0u);
+    }
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return e;
     k_raster_big<<<resident_ctas ? 148 : 148 * 4, 256, 0, st>>>(sc, fr, ch.vtx, ch.keys, ch.big_list, ch.big_count, ch.big_capacity);
