@@ -345,6 +345,17 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
     }
     const uint32_t ychunk0 = ((oi % LPC) * NE) >> 2;   // first 16-byte chunk of this lane's coefficients
     const bool lane_on = oi < (uint32_t)NACT;
+#ifndef VS_SHADE_BF_REGS
+#define VS_SHADE_BF_REGS 1    // 1: the tensor-core path keeps the B fragments (SH basis) of its 8 columns in 16 registers for all layers
+#endif
+    uint2 bfr[8];
+    if (S::MMA && VS_SHADE_BF_REGS) {
+        __syncwarp();
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            bfr[j] = *reinterpret_cast<const uint2*>(reinterpret_cast<const unsigned char*>(ysm) +
+                (oct * 8 + ((uint32_t)j ^ (oct & 1))) * 64 + ((((oi >> 2) * 2 + ((oi & 3) >> 1)) + (oct >> 1) + (j >> 1)) & 3) * 16 + (oi & 1) * 8);
+    }
 
     float Tr = 1.0f, Cr = 0.0f, Cg = 0.0f, Cb = 0.0f;
     bool alive = true;
@@ -427,7 +438,7 @@ k_shade(const VsSceneDev sc, const VsFrame fr, const VsCamDev* __restrict__ cams
             if (S::MMA) {
                 // rows of A = (fragment f = octet, channel), columns of B = (fragment, hi | lo): lane (g = lane >> 2, t = lane & 3)
                 // gets D[g][2t .. 2t+1] and D[g+8][..]; the entries of its OWN fragment are those of t == f
-                const uint2 bf = *reinterpret_cast<const uint2*>(reinterpret_cast<const unsigned char*>(ysm) +
+                const uint2 bf = VS_SHADE_BF_REGS ? bfr[j] : *reinterpret_cast<const uint2*>(reinterpret_cast<const unsigned char*>(ysm) +
                     (oct * 8 + ((uint32_t)j ^ (oct & 1))) * 64 + ((((oi >> 2) * 2 + ((oi & 3) >> 1)) + (oct >> 1) + (j >> 1)) & 3) * 16 + (oi & 1) * 8);
                 float d0, d1, d2, d3, sa, sb;
                 vs_mma_16816(d0, d1, d2, d3, tv[tb_i][0][0], bf.x, bf.y);
