@@ -349,6 +349,22 @@ def test_all_texture_formats(env, dtype, deg):
         check_backward(env, sc, [1])
 
 
+def test_far_scene_takes_the_library_division(env):
+    """k_raster_direct hoists the reciprocal of the triangle's area out of its per-sample loop (csrc/vs_div.cuh) only while
+    1/w stays inside [1e-20, 1e20]; a scene 2^70 units away (1/w ~ 3e-22) must take the library division instead and still
+    give the oracle's ids.  Scaling by a power of two is exact in fp32, so the images are those of the unscaled scene."""
+    sc = env.synth.make_config(1, width=96, height=72, num_cameras=2, tex_size=64)
+    near = gpu_render(env, sc, [0, 1])
+    scale = np.float32(2.0 ** 70)
+    for ly in sc.layers:
+        ly.positions = (ly.positions * scale).astype(np.float32)
+    sc.cameras = sc.cameras.copy()
+    sc.cameras[:, 13:16] *= scale
+    worst, rgba, ids = check_against_oracle(env, sc, [0, 1])
+    assert (ids != env.binding.MISS).mean() > 0.3
+    assert np.array_equal(ids, near[1]) and np.allclose(rgba, near[0], rtol=0.0, atol=1e-6)
+
+
 def test_edge_cases(env):
     s = env.synth
     # early exit with opaque-ish layers, non-zero background, t_min variants
