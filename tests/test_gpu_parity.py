@@ -308,6 +308,17 @@ def test_backward_early_exit_and_errors(env):
         r.close()
 
 
+def test_backward_degenerate_footprints(env):
+    """1x1 and 2x2 textures: all four texels of a footprint coincide (clamped) and whole rows of pixels share one footprint,
+    the extreme case of the run merging in k_shade<BWD>; a 3-texel-wide texture under a 60-pixel object for long runs."""
+    sc = env.synth.make_config(1, width=64, height=40, num_cameras=2, tex_size=16)
+    sc.layers[0].texture = sc.layers[0].texture[:3, :3].copy()
+    sc.layers[1].texture = sc.layers[1].texture[:2, :2].copy()
+    sc.layers[2].texture = sc.layers[2].texture[:1, :1].copy()
+    worst, want = check_backward(env, sc, [0, 1])
+    assert all(np.abs(w).max() > 1e-3 for w in want)
+
+
 def test_determinism_and_chunking(env):
     sc = env.synth.make_config(2, mesh_n=30, width=200, height=150, tex_size=128, num_cameras=6)
     a = gpu_render(env, sc, range(6), views_per_chunk=1)
